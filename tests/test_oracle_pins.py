@@ -1,0 +1,383 @@
+"""Pins for the CPU oracle (oracle/lya_oracle.c): every check here compares the
+oracle with something OTHER than itself -- hand-worked bins, closed forms,
+invariants, textbook/library routines (numpy lstsq, histogram2d), or an
+exhaustive numpy enumeration on tiny inputs.  Names P1..P8 / PD1..PD8 are the
+pin ids of DESIGN.md ("Oracle pins").  CPU only.
+"""
+import os
+from decimal import Decimal, getcontext
+
+import numpy as np
+import pytest
+
+from paper_2507_00129_b200 import gen
+from oracle import oracle as orc
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+# ---------------------------------------------------------------- helpers
+def np_brute_xi(f, pairs, nb=50, rmax=200.0):
+    """Independent exhaustive enumeration with numpy broadcasting + histogram2d."""
+    S = np.zeros((nb, nb)); W = np.zeros((nb, nb)); N = np.zeros((nb, nb), np.int64)
+    n_out = 0
+    edges = np.linspace(0.0, rmax, nb + 1)
+    for p, q in pairs:
+        chord = np.sqrt((f.ux[p] - f.ux[q]) ** 2 + (f.uy[p] - f.uy[q]) ** 2 + (f.uz[p] - f.uz[q]) ** 2)
+        s = chord / 2.0
+        c = np.sqrt(1.0 - s * s)
+        a, b = f.pix_off[p], f.pix_off[p + 1]
+        d, e = f.pix_off[q], f.pix_off[q + 1]
+        ci = f.chi[a:b, None]; cj = f.chi[None, d:e]
+        rpar = (np.abs(ci - cj) * c).ravel(); rperp = ((ci + cj) * s).ravel()
+        ww = (f.w[a:b, None] * f.w[None, d:e]).ravel()
+        dd = ((f.w[a:b] * f.delta[a:b])[:, None] * (f.w[d:e] * f.delta[d:e])[None, :]).ravel()
+        ok = (rpar < rmax) & (rperp < rmax)
+        n_out += int((~ok).sum())
+        N += np.histogram2d(rpar[ok], rperp[ok], bins=[edges, edges])[0].astype(np.int64)
+        W += np.histogram2d(rpar[ok], rperp[ok], bins=[edges, edges], weights=ww[ok])[0]
+        S += np.histogram2d(rpar[ok], rperp[ok], bins=[edges, edges], weights=dd[ok])[0]
+    return S.ravel(), W.ravel(), N.ravel(), n_out
+
+
+@pytest.fixture(scope="module")
+def xi0(cfg0):
+    pq = orc.pairs_all(cfg0.n_forest)
+    return pq, orc.xi(cfg0, pq)
+
+
+# ---------------------------------------------------------------- P6
+def test_P6_hand_built_bins():
+    """tests/golden/p6_hand_cases.txt: bins derived by hand (R-1, R-2, R-3, R-5)."""
+    getcontext().prec = 50
+    rows = [l.split("#")[0].split() for l in open(os.path.join(HERE, "golden", "p6_hand_cases.txt"))
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) >= 10
+    b = orc.binning()
+    for s_txt, ci, cj, ebpar, ebperp, eA in rows:
+        s = float(s_txt)
+        uq = (1.0 - 2.0 * s * s, 2.0 * s * float(Decimal(1 - Decimal(s_txt) ** 2).sqrt()), 0.0)
+        f = gen.two_forests([float(ci)], [float(cj)], (1.0, 0.0, 0.0), uq)
+        so, co = orc.pair_sc(f, 0, 1)
+        assert abs(so - s) < 1e-15 and abs(co - float(Decimal(1 - Decimal(s_txt) ** 2).sqrt())) < 1e-15
+        A = orc.pix_bin(b, so, co, float(ci), float(cj))
+        assert A == int(eA), (s_txt, ci, cj, A, eA)
+        r = orc.xi(f, [[0, 1]])
+        if int(eA) >= 0:
+            assert r["N"].sum() == 1 and r["N"][int(eA)] == 1 and r["n_out"] == 0
+            assert int(eA) == 50 * int(ebpar) + int(ebperp)
+        else:
+            assert r["N"].sum() == 0 and r["n_out"] == 1
+
+
+def test_P6_chord_is_sin_half_theta():
+    """s from the chord equals sin(theta/2) computed from RA/Dec by the haversine formula."""
+    f = gen.make_config(0)
+    for p, q in [(0, 1), (3, 40), (10, 63)]:
+        s, c = orc.pair_sc(f, p, q)
+        hav = np.sin((f.dec[p] - f.dec[q]) / 2) ** 2 + np.cos(f.dec[p]) * np.cos(f.dec[q]) * np.sin((f.ra[p] - f.ra[q]) / 2) ** 2
+        assert abs(s - np.sqrt(hav)) < 1e-14
+        assert abs(s * s + c * c - 1.0) < 1e-15
+
+
+# ---------------------------------------------------------------- P2
+def test_P2_exhaustive_enumeration(cfg0, xi0):
+    pq, r = xi0
+    S, W, N, n_out = np_brute_xi(cfg0, pq)
+    assert np.array_equal(r["N"].astype(np.int64), N)
+    assert r["n_out"] == n_out
+    n = np.diff(cfg0.pix_off)
+    assert int(r["N"].sum()) + r["n_out"] == int(sum(n[p] * n[q] for p, q in pq))
+    assert np.allclose(r["W"], W, rtol=1e-12, atol=0)
+    assert np.all(np.abs(r["S"] - S) <= 1e-12 * r["Sabs"] + 1e-300)
+    nz = r["W"] > 0
+    assert np.allclose(r["xi"][nz], (S[nz] / W[nz]), rtol=0, atol=1e-12)
+    assert np.all(r["xi"][~nz] == 0.0)
+
+
+def test_P2_ragged_forests_and_generic_binning():
+    """Ragged lengths (config-1 recipe) and a non-power-of-two bin width."""
+    f = gen.make_config(1, n_forest=60)
+    pq = orc.pairs_all(f.n_forest)
+    b = orc.binning(150.0, 90.0, 30, 30)
+    r = orc.xi(f, pq, b)
+    # numpy enumeration with explicit (int)(r * (n/rmax)) binning
+    N = np.zeros(900, np.int64)
+    for p, q in pq:
+        s, c = orc.pair_sc(f, p, q)
+        ci = f.chi[f.pix_off[p]:f.pix_off[p + 1], None]; cj = f.chi[None, f.pix_off[q]:f.pix_off[q + 1]]
+        rpar = np.abs(ci - cj) * c; rperp = (ci + cj) * s
+        ok = (rpar < 150.0) & (rperp < 90.0)
+        A = 30 * np.minimum((rpar * (30 / 150.0)).astype(np.int64), 29) + np.minimum((rperp * (30 / 90.0)).astype(np.int64), 29)
+        N += np.bincount(A[ok], minlength=900)
+    assert np.array_equal(r["N"].astype(np.int64), N)
+
+
+# ---------------------------------------------------------------- P1
+def test_P1_neighbour_list_equals_all_pairs(cfg0, xi0):
+    pq_all, r_all = xi0
+    pq_nb = orc.pairs_brute(cfg0)
+    assert len(pq_nb) < len(pq_all)
+    r_nb = orc.xi(cfg0, pq_nb)
+    assert np.array_equal(r_all["N"], r_nb["N"])
+    assert np.allclose(r_all["S"], r_nb["S"], rtol=0, atol=1e-12 * r_all["Sabs"].max())
+    assert np.allclose(r_all["W"], r_nb["W"], rtol=1e-13)
+    # a non-listed pair has no in-grid pixel pair (R-14)
+    listed = set(map(tuple, pq_nb.tolist()))
+    rest = np.array([x for x in pq_all.tolist() if tuple(x) not in listed], np.int32)
+    assert orc.xi(cfg0, rest)["N"].sum() == 0
+
+
+def test_P1_window_prefilter_equals_brute():
+    f = gen.make_config(1, n_forest=1500)
+    a = orc.pairs_brute(f); b = orc.pairs_window(f)
+    assert np.array_equal(a, b)
+    assert len(a) > 0 and np.all(a[:, 0] < a[:, 1])
+    # criterion re-evaluated with numpy for every p<q
+    s = 0.5 * np.sqrt((f.ux[:, None] - f.ux[None]) ** 2 + (f.uy[:, None] - f.uy[None]) ** 2 + (f.uz[:, None] - f.uz[None]) ** 2)
+    cm = f.chi[f.pix_off[:-1]]
+    listed = np.triu(((cm[:, None] + cm[None]) * s) < 200.0, 1)
+    assert listed.sum() == len(a)
+    assert listed[a[:, 0], a[:, 1]].all()
+
+
+# ---------------------------------------------------------------- P3, P4
+@pytest.mark.parametrize("k", [1.0, -0.5])
+def test_P3_constant_delta(cfg0, k):
+    f = gen.make_config(0); f.delta[:] = k
+    r = orc.xi(f, orc.pairs_brute(f))
+    nz = r["N"] > 0
+    assert nz.sum() > 100
+    assert np.allclose(r["xi"][nz], k * k, rtol=1e-13)
+    assert np.allclose(r["S"][nz], k * k * r["W"][nz], rtol=1e-13)
+
+
+def test_P4_unit_weights_W_equals_N(cfg0):
+    f = gen.make_config(0); f.w[:] = 1.0
+    r = orc.xi(f, orc.pairs_brute(f))
+    assert np.array_equal(r["W"], r["N"].astype(np.float64))
+    assert np.array_equal(r["Q"], r["N"].astype(np.float64))
+
+
+# ---------------------------------------------------------------- P5
+def test_P5_independent_gaussian_consistent_with_zero():
+    """Var S_A = sigma^4 Q_A exactly for iid deltas: z_A = S_A/(sigma^2 sqrt Q_A) ~ N(0,1)."""
+    f = gen.make_config(1, n_forest=600)
+    r = orc.xi(f, orc.pairs_window(f))
+    nz = r["N"] > 50
+    assert nz.sum() > 2000
+    z = r["S"][nz] / (0.2 ** 2 * np.sqrt(r["Q"][nz]))
+    assert abs(z.mean()) < 3.0 / np.sqrt(nz.sum())
+    assert abs((z ** 2).mean() - 1.0) < 0.1
+
+
+# ---------------------------------------------------------------- P7, P8
+def test_P7_order_independence(cfg0):
+    pq = orc.pairs_brute(cfg0)
+    r0 = orc.xi(cfg0, pq)
+    rng = np.random.default_rng(5)
+    r1 = orc.xi(cfg0, pq[rng.permutation(len(pq))])
+    r2 = orc.xi(cfg0, pq[:, ::-1])                    # swap p <-> q
+    perm = rng.permutation(cfg0.n_forest)            # relabel forests
+    fp = cfg0.subset(perm)
+    inv = np.empty_like(perm); inv[perm] = np.arange(len(perm))
+    r3 = orc.xi(fp, inv[pq])
+    for r in (r1, r2, r3):
+        assert np.array_equal(r0["N"], r["N"])
+        assert np.allclose(r0["W"], r["W"], rtol=1e-13)
+        assert np.all(np.abs(r0["S"] - r["S"]) <= 1e-13 * r0["Sabs"])
+
+
+def test_P8_degenerate_catalogues():
+    f = gen.make_config(0)
+    one = f.subset([3])
+    assert len(orc.pairs_brute(one)) == 0 and len(orc.pairs_window(one)) == 0
+    r = orc.xi(one, np.zeros((0, 2), np.int32))
+    assert r["N"].sum() == 0 and r["S"].sum() == 0 and np.all(r["xi"] == 0)
+    # two forests 90 degrees apart: not listed, and no pixel pair in the grid
+    far = gen.two_forests(f.chi[:24], f.chi[24:48], (1, 0, 0), (0, 1, 0))
+    assert len(orc.pairs_brute(far)) == 0
+    assert orc.xi(far, [[0, 1]])["N"].sum() == 0
+
+
+# ---------------------------------------------------------------- PD1, PD2
+def _forest(cfg0, p):
+    a, b = cfg0.pix_off[p], cfg0.pix_off[p + 1]
+    return cfg0.w[a:b], cfg0.loglam[a:b]
+
+
+def test_PD1_eta_is_wls_residual_maker(cfg0):
+    """eq. 2.7 == I - X (X^T W X)^-1 X^T W, X = [1, log lambda] (PAPER.md:89 continuum model)."""
+    rng = np.random.default_rng(1)
+    for p in (0, 7, 31):
+        w, ll = _forest(cfg0, p)
+        eta = orc.eta(w, ll)
+        y = rng.normal(size=len(w))
+        X = np.stack([np.ones_like(ll), ll - ll.mean()], 1)     # centred for conditioning only
+        sw = np.sqrt(w)
+        coef = np.linalg.lstsq(X * sw[:, None], y * sw, rcond=None)[0]
+        assert np.allclose(eta @ y, y - X @ coef, rtol=0, atol=1e-10)
+
+
+def test_PD2_projector_identities(cfg0):
+    f1 = gen.make_config(1, n_forest=40)
+    for f, p in ((cfg0, 0), (cfg0, 50), (f1, 3), (f1, 17)):
+        w, ll = _forest(f, p)
+        n = len(w)
+        eta = orc.eta(w, ll)
+        lbar = (w * ll).sum() / w.sum()
+        u = ll - lbar
+        assert np.abs(eta @ np.ones(n)).max() < 1e-11          # annihilates constants
+        assert np.abs(eta @ ll).max() < 1e-10                  # annihilates log-lambda-linear
+        assert np.abs(w @ eta).max() < 1e-10                   # w^T eta = 0
+        assert np.abs((w * u) @ eta).max() < 1e-10
+        assert np.abs(eta @ eta - eta).max() < 1e-10           # idempotent
+        assert abs(np.trace(eta) - (n - 2)) < 1e-10
+        assert np.abs(eta.sum(1)).max() < 1e-11                # rows of the projector sum to zero
+
+
+def test_PD2_degenerate_forest_rejected():
+    with pytest.raises(ValueError):
+        orc.eta(np.ones(3), np.full(3, 3.6))                   # a single distinct lambda: V = 0
+    with pytest.raises(ValueError):
+        orc.eta(np.zeros(3), np.array([3.6, 3.601, 3.602]))    # sum w = 0
+
+
+# ---------------------------------------------------------------- PD3..PD8
+@pytest.fixture(scope="module")
+def d0(cfg0):
+    pq = orc.pairs_brute(cfg0)
+    return pq, orc.dmat(cfg0, pq, 0.0, gen.mask_seed(0))
+
+
+def test_PD3_row_sums_with_overflow_bucket(d0):
+    pq, d = d0
+    scale = np.abs(d["Dn"]).sum(1) + np.abs(d["Dover"])
+    assert np.all(np.abs(d["Dn"].sum(1) + d["Dover"]) <= 1e-11 * scale + 1e-300)
+
+
+def test_PD4_collapsed_equals_naive(cfg0, d0):
+    pq, d = d0
+    dc = orc.dmat(cfg0, pq, 0.0, gen.mask_seed(0), collapsed=True)
+    assert dc["n_kept"] == d["n_kept"]
+    assert np.allclose(dc["Wd"], d["Wd"], rtol=1e-14)
+    assert np.abs(dc["Dn"] - d["Dn"]).max() <= 1e-12 * np.abs(d["Dn"]).max()
+    # and with a mask, on ragged forests
+    f = gen.make_config(1, n_forest=80)
+    pq1 = orc.pairs_window(f)
+    a = orc.dmat(f, pq1, 0.9, 77); b = orc.dmat(f, pq1, 0.9, 77, collapsed=True)
+    assert a["n_kept"] == b["n_kept"] and a["n_kept"] > 0
+    assert np.abs(a["Dn"] - b["Dn"]).max() <= 1e-12 * np.abs(a["Dn"]).max()
+
+
+def test_PD4_tiny_python_quadruple_sum():
+    """Two forests of 5 and 6 pixels: D from a literal Python 4-fold loop with numpy-built eta."""
+    f = gen.make_config(0).subset([0, 1])
+    keep_p = np.r_[0:5]; keep_q = np.r_[24:30]
+    f = gen.two_forests(f.chi[keep_p], f.chi[keep_q], (f.ux[0], f.uy[0], f.uz[0]), (f.ux[1], f.uy[1], f.uz[1]),
+                        f.w[keep_p], f.w[keep_q], f.delta[keep_p], f.delta[keep_q], f.loglam[keep_p], f.loglam[keep_q])
+    s, c = orc.pair_sc(f, 0, 1)
+    b = orc.binning()
+
+    def eta_np(w, ll):
+        n = len(w); lbar = (w * ll).sum() / w.sum(); u = ll - lbar
+        return np.eye(n) - np.outer(np.ones(n), w) / w.sum() - np.outer(u, w * u) / (w * u * u).sum()
+    ep = eta_np(f.w[:5], f.loglam[:5]); eq = eta_np(f.w[5:], f.loglam[5:])
+    Dn = np.zeros((2500, 2500)); Wd = np.zeros(2500)
+    for i in range(5):
+        for j in range(6):
+            A = orc.pix_bin(b, s, c, f.chi[i], f.chi[5 + j])
+            if A < 0:
+                continue
+            om = f.w[i] * f.w[5 + j]; Wd[A] += om
+            for i2 in range(5):
+                for j2 in range(6):
+                    B = orc.pix_bin(b, s, c, f.chi[i2], f.chi[5 + j2])
+                    if B >= 0:
+                        Dn[A, B] += om * ep[i, i2] * eq[j, j2]
+    d = orc.dmat(f, [[0, 1]], 0.0, 0)
+    assert Wd.sum() > 0
+    assert np.allclose(d["Wd"], Wd, rtol=1e-14)
+    assert np.abs(d["Dn"] - Dn).max() <= 1e-12 * np.abs(Dn).max()
+
+
+def test_PD5_two_pixel_forests_have_zero_eta():
+    f = gen.make_config(0)
+    idx = np.concatenate([np.arange(f.pix_off[p], f.pix_off[p] + 2) for p in range(f.n_forest)])
+    g = gen.Forests(f.ra, f.dec, f.ux, f.uy, f.uz, f.zq, np.arange(0, 2 * f.n_forest + 1, 2, dtype=np.int64),
+                    f.chi[idx], f.w[idx], f.delta[idx], f.loglam[idx])
+    assert np.abs(orc.eta(g.w[:2], g.loglam[:2])).max() < 1e-12
+    pq = orc.pairs_brute(g)
+    d = orc.dmat(g, pq, 0.0, 0)
+    x = orc.xi(g, pq)
+    assert np.abs(d["Dn"]).max() <= 1e-9 * d["Wd"].max()
+    assert np.allclose(d["Wd"], x["W"], rtol=1e-13)
+
+
+def test_PD6_no_rejection_matches_xi(cfg0, d0, xi0):
+    pq, d = d0
+    x = orc.xi(cfg0, pq)
+    assert d["n_kept"] == int(x["N"].sum())
+    assert np.allclose(d["Wd"], x["W"], rtol=1e-12)
+
+
+def test_PD7_mask_statistics_and_symmetry():
+    thr = orc.mask_threshold(0.99)
+    assert thr == round(0.99 * 2 ** 32)
+    assert orc.mask_threshold(0.0) == 0 and orc.mask_threshold(1.0) == 2 ** 32
+    n = 400
+    kept = np.array([[orc.keep(12345, i, 1000 + j, thr) for j in range(n)] for i in range(n)])
+    tot = n * n
+    assert abs(kept.mean() - 0.01) < 4 * np.sqrt(0.01 * 0.99 / tot)
+    assert orc.keep(12345, 5, 1007, thr) == orc.keep(12345, 1007, 5, thr)
+    assert all(orc.keep(1, i, i + 1, 0) for i in range(50))                  # f = 0 keeps all
+    assert not any(orc.keep(1, i, i + 1, 2 ** 32) for i in range(50))        # f = 1 keeps none
+    # no visible structure: rows / columns / diagonals all at the nominal rate (f = 0.5 for power)
+    thr5 = orc.mask_threshold(0.5)
+    k5 = np.array([[orc.keep(999, i, 5000 + j, thr5) for j in range(n)] for i in range(n)], float)
+    for v in (k5.mean(0), k5.mean(1)):
+        chi2 = (((v - 0.5) ** 2) / (0.25 / n)).sum()
+        assert abs(chi2 - n) < 5 * np.sqrt(2 * n)
+    # 2x2 minors: keep(i,j) keep(i,j') keep(i',j) keep(i',j') independent -> product mean = 1/16
+    m = (k5[:-1, :-1] * k5[:-1, 1:] * k5[1:, :-1] * k5[1:, 1:]).mean()
+    assert abs(m - 1 / 16) < 5 * np.sqrt((1 / 16) * (15 / 16) / ((n - 1) ** 2)) * 2
+    # a different seed gives a different, equally dense mask
+    k6 = np.array([[orc.keep(1000, i, 5000 + j, thr5) for j in range(100)] for i in range(100)], float)
+    assert abs((k6 == k5[:100, :100]).mean() - 0.5) < 0.03
+
+
+def test_PD7_kept_fraction_in_dmat(cfg0):
+    pq = orc.pairs_brute(cfg0)
+    x = orc.xi(cfg0, pq)
+    tot = int(x["N"].sum())
+    d = orc.dmat(cfg0, pq, 0.9, gen.mask_seed(3))
+    assert abs(d["n_kept"] / tot - 0.1) < 4 * np.sqrt(0.1 * 0.9 / tot)
+    # kept fraction per bin shows no structure (chi^2 over well-filled bins)
+    Nk = np.zeros(2500)
+    thr = orc.mask_threshold(0.9)
+    b = orc.binning()
+    for p, q in pq[:300]:
+        s, c = orc.pair_sc(cfg0, p, q)
+        for i in range(cfg0.pix_off[p], cfg0.pix_off[p + 1]):
+            for j in range(cfg0.pix_off[q], cfg0.pix_off[q + 1]):
+                A = orc.pix_bin(b, s, c, cfg0.chi[i], cfg0.chi[j])
+                if A >= 0 and orc.keep(gen.mask_seed(3), i, j, thr):
+                    Nk[A] += 1
+    x300 = orc.xi(cfg0, pq[:300])["N"].astype(float)
+    sel = x300 >= 50
+    chi2 = (((Nk[sel] - 0.1 * x300[sel]) ** 2) / (0.09 * x300[sel])).sum()
+    assert abs(chi2 - sel.sum()) < 5 * np.sqrt(2 * sel.sum())
+
+
+def test_PD8_normalisation_sanity(cfg0, d0):
+    pq, d = d0
+    D = d["D"]; nz = d["Wd"] > 0
+    diag = np.diag(D)[nz]
+    assert np.all(diag > 0.5) and np.all(diag < 1.0)             # 1 - O(1/n), n = 24
+    off = D[nz][:, nz] - np.diag(diag)
+    assert np.abs(off).max() < 0.5 and np.all(np.abs(off).max(1) < diag)   # diagonally dominant
+    # large-grid variant: nothing is out of the grid, so rows of Dn sum to zero with no bucket
+    big = orc.binning(8192.0, 8192.0, 16, 16)
+    db = orc.dmat(cfg0, pq[:400], 0.0, 0, b=big)
+    assert np.abs(db["Dover"]).max() == 0.0
+    assert np.all(np.abs(db["Dn"].sum(1)) <= 1e-11 * np.abs(db["Dn"]).sum(1) + 1e-300)
