@@ -1,0 +1,185 @@
+/*
+ * lya.h -- C-ABI of liblya.so: the B200 (sm_100a) pixel-pair hot path of the
+ * Lya2pcf method (arxiv 2507.00129; citations are /root/reference/PAPER.md lines).
+ *
+ *   lya_neighbours  forest pairs closer than the maximum transverse separation
+ *                   ("only takes forests within a pre-ordered
+ *                   neighborhood defined by this maximum distance")
+ *   lya_xi2pcf      eq. 2.4: S_A = sum w_i d_i w_j d_j,
+ *                   W_A = sum w_i w_j, N_A = pair count, xi_A = S_A / W_A over
+ *                   pixel pairs of DIFFERENT forests on the (r_par, r_perp) grid
+ *   lya_dmat        eqs. 2.6-2.7: the distortion matrix
+ *                   D_AB = W_A^-1 sum_{(i,j) in A} w_i w_j sum_{(i',j') in B}
+ *                   eta_ii' eta_jj', with a seeded pixel-pair keep mask
+ *
+ * Conventions
+ *   - Plain C, no C++/torch types.  Unless a parameter says "host", every
+ *     pointer is a DEVICE pointer on the ctx's device, caller-owned; inputs are
+ *     never modified or freed; outputs are caller-allocated and OVERWRITTEN.
+ *   - Work is enqueued on the ctx stream; device outputs are valid once the
+ *     caller has synchronised that stream (calls that return host values
+ *     synchronise internally and say so).
+ *   - Every call returns a status and never throws, prints or exits.  On error,
+ *     outputs are unspecified and lya_last_error(ctx) holds a message.
+ *   - One ctx per host thread.  There is no CPU fallback: without a CUDA device
+ *     lya_create fails with LYA_ERR_CUDA.
+ *
+ * Geometry (readings G1-G6; the paper gives no formulas at this level):
+ *   forest pair: s = 0.5*sqrt(|u_p - u_q|^2) = sin(theta/2), c = sqrt(1 - s*s)
+ *   pixel pair:  r_par = |chi_i - chi_j| * c,   r_perp = (chi_i + chi_j) * s
+ *   in grid iff r_par < rpar_max and r_perp < rperp_max;
+ *   b = (int)(r * (n / r_max)) clamped to n-1;  A = n_perp * b_par + b_perp.
+ *   All of it in IEEE binary64, each operation rounded separately (no FMA), so
+ *   that bins -- hence pair counts -- are bit-identical to the CPU oracle.
+ */
+#ifndef LYA_H
+#define LYA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lya_ctx lya_ctx;      /* opaque: device, stream, scratch, last error */
+typedef struct lya_pairs lya_pairs;  /* opaque, library-owned device forest-pair list */
+
+typedef enum {
+    LYA_OK = 0,
+    LYA_ERR_INVALID_ARG = 1,        /* NULL/negative sizes/inconsistent offsets/non-finite input */
+    LYA_ERR_UNSORTED = 2,           /* chi not strictly increasing inside a forest */
+    LYA_ERR_DEGENERATE_FOREST = 3,  /* lya_dmat: a forest with sum w == 0 or sum w (L-Lbar)^2 == 0 */
+    LYA_ERR_CAPACITY = 4,           /* a size exceeds what the library supports (see each call) */
+    LYA_ERR_OOM = 5,                /* device allocation failed */
+    LYA_ERR_CUDA = 6,               /* any other CUDA runtime error (message in lya_last_error) */
+    LYA_ERR_UNIMPLEMENTED = 7
+} lya_status;
+
+/* Forest catalogue, CSR over pixels (a skewer = sky position + a
+ * variable-length table of delta, weight, wavelength).
+ *   ux,uy,uz: unit vectors of the sightlines.  They are INPUTS (like chi) so that
+ *     both this library and a checker consume identical values; pass NULL for all
+ *     three to have them derived on the device from ra/dec (not bit-reproducible
+ *     against a host libm).  ra/dec [radians] may be NULL when ux,uy,uz are given.
+ *   pix_off: [n_forest+1], pix_off[0] = 0, non-decreasing, pix_off[n_forest] = n_pix.
+ *   chi [Mpc/h]: comoving distance of each pixel, strictly increasing inside a
+ *     forest, 0 <= chi < 1e6.   w >= 0.   loglam = log(lambda) in any base
+ *     (eq. 2.7 is invariant under affine maps of it); only lya_dmat reads it,
+ *     it may be NULL for lya_neighbours / lya_xi2pcf.
+ *   n_forest < 2^31, n_pix < 2^40. */
+typedef struct {
+    int64_t n_forest, n_pix;
+    const double *ra, *dec;
+    const double *ux, *uy, *uz;
+    const int64_t *pix_off;
+    const double *chi, *w, *delta, *loglam;
+} lya_forests;
+
+/* (r_par, r_perp) grid (4 Mpc/h bins up to 200 Mpc/h -> 50 x 50).
+ * Requires 0 < r*_max, 1 <= n_* and n_par*n_perp <= 4096, bin width >= 0.01. */
+typedef struct {
+    double rpar_max, rperp_max;
+    int32_t n_par, n_perp;
+} lya_binning;
+
+/* Counters filled by the compute calls (host struct; valid after the call
+ * returns -- the calls that take it synchronise the ctx stream). */
+typedef struct {
+    uint64_t n_forest_pairs;   /* forest pairs traversed */
+    uint64_t n_visited;        /* sum over traversed forest pairs of n_p * n_q */
+    uint64_t n_evaluated;      /* pixel pairs whose separation was actually computed */
+    uint64_t n_binned;         /* pixel pairs inside the grid (= sum_A N_A) */
+    uint64_t n_kept;           /* lya_dmat: in-grid pixel pairs that passed the keep mask */
+    float    ms_main;          /* device time of the dominant kernel (CUDA events on the ctx stream) */
+    float    ms_total;         /* device time of the whole call */
+} lya_stats;
+
+/* ---- context ------------------------------------------------------------------ */
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t (e.g. torch's current
+ * stream) or NULL for the legacy default stream. */
+lya_status  lya_create(lya_ctx **ctx, int device, void *cuda_stream);
+void        lya_destroy(lya_ctx *ctx);
+const char *lya_last_error(const lya_ctx *ctx);   /* host string, owned by ctx */
+const char *lya_version(void);
+
+/* ---- stage 1: neighbour search (north_star stage 1) ------------ */
+/* Lists every unordered pair of distinct non-empty forests {p<q} with
+ *   (chi_p[0] + chi_q[0]) * s_pq < rperp_max            (reading G4)
+ * i.e. theta below the angle that gives r_perp = rperp_max at the pair's minimum
+ * comoving distances.  Any pair with at least one in-grid pixel pair is listed.
+ * Method: uniform 3-D cell grid over the unit vectors (cell edge >= the largest
+ * admissible chord), counting sort by cell, count -> exclusive scan -> fill.
+ * The list is a set (order unspecified but deterministic); entries have p < q.
+ * *out is library-owned (free with lya_pairs_free).  n_pairs: host out.
+ * Synchronises the ctx stream.  LYA_ERR_CAPACITY if n_pairs >= 2^40. */
+lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
+                          lya_pairs **out, int64_t *n_pairs);
+/* Copies the list to pq, device int32 [n_pairs][2] (p, q). */
+lya_status lya_pairs_export(lya_ctx *ctx, const lya_pairs *pairs, int32_t *pq);
+/* Builds a list from caller pairs (device int32 [n_pairs][2]); entries must be
+ * distinct forests, either order; no criterion is applied (tests, sharding). */
+lya_status lya_pairs_import(lya_ctx *ctx, const int32_t *pq, int64_t n_pairs, lya_pairs **out);
+int64_t    lya_pairs_count(const lya_pairs *pairs);
+void       lya_pairs_free(lya_ctx *ctx, lya_pairs *pairs);
+
+/* ---- stage 2: pair kernel, eq. 2.4 ------------------------------ */
+/* S, W: double [n_par*n_perp]; N: uint64 [n_par*n_perp]; xi: double [n_par*n_perp]
+ * (xi_A = S_A / W_A, 0 where W_A == 0); row-major [b_par][b_perp].  Any of S, W,
+ * N, xi may be NULL.  Each unordered pixel pair of each listed forest pair counts
+ * once.  stats: host out, may be NULL (when non-NULL the call synchronises). */
+lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
+                      const lya_pairs *pairs,
+                      double *S, double *W, uint64_t *N, double *xi, lya_stats *stats);
+
+/* ---- stages 3+4: distortion matrix, eqs. 2.6-2.7 ----------------- */
+/* eta_ii' = delta^K_ii' - w_i'/sum_k w_k - (L_i-Lbar) w_i' (L_i'-Lbar) / sum_k w_k (L_k-Lbar)^2
+ * inside a forest (0 across forests), L = loglam, Lbar the w-weighted mean (R-10).
+ * For every listed forest pair and every in-grid pixel pair (i,j) that passes the
+ * keep mask (A = its bin, om = w_i w_j):
+ *     Wd[A] += om;   Dn[A][B] += om * sum_{(i',j') in B} eta_ii' eta_jj'
+ * over i' in the forest of i and j' in the forest of j ((i',j') outside the grid
+ * are dropped; the inner sum is never masked, reading R-8).  D[A][B] = Dn[A][B]/Wd[A]
+ * (row 0 where Wd[A] == 0).
+ * Keep mask (stage 4): a pure-integer hash of (seed, the two
+ * pixels' offsets in the flat arrays, smaller first); keep iff its top 32 bits
+ * >= round(reject_fraction * 2^32).  reject_fraction in [0,1]; 0 keeps all.
+ * D: double [NB*NB] row-major [A][B], NB = n_par*n_perp (NULL to skip the final
+ * division); Dn: double [NB*NB] un-normalised sums (may be NULL if D is given; at
+ * least one of D, Dn); Wd: double [NB] (may be NULL); stats as above (n_kept).
+ * Every forest on the list must be non-degenerate (LYA_ERR_DEGENERATE_FOREST). */
+lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
+                    const lya_pairs *pairs, double reject_fraction, uint64_t seed,
+                    double *D, double *Dn, double *Wd, lya_stats *stats);
+
+/* ---- end-to-end convenience with HOST buffers ------------------------------------- */
+/* Uploads a HOST catalogue (every pointer in *f_host is a host pointer; ux/uy/uz
+ * required), runs lya_neighbours, then lya_xi2pcf when do_xi and lya_dmat when
+ * do_dmat, and downloads the results into HOST arrays (any may be NULL):
+ * S, W, xi [NB] double, N [NB] uint64, D [NB*NB] double, Wd [NB] double.
+ * stats_xi / stats_dmat: host out, may be NULL.  Synchronises. */
+lya_status lya_run_host(lya_ctx *ctx, const lya_forests *f_host, const lya_binning *b,
+                        int do_xi, int do_dmat, double reject_fraction, uint64_t seed,
+                        double *S, double *W, uint64_t *N, double *xi,
+                        double *D, double *Wd,
+                        int64_t *n_pairs, lya_stats *stats_xi, lya_stats *stats_dmat);
+
+/* ---- measured roofline denominators ------------------------ */
+/* Microbenchmarks of the units that bound the pair loops, run on the ctx device.
+ * Each returns operations per second through *rate (host out) and synchronises.
+ *   LYA_PEAK_FP64_FMA     warp-level DFMA instructions x 32 lanes per second
+ *   LYA_PEAK_FP64_ADD     same for DADD
+ *   LYA_PEAK_SMEM_CAS64   lane-level shared-memory fp64 atomic adds (CAS loop) per second,
+ *                         random bins of a 2500-entry histogram
+ *   LYA_PEAK_SMEM_ADD32   lane-level native shared-memory u32 atomic adds per second
+ *   LYA_PEAK_L2_RED64     lane-level red.global.add.f64 per second into an L2-resident
+ *                         2500 x 2500 double matrix (random row, contiguous segment) */
+typedef enum {
+    LYA_PEAK_FP64_FMA = 0, LYA_PEAK_FP64_ADD = 1, LYA_PEAK_SMEM_CAS64 = 2,
+    LYA_PEAK_SMEM_ADD32 = 3, LYA_PEAK_L2_RED64 = 4
+} lya_peak_kind;
+lya_status lya_measure_peak(lya_ctx *ctx, lya_peak_kind kind, double *rate);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LYA_H */

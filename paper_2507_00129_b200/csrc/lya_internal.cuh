@@ -1,0 +1,129 @@
+// lya_internal.cuh -- shared declarations of liblya.so's translation units.
+// (CUDA path only; the CPU oracle under oracle/ shares nothing with this.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include "../../include/lya.h"
+
+#define LYA_CHI_MAX 1.0e6          // inputs must satisfy 0 <= chi < LYA_CHI_MAX
+#define LYA_CHI_SENTINEL 1.0e7     // padding pixels: far outside any grid, still < 2^32 bins
+#define LYA_MAX_BINS 4096
+
+struct lya_ctx {
+    int device;
+    cudaStream_t stream;
+    char err[512];
+    int sm_count;
+    // small persistent device scratch
+    unsigned long long *d_counters;   // [16] work counters / flags
+    int xi_variant;                   // kernel variant selector (env LYA_XI_VARIANT; tuning)
+    int dmat_variant;
+    cudaEvent_t ev[4];
+};
+
+struct lya_pairs {
+    int64_t n;
+    int32_t *pq;       // device [n][2], p < q
+    int max_len_hint;  // 0 = unknown
+};
+
+// device-visible error codes written by validation kernels (atomicMax)
+enum { LYA_DEV_OK = 0, LYA_DEV_BAD_OFFSETS = 1, LYA_DEV_NONFINITE = 2, LYA_DEV_UNSORTED = 3,
+       LYA_DEV_BAD_PAIR = 4, LYA_DEV_DEGENERATE = 5, LYA_DEV_TOO_LONG = 6 };
+
+lya_status lya_fail(lya_ctx *ctx, lya_status st, const char *fmt, ...);
+lya_status lya_cuda_fail(lya_ctx *ctx, cudaError_t e, const char *what);
+lya_status lya_check_binning(lya_ctx *ctx, const lya_binning *b);
+lya_status lya_check_forests_host(lya_ctx *ctx, const lya_forests *f, bool need_u, bool need_delta, bool need_loglam);
+// device-side validation of the catalogue (offsets, finiteness, monotone chi, w >= 0).
+// Returns LYA_OK or the matching error; max forest length through *max_len.  Synchronises.
+lya_status lya_validate_forests(lya_ctx *ctx, const lya_forests *f, bool need_delta, bool need_loglam,
+                                int *max_len);
+
+#define LYA_CUDA(call)                                                          \
+    do {                                                                        \
+        cudaError_t e__ = (call);                                               \
+        if (e__ != cudaSuccess) return lya_cuda_fail(ctx, e__, #call);          \
+    } while (0)
+
+// Binning constants handed to kernels.
+struct BinParams {
+    double rpar_max, rperp_max;
+    double inv_par, inv_perp;     // n / r_max
+    int n_par, n_perp;
+    int pow2;                     // both inverse widths are exact powers of two
+};
+static inline bool lya_is_pow2(double x)
+{
+    int e;
+    return x > 0 && frexp(x, &e) == 0.5;
+}
+static inline BinParams lya_make_binparams(const lya_binning *b)
+{
+    BinParams bp;
+    bp.rpar_max = b->rpar_max; bp.rperp_max = b->rperp_max;
+    bp.n_par = b->n_par; bp.n_perp = b->n_perp;
+    bp.inv_par = (double)b->n_par / b->rpar_max;
+    bp.inv_perp = (double)b->n_perp / b->rperp_max;
+    bp.pow2 = lya_is_pow2(bp.inv_par) && lya_is_pow2(bp.inv_perp) &&
+              bp.inv_par * b->rpar_max == (double)b->n_par && bp.inv_perp * b->rperp_max == (double)b->n_perp;
+    return bp;
+}
+
+#ifdef __CUDACC__
+// ---- geometry, one separately rounded binary64 operation each (readings G2-G6) ----
+// (explicit _rn intrinsics are never contracted into FMAs by nvcc)
+__device__ __forceinline__ void lya_pair_sc(double uxp, double uyp, double uzp,
+                                            double uxq, double uyq, double uzq, double &s, double &c)
+{
+    double dx = __dsub_rn(uxp, uxq), dy = __dsub_rn(uyp, uyq), dz = __dsub_rn(uzp, uzq);
+    double h2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    s = __dmul_rn(0.5, __dsqrt_rn(h2));
+    c = __dsqrt_rn(__dsub_rn(1.0, __dmul_rn(s, s)));
+}
+
+// floor of 0 <= x < 2^32 without a cvt instruction: round-down add of 2^52, low word.
+__device__ __forceinline__ unsigned lya_floor_u32(double x)
+{
+    return (unsigned)__double2loint(__dadd_rd(x, 4503599627370496.0));
+}
+
+// Per-forest-pair constants for binning pixel pairs.
+struct PairBin {
+    double c, s;        // cos, sin of theta/2
+    double cx, sy;      // pow2 path: c*inv_par, s*inv_perp (exact scalings)
+};
+
+// Bin of a pixel pair, -1 outside the grid.  POW2: bin widths are powers of two, so
+// (|d|*c)*inv == |d|*(c*inv) exactly and r < r_max <=> floor(r*inv) < n.
+template <bool POW2>
+__device__ __forceinline__ int lya_pix_bin(const BinParams &bp, const PairBin &g, double chi_i, double chi_j)
+{
+    double d = __dsub_rn(chi_i, chi_j);
+    double t = __dadd_rn(chi_i, chi_j);
+    if (POW2) {
+        unsigned bx = lya_floor_u32(__dmul_rn(fabs(d), g.cx));
+        unsigned by = lya_floor_u32(__dmul_rn(t, g.sy));
+        bool ok = (bx < (unsigned)bp.n_par) & (by < (unsigned)bp.n_perp);
+        return ok ? (int)(bx * (unsigned)bp.n_perp + by) : -1;
+    } else {
+        double rpar = __dmul_rn(fabs(d), g.c);
+        double rperp = __dmul_rn(t, g.s);
+        bool ok = (rpar < bp.rpar_max) & (rperp < bp.rperp_max);
+        unsigned bx = min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1));
+        unsigned by = min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1));
+        return ok ? (int)(bx * (unsigned)bp.n_perp + by) : -1;
+    }
+}
+
+__device__ __forceinline__ PairBin lya_make_pairbin(const BinParams &bp, double s, double c)
+{
+    PairBin g;
+    g.c = c; g.s = s;
+    g.cx = __dmul_rn(c, bp.inv_par);
+    g.sy = __dmul_rn(s, bp.inv_perp);
+    return g;
+}
+#endif

@@ -1,0 +1,331 @@
+// xi2pcf.cu -- stage 2 (lya_xi2pcf): the pair kernel of eq. 2.4.
+//
+//   S_A = sum (w_i d_i)(w_j d_j),  W_A = sum w_i w_j,  N_A = #pairs,  xi_A = S_A / W_A
+// over pixel pairs (i in p, j in q) of the listed forest pairs whose separation
+// r_par = |chi_i - chi_j| c, r_perp = (chi_i + chi_j) s falls in bin A.
+//
+// Design (B200): persistent grid, one WARP per forest pair at a time.
+//   * both forests are staged in shared memory (coalesced 8-byte loads; forest p is
+//     reused across the consecutive pairs of the list that share it);
+//   * lanes own DIAGONALS d = j - i of the (i, j) pixel-pair matrix.  Along a diagonal
+//     r_par is nearly constant and r_perp grows slowly, so consecutive pairs fall in the
+//     same bin: each lane accumulates a RUN (S, W, count) in registers and touches the
+//     histogram only when the bin changes (run-length accumulation);
+//   * only diagonals that can hold an in-grid pair are walked: chi is increasing, so
+//     the in-window j of every row i is a contiguous range found by binary search;
+//   * each lane walks D adjacent diagonals with a sliding register window over q, so a
+//     step costs one new q pixel per lane and one broadcast p pixel per warp;
+//   * runs are flushed into a per-block shared-memory histogram (u32 native atomic for
+//     N, fp64 CAS for S and W -- B200 has no native 64-bit shared atomic add), and the
+//     block histogram goes to global fp64/u64 with red.global once per launch.
+// Geometry is exact binary64, operation by operation (lya_internal.cuh), so N is
+// bit-identical to the oracle for any traversal order.
+#include <stdlib.h>
+#include "lya_internal.cuh"
+
+namespace {
+
+constexpr int XI_WARPS = 8;                 // warps per block
+constexpr int XI_THREADS = XI_WARPS * 32;
+constexpr int TILE = 128;                   // pixels of a forest staged per tile
+constexpr int QPAD = 8;                     // sentinel slots either side of the q tile
+constexpr int CHUNK = 16;                   // forest pairs claimed per atomic
+constexpr unsigned long long WARP_BUDGET = 1ull << 28;   // visited pairs per warp per launch (u32 N safety)
+
+struct XiParams {
+    const int64_t *pix_off;
+    const double *chi, *w, *delta;
+    const double *ux, *uy, *uz;
+    const int32_t *pq;
+    int64_t n_pairs;
+    int64_t n_forest;
+    BinParams bp;
+    double *S, *W;                    // global accumulators [nb]
+    unsigned long long *N;            // [nb]
+    unsigned long long *counters;     // [0] next chunk, [1] visited, [2] evaluated, [3] error flag
+};
+
+struct WarpSmem {
+    double pc[TILE], pa[TILE], pw[TILE];
+    double qc[TILE + 2 * QPAD], qa[TILE + 2 * QPAD], qw[TILE + 2 * QPAD];
+};
+
+__device__ __forceinline__ void flush_run(double *sS, double *sW, unsigned *sN, int bin, double accS, double accW, unsigned cnt)
+{
+    atomicAdd(&sN[bin], cnt);
+    atomicAdd(&sS[bin], accS);
+    atomicAdd(&sW[bin], accW);
+}
+
+// One tile (mp x mq pixels, already staged) of one forest pair, D diagonals per lane.
+template <int D, bool POW2>
+__device__ __forceinline__ void tile_diagonals(const WarpSmem &ws, int mp, int mq, int dlo, int dhi,
+                                               const BinParams &bp, const PairBin &g,
+                                               double *sS, double *sW, unsigned *sN, int lane,
+                                               unsigned long long &evaluated)
+{
+    const double *qc = ws.qc + QPAD, *qa = ws.qa + QPAD, *qw = ws.qw + QPAD;
+    for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
+        const int dl = d0 + lane * D;                       // first diagonal of this lane
+        const int dpass_hi = min(dhi, d0 + 32 * D - 1);
+        int i_begin = max(0, -dpass_hi);
+        int i_end = min(mp, mq - d0);                       // exclusive
+        if (i_end <= i_begin) continue;
+        // round the trip count up to a multiple of D (extra rows hit p padding = sentinel-free
+        // but masked by row validity below)
+        int cur[D]; double accS[D], accW[D]; unsigned cnt[D];
+        double wc[D], wa[D], ww[D];                         // sliding window over q
+#pragma unroll
+        for (int k = 0; k < D; ++k) { cur[k] = -1; accS[k] = 0.0; accW[k] = 0.0; cnt[k] = 0; }
+        // preload window slots 0..D-2 with q[i_begin + dl + k]
+#pragma unroll
+        for (int k = 0; k < D - 1; ++k) {
+            int j = min(max(i_begin + dl + k, -QPAD), mq + QPAD - 1);
+            wc[k] = qc[j]; wa[k] = qa[j]; ww[k] = qw[j];
+        }
+        evaluated += (unsigned long long)(i_end - i_begin) * D;
+        for (int ib = i_begin; ib < i_end; ib += D) {
+#pragma unroll
+            for (int u = 0; u < D; ++u) {
+                const int i = ib + u;
+                if (i < i_end) {                            // warp-uniform
+                    const double pci = ws.pc[i], pai = ws.pa[i], pwi = ws.pw[i];
+                    {   // new q pixel for the last diagonal of the lane goes into slot (u + D - 1) % D
+                        int j = min(max(i + dl + D - 1, -QPAD), mq + QPAD - 1);
+                        wc[(u + D - 1) % D] = qc[j]; wa[(u + D - 1) % D] = qa[j]; ww[(u + D - 1) % D] = qw[j];
+                    }
+#pragma unroll
+                    for (int k = 0; k < D; ++k) {
+                        const int sl = (k + u) % D;         // slot holding q[i + dl + k]
+                        const int bin = lya_pix_bin<POW2>(bp, g, pci, wc[sl]);
+                        if (bin != cur[k]) {
+                            if (cur[k] >= 0) flush_run(sS, sW, sN, cur[k], accS[k], accW[k], cnt[k]);
+                            cur[k] = bin; accS[k] = 0.0; accW[k] = 0.0; cnt[k] = 0;
+                        }
+                        if (bin >= 0) {
+                            accS[k] = fma(pai, wa[sl], accS[k]);
+                            accW[k] = fma(pwi, ww[sl], accW[k]);
+                            cnt[k] += 1;
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < D; ++k)
+            if (cur[k] >= 0) flush_run(sS, sW, sN, cur[k], accS[k], accW[k], cnt[k]);
+    }
+}
+
+template <int D, bool POW2>
+__global__ void __launch_bounds__(XI_THREADS, 2) k_xi(XiParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nb = P.bp.n_par * P.bp.n_perp;
+    double *sS = (double *)smem_raw;
+    double *sW = sS + nb;
+    unsigned *sN = (unsigned *)(sW + nb);
+    WarpSmem *wsm = (WarpSmem *)(smem_raw + (((size_t)nb * 20 + 15) & ~(size_t)15));
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    WarpSmem &ws = wsm[wid];
+
+    for (int k = threadIdx.x; k < nb; k += XI_THREADS) { sS[k] = 0.0; sW[k] = 0.0; sN[k] = 0u; }
+    __syncthreads();
+
+    const BinParams bp = P.bp;
+    unsigned long long visited = 0, evaluated = 0;
+    int cur_p = -1, cur_ip0 = -1;
+    const int64_t n_chunks = (P.n_pairs + CHUNK - 1) / CHUNK;
+    // conservative half-width of the r_par window in chi: |chi_i - chi_j| * c < rpar_max
+    while (visited < WARP_BUDGET) {
+        unsigned long long chunk = 0;
+        if (lane == 0) chunk = atomicAdd(&P.counters[0], 1ull);
+        chunk = __shfl_sync(0xffffffffu, chunk, 0);
+        if ((int64_t)chunk >= n_chunks) break;
+        const int64_t k0 = (int64_t)chunk * CHUNK, k1 = min(k0 + CHUNK, P.n_pairs);
+        for (int64_t k = k0; k < k1; ++k) {
+            const int p = P.pq[2 * k], q = P.pq[2 * k + 1];
+            if ((unsigned)p >= (unsigned)P.n_forest || (unsigned)q >= (unsigned)P.n_forest) {
+                if (lane == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_BAD_PAIR);
+                continue;
+            }
+            const int64_t op = P.pix_off[p], oq = P.pix_off[q];
+            const int np = (int)(P.pix_off[p + 1] - op), nq = (int)(P.pix_off[q + 1] - oq);
+            if (np == 0 || nq == 0) continue;
+            visited += (unsigned long long)np * nq;
+            double s, c;
+            lya_pair_sc(P.ux[p], P.uy[p], P.uz[p], P.ux[q], P.uy[q], P.uz[q], s, c);
+            const PairBin g = lya_make_pairbin(bp, s, c);
+            // chi window: r_par < rpar_max  <=>  |dchi| < rpar_max / c  (margin: conservative superset)
+            const double R = (c > 0.0) ? (bp.rpar_max / c) * (1.0 + 1e-12) + 1e-9 : 1e300;
+
+            for (int ip0 = 0; ip0 < np; ip0 += TILE) {
+                const int mp = min(TILE, np - ip0);
+                if (p != cur_p || ip0 != cur_ip0) {
+                    __syncwarp();
+                    for (int t = lane; t < mp; t += 32) {
+                        double wv = P.w[op + ip0 + t];
+                        ws.pc[t] = P.chi[op + ip0 + t];
+                        ws.pw[t] = wv;
+                        ws.pa[t] = wv * P.delta[op + ip0 + t];
+                    }
+                    cur_p = p; cur_ip0 = ip0;
+                }
+                for (int jq0 = 0; jq0 < nq; jq0 += TILE) {
+                    const int mq = min(TILE, nq - jq0);
+                    __syncwarp();
+                    for (int t = lane; t < mq + 2 * QPAD; t += 32) {
+                        int j = t - QPAD;
+                        bool in = (j >= 0) && (j < mq);
+                        double wv = in ? P.w[oq + jq0 + j] : 0.0;
+                        ws.qc[t] = in ? P.chi[oq + jq0 + j] : LYA_CHI_SENTINEL;
+                        ws.qw[t] = wv;
+                        ws.qa[t] = in ? wv * P.delta[oq + jq0 + j] : 0.0;
+                    }
+                    __syncwarp();
+                    // diagonal range [dlo, dhi] of rows with a non-empty r_par window (exact, from
+                    // per-row binary searches; chi_q is increasing)
+                    int dlo = 1 << 30, dhi = -(1 << 30);
+                    const double *qc = ws.qc + QPAD;
+                    for (int i = lane; i < mp; i += 32) {
+                        const double x = ws.pc[i];
+                        int lo = 0, hi = mq;                 // first j with qc[j] > x - R
+                        while (lo < hi) { int mid = (lo + hi) >> 1; if (qc[mid] > x - R) hi = mid; else lo = mid + 1; }
+                        int jlo = lo;
+                        lo = jlo; hi = mq;                   // first j with qc[j] >= x + R
+                        while (lo < hi) { int mid = (lo + hi) >> 1; if (qc[mid] >= x + R) hi = mid; else lo = mid + 1; }
+                        int jhi = lo;
+                        if (jhi > jlo) { dlo = min(dlo, jlo - i); dhi = max(dhi, jhi - 1 - i); }
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        dlo = min(dlo, __shfl_xor_sync(0xffffffffu, dlo, o));
+                        dhi = max(dhi, __shfl_xor_sync(0xffffffffu, dhi, o));
+                    }
+                    if (dhi >= dlo)
+                        tile_diagonals<D, POW2>(ws, mp, mq, dlo, dhi, bp, g, sS, sW, sN, lane, evaluated);
+                }
+            }
+        }
+    }
+    // warp counters
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
+    if (lane == 0) {
+        atomicAdd(&P.counters[1], visited);
+        atomicAdd(&P.counters[2], evaluated);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nb; k += XI_THREADS) {
+        unsigned n = sN[k];
+        if (n) {
+            atomicAdd(&P.N[k], (unsigned long long)n);
+            atomicAdd(&P.S[k], sS[k]);
+            atomicAdd(&P.W[k], sW[k]);
+        }
+    }
+}
+
+__global__ void k_xi_finalize(const double *S, const double *W, const unsigned long long *N, int nb,
+                              double *S_out, double *W_out, unsigned long long *N_out, double *xi_out)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nb) return;
+    double s = S[k], w = W[k];
+    if (S_out) S_out[k] = s;
+    if (W_out) W_out[k] = w;
+    if (N_out) N_out[k] = N[k];
+    if (xi_out) xi_out[k] = (w != 0.0) ? s / w : 0.0;
+}
+
+template <int D>
+cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
+{
+    cudaError_t e;
+    if (P.bp.pow2) {
+        e = cudaFuncSetAttribute(k_xi<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_xi<D, true><<<grid, XI_THREADS, smem, s>>>(P);
+    } else {
+        e = cudaFuncSetAttribute(k_xi<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_xi<D, false><<<grid, XI_THREADS, smem, s>>>(P);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                                 double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (!pairs) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf: pairs is NULL");
+    lya_status st = lya_check_binning(ctx, b);
+    if (st) return st;
+    st = lya_check_forests_host(ctx, f, true, true, false);
+    if (st) return st;
+    if (f->n_forest > 0 && !(f->ux && f->uy && f->uz))
+        return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf needs ux,uy,uz (device); derive them once with the catalogue");
+    LYA_CUDA(cudaSetDevice(ctx->device));
+    st = lya_validate_forests(ctx, f, true, false, NULL);
+    if (st) return st;
+
+    const int nb = b->n_par * b->n_perp;
+    cudaStream_t s = ctx->stream;
+    double *acc = NULL;                         // [S | W | N] accumulators
+    LYA_CUDA(cudaMalloc(&acc, (size_t)nb * 24));
+    cudaMemsetAsync(acc, 0, (size_t)nb * 24, s);
+    cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
+
+    XiParams P;
+    P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.delta = f->delta;
+    P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
+    P.pq = pairs->pq; P.n_pairs = pairs->n; P.n_forest = f->n_forest;
+    P.bp = lya_make_binparams(b);
+    P.S = acc; P.W = acc + nb; P.N = (unsigned long long *)(acc + 2 * nb);
+    P.counters = ctx->d_counters;
+
+    const size_t smem = (((size_t)nb * 20 + 15) & ~(size_t)15) + sizeof(WarpSmem) * XI_WARPS;
+    const int grid = ctx->sm_count * 2;
+    const int64_t n_chunks = (pairs->n + CHUNK - 1) / CHUNK;
+    cudaEventRecord(ctx->ev[0], s);
+    int launches = 0;
+    unsigned long long h[4] = {0, 0, 0, 0};
+    while (pairs->n > 0) {
+        cudaError_t e;
+        switch (ctx->xi_variant) {
+        case 1: e = launch_xi<1>(P, grid, smem, s); break;
+        case 4: e = launch_xi<4>(P, grid, smem, s); break;
+        default: e = launch_xi<2>(P, grid, smem, s); break;
+        }
+        if (e != cudaSuccess) { cudaFree(acc); return lya_cuda_fail(ctx, e, "k_xi launch"); }
+        ++launches;
+        e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) { cudaFree(acc); return lya_cuda_fail(ctx, e, "k_xi"); }
+        if ((int64_t)h[0] >= n_chunks) break;      // every chunk claimed (warps stop at their u32 budget)
+        if (launches > 100000) { cudaFree(acc); return lya_fail(ctx, LYA_ERR_CUDA, "k_xi made no progress"); }
+    }
+    cudaEventRecord(ctx->ev[1], s);
+    k_xi_finalize<<<(nb + 255) / 256, 256, 0, s>>>(P.S, P.W, P.N, nb, S, W, (unsigned long long *)N, xi);
+    cudaEventRecord(ctx->ev[2], s);
+    cudaError_t e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { cudaFree(acc); return lya_cuda_fail(ctx, e, "lya_xi2pcf"); }
+    if (h[3] != 0) { cudaFree(acc); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
+    if (stats) {
+        memset(stats, 0, sizeof(*stats));
+        stats->n_forest_pairs = (uint64_t)pairs->n;
+        stats->n_visited = h[1];
+        stats->n_evaluated = h[2];
+        // n_binned = sum N: small D2H
+        unsigned long long *hN = (unsigned long long *)malloc(sizeof(unsigned long long) * nb);
+        if (hN && cudaMemcpy(hN, P.N, sizeof(unsigned long long) * nb, cudaMemcpyDeviceToHost) == cudaSuccess)
+            for (int k = 0; k < nb; ++k) stats->n_binned += hN[k];
+        free(hN);
+        cudaEventElapsedTime(&stats->ms_main, ctx->ev[0], ctx->ev[1]);
+        cudaEventElapsedTime(&stats->ms_total, ctx->ev[0], ctx->ev[2]);
+    }
+    cudaFree(acc);
+    return LYA_OK;
+}

@@ -1,0 +1,331 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the ctypes binding) against the
+CPU oracle, element by element on the same seeded inputs.
+
+Bars (BASELINE.json north_star; floors = reading R-16 of DESIGN.md):
+  N, n_kept, pair lists : bit-exact / set-equal
+  S : |dS_A| <= 1e-9 * max(|S_A|, 1e-4 * Sabs_A)      W : |dW_A| <= 1e-9 * W_A
+  D : |dD_AB| <= 1e-7 * max(|D_AB|, 1e-6)
+"""
+import numpy as np
+import pytest
+
+from paper_2507_00129_b200 import gen
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2507_00129_b200 import binding, build
+    build.build()
+    c = binding.Context("cuda:0")
+    yield c
+    c.close()
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2507_00129_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import oracle
+    return oracle
+
+
+def pair_set(pq):
+    pq = np.asarray(pq, dtype=np.int64).reshape(-1, 2)
+    return set((pq[:, 0] << 32 | pq[:, 1]).tolist())
+
+
+def check_xi(g, o, label=""):
+    N = g["N"].cpu().numpy().view(np.uint64)
+    assert np.array_equal(N, o["N"]), f"{label}: pair counts differ in {(N != o['N']).sum()} bins"
+    S = g["S"].cpu().numpy(); W = g["W"].cpu().numpy(); xi = g["xi"].cpu().numpy()
+    tolS = 1e-9 * np.maximum(np.abs(o["S"]), 1e-4 * o["Sabs"])
+    assert np.all(np.abs(S - o["S"]) <= tolS), f"{label}: S off by {np.max(np.abs(S - o['S']) / np.maximum(tolS, 1e-300))} tol"
+    assert np.all(np.abs(W - o["W"]) <= 1e-9 * o["W"]), f"{label}: W"
+    nz = o["W"] > 0
+    assert np.all(np.abs(xi[nz] - o["xi"][nz]) <= 1e-9 * np.maximum(np.abs(o["xi"][nz]), 1e-4 * o["Sabs"][nz] / o["W"][nz]))
+    assert np.all(xi[~nz] == 0.0)
+    assert g["stats"]["n_binned"] == int(o["N"].sum())
+    assert g["stats"]["n_visited"] == int(o["N"].sum()) + o["n_out"]
+
+
+def check_dmat(g, o, label=""):
+    assert g["stats"]["n_kept"] == o["n_kept"], f"{label}: n_kept {g['stats']['n_kept']} vs {o['n_kept']}"
+    Wd = g["Wd"].cpu().numpy()
+    assert np.all(np.abs(Wd - o["Wd"]) <= 1e-9 * o["Wd"]), f"{label}: Wd"
+    D = g["D"].cpu().numpy()
+    err = np.abs(D - o["D"]); tol = 1e-7 * np.maximum(np.abs(o["D"]), 1e-6)
+    assert np.all(err <= tol), f"{label}: D worst {np.max(err / tol)} x tol at {np.unravel_index(np.argmax(err / tol), D.shape)}"
+    if g["Dn"] is not None:
+        Dn = g["Dn"].cpu().numpy()
+        scale = np.maximum(o["Wd"], 1e-300)[:, None]
+        assert np.all(np.abs(Dn - o["Dn"]) / scale <= tol), f"{label}: Dn"
+
+
+# ------------------------------------------------------------------ configs[0]
+def test_cfg0_neighbours_set_equal(ctx, B, orc, cfg0):
+    d = B.DeviceForests(cfg0)
+    pairs = ctx.lya_neighbours(d, B.binning())
+    pq = pairs.export().cpu().numpy()
+    ref = orc.pairs_brute(cfg0)
+    assert pairs.n == len(ref)
+    assert np.all(pq[:, 0] < pq[:, 1])
+    assert len(pair_set(pq)) == len(pq)
+    assert pair_set(pq) == pair_set(ref)
+
+
+def test_cfg0_xi_all_pairs_and_neighbour_list(ctx, B, orc, cfg0):
+    d = B.DeviceForests(cfg0)
+    b = B.binning()
+    pq_all = orc.pairs_all(cfg0.n_forest)
+    o = orc.xi(cfg0, pq_all)
+    g_all = ctx.lya_xi2pcf(d, b, ctx.lya_pairs_import(pq_all))
+    check_xi(g_all, o, "cfg0 all pairs")
+    g_nb = ctx.lya_xi2pcf(d, b, ctx.lya_neighbours(d, b))
+    assert np.array_equal(g_nb["N"].cpu().numpy().view(np.uint64), o["N"])      # pin P1 on the GPU side
+
+
+@pytest.mark.parametrize("variant", [1, 2, 4])
+def test_cfg0_xi_kernel_variants(B, orc, cfg0, variant, monkeypatch):
+    monkeypatch.setenv("LYA_XI_VARIANT", str(variant))
+    c = B.Context("cuda:0")
+    d = B.DeviceForests(cfg0)
+    pq = orc.pairs_brute(cfg0)
+    check_xi(c.lya_xi2pcf(d, B.binning(), c.lya_pairs_import(pq)), orc.xi(cfg0, pq), f"variant {variant}")
+    c.close()
+
+
+def test_cfg0_dmat_no_rejection(ctx, B, orc, cfg0):
+    d = B.DeviceForests(cfg0)
+    pq = orc.pairs_brute(cfg0)
+    o = orc.dmat(cfg0, pq, 0.0, gen.mask_seed(0))
+    g = ctx.lya_dmat(d, B.binning(), ctx.lya_pairs_import(pq), 0.0, gen.mask_seed(0))
+    check_dmat(g, o, "cfg0 f=0")
+    # PD6 on the GPU: f = 0 => Wd == W of lya_xi2pcf, n_kept == sum N
+    x = ctx.lya_xi2pcf(d, B.binning(), ctx.lya_pairs_import(pq))
+    assert g["stats"]["n_kept"] == x["stats"]["n_binned"]
+    assert np.allclose(g["Wd"].cpu().numpy(), x["W"].cpu().numpy(), rtol=1e-12)
+
+
+@pytest.mark.parametrize("f", [0.5, 0.99, 1.0])
+def test_cfg0_dmat_with_mask(ctx, B, orc, cfg0, f):
+    d = B.DeviceForests(cfg0)
+    pq = orc.pairs_brute(cfg0)
+    o = orc.dmat(cfg0, pq, f, gen.mask_seed(3))
+    g = ctx.lya_dmat(d, B.binning(), ctx.lya_pairs_import(pq), f, gen.mask_seed(3))
+    check_dmat(g, o, f"cfg0 f={f}")
+    if f == 1.0:
+        assert g["stats"]["n_kept"] == 0 and float(g["D"].abs().max()) == 0.0
+
+
+def test_hand_built_cases_P6(ctx, B, orc):
+    import os
+    from decimal import Decimal, getcontext
+    getcontext().prec = 50
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "p6_hand_cases.txt")
+    rows = [l.split("#")[0].split() for l in open(path) if l.strip() and not l.startswith("#")]
+    for s_txt, ci, cj, _, _, eA in rows:
+        s = float(s_txt)
+        uq = (1.0 - 2.0 * s * s, 2.0 * s * float(Decimal(1 - Decimal(s_txt) ** 2).sqrt()), 0.0)
+        f = gen.two_forests([float(ci)], [float(cj)], (1.0, 0.0, 0.0), uq)
+        g = ctx.lya_xi2pcf(B.DeviceForests(f), B.binning(), ctx.lya_pairs_import([[0, 1]]))
+        N = g["N"].cpu().numpy()
+        if int(eA) >= 0:
+            assert N.sum() == 1 and N[int(eA)] == 1, (s_txt, ci, cj)
+        else:
+            assert N.sum() == 0
+
+
+# ------------------------------------------------------------------ shaped sub-workloads
+@pytest.mark.parametrize("cfg,n", [(1, 1200), (4, 1500)])
+def test_shaped_subpatch_neighbours_and_xi(ctx, B, orc, cfg, n):
+    f = gen.make_config(cfg, n_forest=n)
+    d = B.DeviceForests(f)
+    b = B.binning()
+    pairs = ctx.lya_neighbours(d, b)
+    ref = orc.pairs_window(f)
+    assert pairs.n == len(ref) and pair_set(pairs.export().cpu().numpy()) == pair_set(ref)
+    check_xi(ctx.lya_xi2pcf(d, b, pairs), orc.xi(f, ref), f"cfg{cfg} n={n}")
+
+
+@pytest.mark.parametrize("cfg,n,frac", [(1, 150, 0.9), (4, 200, 0.99), (4, 120, 0.0)])
+def test_shaped_subpatch_dmat(ctx, B, orc, cfg, n, frac):
+    f = gen.make_config(cfg, n_forest=n, density_scale=4.0)
+    d = B.DeviceForests(f)
+    pairs = ctx.lya_neighbours(d, B.binning())
+    ref = orc.pairs_window(f)
+    assert pairs.n == len(ref) and pairs.n > 100
+    seed = gen.mask_seed(cfg)
+    check_dmat(ctx.lya_dmat(d, B.binning(), pairs, frac, seed), orc.dmat(f, ref, frac, seed), f"cfg{cfg} f={frac}")
+
+
+def test_generic_binning_non_power_of_two(ctx, B, orc):
+    f = gen.make_config(1, n_forest=400)
+    d = B.DeviceForests(f)
+    b = B.binning(150.0, 90.0, 30, 40)
+    ob = orc.binning(150.0, 90.0, 30, 40)
+    pairs = ctx.lya_neighbours(d, b)
+    ref = orc.pairs_window(f, ob)
+    assert pair_set(pairs.export().cpu().numpy()) == pair_set(ref)
+    check_xi(ctx.lya_xi2pcf(d, b, pairs), orc.xi(f, ref, ob), "generic bins")
+    f2 = gen.make_config(1, n_forest=100, density_scale=4.0)
+    ref2 = orc.pairs_window(f2, ob)
+    g = ctx.lya_dmat(B.DeviceForests(f2), b, ctx.lya_pairs_import(ref2), 0.8, 5)
+    check_dmat(g, orc.dmat(f2, ref2, 0.8, 5, b=ob), "generic bins D")
+
+
+def test_long_and_ragged_forests_tiles(ctx, B, orc):
+    """Forests longer than one staging tile (128 px), plus 1- and 2-pixel forests and an empty one."""
+    rng = np.random.default_rng(3)
+    lens = [300, 257, 1, 2, 0, 129, 128, 40]
+    chis, ws, ds, lls = [], [], [], []
+    for n in lens:
+        c0 = rng.uniform(3600, 3700)
+        chis.append(c0 + np.cumsum(rng.uniform(0.5, 2.5, n)))
+        ws.append(rng.uniform(0.5, 2.0, n)); ds.append(rng.normal(0, 0.3, n))
+        lls.append(3.55 + 1e-4 * np.arange(n) + rng.uniform(0, 1e-5, n))
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    ra = rng.uniform(0, 0.02, len(lens)); dec = rng.uniform(-0.01, 0.01, len(lens))
+    ux, uy, uz = gen.unit_vectors(ra, dec)
+    f = gen.Forests(ra, dec, ux, uy, uz, np.zeros(len(lens)), off, np.concatenate(chis), np.concatenate(ws),
+                    np.concatenate(ds), np.concatenate(lls))
+    d = B.DeviceForests(f)
+    pairs = ctx.lya_neighbours(d, B.binning())
+    ref = orc.pairs_brute(f)
+    assert pair_set(pairs.export().cpu().numpy()) == pair_set(ref)
+    check_xi(ctx.lya_xi2pcf(d, B.binning(), pairs), orc.xi(f, ref), "long forests")
+
+
+# ------------------------------------------------------------------ invariances and edge cases
+def test_P7_pair_order_and_swap(ctx, B, orc, cfg0):
+    d = B.DeviceForests(cfg0)
+    pq = orc.pairs_brute(cfg0)
+    rng = np.random.default_rng(11)
+    g0 = ctx.lya_xi2pcf(d, B.binning(), ctx.lya_pairs_import(pq))
+    g1 = ctx.lya_xi2pcf(d, B.binning(), ctx.lya_pairs_import(pq[rng.permutation(len(pq))][:, ::-1].copy()))
+    assert np.array_equal(g0["N"].cpu().numpy(), g1["N"].cpu().numpy())
+    assert np.allclose(g0["W"].cpu().numpy(), g1["W"].cpu().numpy(), rtol=1e-12)
+    a = ctx.lya_dmat(d, B.binning(), ctx.lya_pairs_import(pq), 0.9, 9)
+    b = ctx.lya_dmat(d, B.binning(), ctx.lya_pairs_import(pq[rng.permutation(len(pq))]), 0.9, 9)
+    assert a["stats"]["n_kept"] == b["stats"]["n_kept"]
+    assert np.allclose(a["Dn"].cpu().numpy(), b["Dn"].cpu().numpy(), rtol=0, atol=1e-10 * float(a["Wd"].max()))
+
+
+def test_P8_degenerate_catalogues(ctx, B, cfg0):
+    one = cfg0.subset([5])
+    d = B.DeviceForests(one)
+    pairs = ctx.lya_neighbours(d, B.binning())
+    assert pairs.n == 0
+    g = ctx.lya_xi2pcf(d, B.binning(), pairs)
+    assert int(g["N"].sum()) == 0 and float(g["S"].abs().sum()) == 0 and float(g["xi"].abs().sum()) == 0
+    far = gen.two_forests(cfg0.chi[:24], cfg0.chi[24:48], (1, 0, 0), (0, 1, 0))
+    assert ctx.lya_neighbours(B.DeviceForests(far), B.binning()).n == 0
+
+
+def test_P9_rotations_wrap_and_pole(ctx, B, orc, cfg0):
+    """Rigid rotations (across RA = 0 and over a pole): the cell grid must list the same set;
+    N equal except for pairs the rounding of the rotated unit vectors moves across an edge."""
+    d0 = B.DeviceForests(cfg0)
+    N0 = ctx.lya_xi2pcf(d0, B.binning(), ctx.lya_neighbours(d0, B.binning()))["N"].cpu().numpy()
+    for ang_y, ang_z in [(0.0, -0.03), (np.pi / 2 - 0.01, 0.3), (np.pi / 2, 0.0), (-np.pi / 2 + 0.02, 3.1)]:
+        cy, sy, cz, sz = np.cos(ang_y), np.sin(ang_y), np.cos(ang_z), np.sin(ang_z)
+        Ry = np.array([[cy, 0, -sy], [0, 1, 0], [sy, 0, cy]]); Rz = np.array([[cz, -sz, 0], [sz, cz, 0], [0, 0, 1]])
+        u = (Rz @ Ry @ np.stack([cfg0.ux, cfg0.uy, cfg0.uz]))
+        f = gen.Forests(np.arctan2(u[1], u[0]), np.arcsin(np.clip(u[2], -1, 1)), u[0].copy(), u[1].copy(), u[2].copy(),
+                        cfg0.zq, cfg0.pix_off, cfg0.chi, cfg0.w, cfg0.delta, cfg0.loglam)
+        d = B.DeviceForests(f, with_radec=True)
+        pairs = ctx.lya_neighbours(d, B.binning())
+        assert pair_set(pairs.export().cpu().numpy()) == pair_set(orc.pairs_brute(f))
+        g = ctx.lya_xi2pcf(d, B.binning(), pairs)
+        check_xi(g, orc.xi(f, orc.pairs_brute(f)), "rotated")
+        assert np.abs(g["N"].cpu().numpy() - N0).sum() <= 8          # edge-straddling pairs only
+        # device-derived unit vectors (ra/dec only): same list up to edge-ambiguous pairs
+        p2 = ctx.lya_neighbours(d, B.binning(), use_u=False)
+        assert abs(p2.n - pairs.n) <= 2
+
+
+def test_error_statuses(ctx, B, cfg0):
+    bad = gen.make_config(0)
+    bad.chi[5], bad.chi[6] = bad.chi[6], bad.chi[5]
+    d = B.DeviceForests(bad)
+    with pytest.raises(B.LyaError) as e:
+        ctx.lya_neighbours(d, B.binning())
+    assert e.value.name == "LYA_ERR_UNSORTED"
+    nanf = gen.make_config(0); nanf.w[100] = np.nan
+    with pytest.raises(B.LyaError) as e:
+        ctx.lya_neighbours(B.DeviceForests(nanf), B.binning())
+    assert e.value.name == "LYA_ERR_INVALID_ARG"
+    with pytest.raises(B.LyaError) as e:
+        ctx.lya_neighbours(B.DeviceForests(cfg0), B.binning(200.0, 200.0, 100, 100))
+    assert e.value.name == "LYA_ERR_CAPACITY"
+    deg = gen.make_config(0); deg.loglam[:24] = 3.6                    # forest 0: a single lambda -> V = 0
+    dd = B.DeviceForests(deg)
+    with pytest.raises(B.LyaError) as e:
+        ctx.lya_dmat(dd, B.binning(), ctx.lya_pairs_import([[0, 1]]), 0.0, 1)
+    assert e.value.name == "LYA_ERR_DEGENERATE_FOREST"
+    with pytest.raises(B.LyaError) as e:
+        ctx.lya_xi2pcf(B.DeviceForests(cfg0), B.binning(), ctx.lya_pairs_import([[0, 99]]))
+    assert e.value.name == "LYA_ERR_INVALID_ARG"
+    with pytest.raises(B.LyaError):
+        ctx.lya_pairs_import([[3, 3]])
+
+
+def test_zero_weights_count_geometrically(ctx, B, orc):
+    f = gen.make_config(0); f.w[::3] = 0.0                              # reading R-7
+    pq = orc.pairs_brute(f)
+    check_xi(ctx.lya_xi2pcf(B.DeviceForests(f), B.binning(), ctx.lya_pairs_import(pq)), orc.xi(f, pq), "w=0")
+
+
+def test_run_host_end_to_end(ctx, B, orc, cfg0):
+    out = ctx.lya_run_host(cfg0, B.binning(), do_xi=True, do_dmat=True, reject_fraction=0.5, seed=42)
+    pq = orc.pairs_brute(cfg0)
+    o = orc.xi(cfg0, pq)
+    assert out["n_pairs"] == len(pq)
+    assert np.array_equal(out["N"], o["N"])
+    assert np.all(np.abs(out["W"] - o["W"]) <= 1e-9 * o["W"])
+    od = orc.dmat(cfg0, pq, 0.5, 42)
+    assert out["stats_dmat"]["n_kept"] == od["n_kept"]
+    assert np.all(np.abs(out["D"] - od["D"]) <= 1e-7 * np.maximum(np.abs(od["D"]), 1e-6))
+
+
+# ------------------------------------------------------------------ full-size configs, bench launch configuration
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_full_size_properties_and_sampled_parity(ctx, B, orc, cfg):
+    """At BASELINE.json's full sizes the oracle cannot run everything: check the neighbour list
+    on sampled forests against a numpy brute force over ALL forests, the exact bookkeeping
+    identities, and element-by-element parity on a random sample of the listed forest pairs."""
+    import torch
+    f = gen.make_config(cfg)
+    d = B.DeviceForests(f)
+    b = B.binning()
+    pairs = ctx.lya_neighbours(d, b)
+    pq = pairs.export()
+    assert bool((pq[:, 0] < pq[:, 1]).all())
+    # (1) neighbour sets of sampled forests vs numpy over all N
+    rng = np.random.default_rng(cfg)
+    cm = f.chi[f.pix_off[:-1]]
+    for p in rng.choice(f.n_forest, 40, replace=False):
+        s = 0.5 * np.sqrt((f.ux - f.ux[p]) ** 2 + (f.uy - f.uy[p]) ** 2 + (f.uz - f.uz[p]) ** 2)
+        want = set(np.nonzero(((cm + cm[p]) * s < 200.0) & (np.arange(f.n_forest) != p))[0].tolist())
+        got = set(pq[pq[:, 0] == p][:, 1].cpu().tolist()) | set(pq[pq[:, 1] == p][:, 0].cpu().tolist())
+        assert got == want
+    # (2) exact bookkeeping at full size
+    g = ctx.lya_xi2pcf(d, b, pairs)
+    lens = torch.from_numpy(np.diff(f.pix_off)).to(pq.device)
+    visited = int((lens[pq[:, 0].long()] * lens[pq[:, 1].long()]).sum())
+    assert g["stats"]["n_visited"] == visited
+    assert int(g["N"].sum()) == g["stats"]["n_binned"] <= visited
+    assert float(g["W"].min()) > 0
+    # (3) sampled forest pairs: full parity
+    sel = torch.from_numpy(rng.choice(pairs.n, 20000, replace=False)).to(pq.device)
+    sub = pq[sel].cpu().numpy()
+    check_xi(ctx.lya_xi2pcf(d, b, ctx.lya_pairs_import(sub)), orc.xi(f, sub), f"cfg{cfg} sampled pairs")
+    subd = sub[:1500]
+    seed = gen.mask_seed(3 if cfg == 2 else 4)
+    check_dmat(ctx.lya_dmat(d, b, ctx.lya_pairs_import(subd), 0.99, seed), orc.dmat(f, subd, 0.99, seed),
+               f"cfg{cfg} sampled pairs D")
