@@ -1,0 +1,339 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Lya2pcf pixel-pair hot path on B200.
+
+A "step" is one pass of the whole hot path over one synthetic catalogue:
+lya_neighbours -> lya_xi2pcf -> lya_dmat (stages 1-4 of BASELINE.json north_star).
+`value` = pixel pairs binned per second over the step (xi: sum_A N_A, D: the in-grid
+pairs scanned by the keep mask), inputs resident in HBM; `e2e` = the same through
+lya_run_host with pinned HOST buffers (H2D of the catalogue and D2H of xi, D inside the
+timed region).  Prints ONE JSON line on rank 0.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg2|cfg1|cfg0]
+  python bench.py --impl reference ...     # the CPU oracle on a bounded sample
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "xi + D-matrix pixel-pairs/s (binned pairs per second over neighbours+xi+D)"
+UNIT = "pixel-pairs/s"
+WORKLOADS = {
+    "cfg4": dict(cfg=4, mask_cfg=4, desc="configs[4] DESI-Y5-shaped: 900k forests, 14000 deg2, xi + D (f=0.99)"),
+    "cfg2": dict(cfg=2, mask_cfg=3, desc="configs[2]+[3] DR16-shaped: 210k forests, 9400 deg2, xi + D (f=0.99)"),
+    "cfg1": dict(cfg=1, mask_cfg=1, desc="configs[1] small patch: 20k forests, 100 deg2, xi + D (f=0.99)"),
+    "cfg0": dict(cfg=0, mask_cfg=0, desc="configs[0] tiny: 64 forests, xi + D (f=0)"),
+}
+FP64_LANES_PER_SM = 64      # B200 fp64 vector units per SM (DFMA/DADD/DMUL lanes per clock)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0), "fallback"
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    from paper_2507_00129_b200 import gen
+    wl = WORKLOADS[args.workload]
+    n_s = min(args.ref_forests, gen.CONFIGS[wl["cfg"]]["n"])
+    f = gen.make_config(wl["cfg"], n_forest=n_s)
+    cat = orc.Catalogue(f)
+    pq = orc.pairs_window(cat)
+    pq_d = pq[: max(1, len(pq) // args.ref_dmat_div)]
+    seed = gen.mask_seed(wl["mask_cfg"])
+    frac = 0.0 if wl["cfg"] == 0 else 0.99
+
+    def step():
+        x = orc.xi(cat, pq)
+        d = orc.dmat(cat, pq_d, frac, seed, want_D=False)
+        nd = int(orc.xi(cat, pq_d)["N"].sum()) if len(pq_d) != len(pq) else int(x["N"].sum())
+        return int(x["N"].sum()) + nd
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    pairs = 0
+    for _ in range(args.steps):
+        pairs += step()
+    dt = time.perf_counter() - t0
+    val = pairs / dt
+    sample = (f"{n_s} forests of {args.workload} at the config's sky density: xi on {len(pq)} forest pairs, "
+              f"naive D on {len(pq_d)} forest pairs, per step")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "description": wl["desc"], "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def cpu_baseline(wl, budget_forests):
+    """The oracle timed on this box's host cores on a bounded sample (about 10-30 s)."""
+    from oracle import oracle as orc
+    from paper_2507_00129_b200 import gen
+    n_s = min(budget_forests, gen.CONFIGS[wl["cfg"]]["n"])
+    f = gen.make_config(wl["cfg"], n_forest=n_s)
+    cat = orc.Catalogue(f)
+    pq = orc.pairs_window(cat)
+    t0 = time.perf_counter()
+    x = orc.xi(cat, pq)
+    t_xi = time.perf_counter() - t0
+    pq_d = pq[: max(1, len(pq) // 50)]
+    frac = 0.0 if wl["cfg"] == 0 else 0.99
+    t0 = time.perf_counter()
+    orc.dmat(cat, pq_d, frac, gen.mask_seed(wl["mask_cfg"]), want_D=False)
+    t_d = time.perf_counter() - t0
+    nd = int(orc.xi(cat, pq_d)["N"].sum())
+    nx = int(x["N"].sum())
+    return {"value": (nx + nd) / (t_xi + t_d), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "xi_pairs_per_s": nx / t_xi, "dmat_pairs_per_s": nd / max(t_d, 1e-9),
+            "sample": f"{n_s} forests at the workload's sky density: xi over {len(pq)} forest pairs ({t_xi:.1f} s), "
+                      f"naive D (f={frac}) over {len(pq_d)} forest pairs ({t_d:.1f} s)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=os.environ.get("LYA_BENCH_WORKLOAD", "cfg4"), choices=list(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-dmat", action="store_true")
+    ap.add_argument("--ref-forests", type=int, default=3000)
+    ap.add_argument("--ref-dmat-div", type=int, default=50)
+    ap.add_argument("--cpu-forests", type=int, default=3000)
+    ap.add_argument("--forests", type=int, default=0,
+                    help="profiling only: a shaped sub-catalogue of this many forests (same sky density)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2507_00129_b200 import binding as B, build, gen
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    wl = WORKLOADS[args.workload]
+    frac = 0.0 if wl["cfg"] == 0 else 0.99
+    mseed = gen.mask_seed(wl["mask_cfg"])
+    # weak scaling: every rank owns an independent catalogue of the same shape (seed + rank)
+    f = gen.make_config(wl["cfg"], n_forest=args.forests or None,
+                        seed=None if rank == 0 else gen.SEED_BASE + wl["cfg"] + 1000 * rank)
+    ctx = B.Context(f"cuda:{local}")
+    d = B.DeviceForests(f, device=f"cuda:{local}")
+    b = B.binning()
+    do_d = not args.no_dmat
+
+    def step():
+        pairs = ctx.lya_neighbours(d, b)
+        x = ctx.lya_xi2pcf(d, b, pairs)
+        dm = ctx.lya_dmat(d, b, pairs, frac, mseed, want_Dn=False) if do_d else None
+        pairs.free()
+        return x, dm
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    ms_xi, ms_dm, launches = [], [], 0
+    pairs_total = 0
+    for _ in range(args.steps):
+        x, dm = step()
+        ms_xi.append(x["stats"]["ms_main"])
+        pairs_total += x["stats"]["n_binned"]
+        launches += 12 + 3           # neighbour pipeline kernels + xi (main, finalize) + validation
+        if dm is not None:
+            ms_dm.append(dm["stats"]["ms_main"])
+            pairs_total += dm["stats"]["n_binned"]
+            launches += 4
+    ev1.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms, float(pairs_total)], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, pairs_all = float(tmax[0]), float(tsum[1])
+    else:
+        pairs_all = float(pairs_total)
+    value = pairs_all / (ms * 1e-3)
+
+    # ---- e2e: host buffers through lya_run_host (pinned), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        pin = {}
+        for k in ("ux", "uy", "uz", "pix_off", "chi", "w", "delta", "loglam"):
+            tt = torch.from_numpy(np.ascontiguousarray(getattr(f, k))).pin_memory()
+            pin[k] = tt
+        class HostF:
+            pass
+        hf = HostF()
+        for k, v in pin.items():
+            setattr(hf, k, v.numpy())
+        nb = b.n_par * b.n_perp
+        out = {k: torch.empty(nb, dtype=torch.float64).pin_memory().numpy() for k in ("S", "W", "xi")}
+        out["N"] = torch.empty(nb, dtype=torch.int64).pin_memory().numpy().view(np.uint64)
+        if do_d:
+            out["D"] = torch.empty((nb, nb), dtype=torch.float64).pin_memory().numpy()
+            out["Wd"] = torch.empty(nb, dtype=torch.float64).pin_memory().numpy()
+        h2d = sum(v.numel() * v.element_size() for v in pin.values())
+        d2h = sum(v.nbytes for v in out.values())
+        ctx.lya_run_host(hf, b, True, do_d, frac, mseed, out=dict(out))
+        barrier()
+        n_e2e = max(1, min(args.steps, 2))
+        t0 = time.perf_counter()
+        pe = 0
+        for _ in range(n_e2e):
+            r = ctx.lya_run_host(hf, b, True, do_d, frac, mseed, out=dict(out))
+            pe += r["stats_xi"]["n_binned"] + (r["stats_dmat"]["n_binned"] if do_d else 0)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        te = torch.tensor([dt, float(pe)], dtype=torch.float64, device=f"cuda:{local}")
+        if world > 1:
+            tm = te.clone(); dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+            ts = te.clone(); dist.all_reduce(ts, op=dist.ReduceOp.SUM)
+            dt, pe = float(tm[0]), float(ts[1])
+        e2e = {"value": pe / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3}
+
+    if rank == 0:
+        peaks, peak_kind = measured_peaks()
+        sx, sd = x["stats"], (dm["stats"] if dm is not None else None)
+        t_xi = float(np.mean(ms_xi)) * 1e-3
+        t_dm = float(np.mean(ms_dm)) * 1e-3 if ms_dm else 0.0
+        sm_clk = (clocks.get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)) * 1e6
+        # roofline: algorithmic fp64-pipe instructions per launch
+        #   xi: 6 per visited pixel pair (sub, add, 2 mul, 2 floor) + 2 per binned pair (2 FMA)
+        alg_xi = 6.0 * sx["n_visited"] + 2.0 * sx["n_binned"]
+        peak_alu = ctx.sm_count() * FP64_LANES_PER_SM * peaks.get("sm_max_mhz", 1965.0) * 1e6
+        roof_xi = {"bound": "alu", "kernel": "k_xi", "achieved": alg_xi / t_xi / 1e12, "peak": peak_alu / 1e12,
+                   "unit": "Tinst/s (fp64 lane-instructions)", "frac": alg_xi / t_xi / peak_alu, "traffic": None,
+                   "peak_source": f"derived: {ctx.sm_count()} SMs x {FP64_LANES_PER_SM} fp64 lanes x sm_max_mhz ({peak_kind} MEASURED_PEAKS.json)",
+                   "frac_at_sampled_clock": alg_xi / t_xi / (ctx.sm_count() * FP64_LANES_PER_SM * sm_clk),
+                   "measured_peaks": {k: ctx.lya_measure_peak(k) for k in ("fp64_fma", "fp64_add", "smem_cas64", "smem_add32", "l2_red64")}}
+        roof = roof_xi
+        extra = {"xi": {"binned_pairs_per_s": sx["n_binned"] / t_xi, "visited_pairs_per_s": sx["n_visited"] / t_xi,
+                        "evaluated_pairs_per_s": sx["n_evaluated"] / t_xi, "ms": t_xi * 1e3,
+                        "forest_pairs": sx["n_forest_pairs"], "roofline": roof_xi}}
+        if sd is not None:
+            # D: algorithmic fp64 instructions = H pass (6 per visited + 4 FMA per binned) + per kept pair
+            # (n_p + n_q) x (6 geometry + 2) for T2/T3 and 4 per support bin for T4 -- reported as scatter rate
+            extra["dmat"] = {"scanned_pairs_per_s": sd["n_binned"] / t_dm, "kept_pairs_per_s": sd["n_kept"] / t_dm,
+                             "ms": t_dm * 1e3, "n_kept": sd["n_kept"]}
+            if t_dm > t_xi:
+                alg_d = 6.0 * sd["n_visited"] + 4.0 * sd["n_binned"]
+                roof = {"bound": "alu", "kernel": "k_dmat", "achieved": alg_d / t_dm / 1e12, "peak": peak_alu / 1e12,
+                        "unit": "Tinst/s (fp64 lane-instructions)", "frac": alg_d / t_dm / peak_alu, "traffic": None,
+                        "note": "H-table pass only; the per-kept-pair scatter is bounded by L2 fp64 red throughput, see dmat.red_per_s",
+                        "peak_source": roof_xi["peak_source"]}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "description": wl["desc"], "n_forest": f.n_forest, "n_pix": f.n_pix,
+                       "bins": "50x50x4Mpc/h", "reject_fraction": frac, "dmat": do_d,
+                       "l2": "inputs (%.2f GB) larger than L2; Dn (50 MB) re-zeroed every step" % (f.n_pix * 32 / 1e9),
+                       "parallelism": f"independent catalogue per GPU x{world}"},
+            "roofline": roof, "clocks": clocks, "gpu_launches": launches, "e2e": e2e, **extra,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(wl, args.cpu_forests)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -172,6 +172,9 @@ class Context:
     def sync(self):
         self.stream.synchronize()
 
+    def sm_count(self) -> int:
+        return int(self.torch.cuda.get_device_properties(self.device).multi_processor_count)
+
     def _check(self, st):
         if st:
             raise LyaError(st, load().lya_last_error(self.h).decode())
