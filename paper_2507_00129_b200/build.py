@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblya.so")
-SOURCES = ["lya_api.cu", "neighbours.cu", "xi2pcf.cu", "dmat.cu", "peaks.cu"]
+SOURCES = ["lya_api.cu", "neighbours.cu", "prep.cu", "xi2pcf.cu", "dmat.cu", "peaks.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

@@ -42,6 +42,55 @@ lya_status lya_check_forests_host(lya_ctx *ctx, const lya_forests *f, bool need_
 lya_status lya_validate_forests(lya_ctx *ctx, const lya_forests *f, bool need_delta, bool need_loglam,
                                 int *max_len);
 
+struct BinParams;
+// ---- prepared catalogue (prep.cu): padded, 16-byte aligned SoA copy of the forests ----
+// Every forest starts at an even offset and is padded to an even length, so each
+// sub-array of a forest can be moved with 16-byte vector loads.  Pad pixels hold
+// chi = LYA_CHI_SENTINEL and 0 elsewhere (never inside any grid).
+struct __align__(16) ForestHead {   // 64 bytes, one per forest
+    double ux, uy, uz;              // sightline unit vector
+    double dmin;                    // smallest chi spacing inside the forest (1e300 if < 2 pixels)
+    double chi0, chi1;              // first / last pixel (valid when len > 0)
+    long long off;                  // offset of the forest in the packed arrays (even)
+    int len;                        // pixels
+    int flags;                      // bit 0: degenerate for eq. 2.7 (sum w == 0 or sum w u^2 == 0)
+};
+struct LyaPrep {
+    int64_t n_forest, n_pack;
+    ForestHead *head;               // [n_forest]
+    double *chi, *w;                // [n_pack]
+    double *a;                      // xi: w * delta
+    double *u, *ea, *eg;            // dmat: u = L - Lbar, ea = w / sum w, eg = w u / sum w u^2 (eq. 2.7)
+    void *base;                     // single allocation behind all of the above
+    int max_len;
+};
+// Builds the prepared catalogue on the ctx stream (no host synchronisation except the
+// one that returns n_pack).  want_xi -> a;  want_dmat -> u, ea, eg.
+lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool want_dmat, LyaPrep *out);
+void lya_prep_free(LyaPrep *p);
+
+// ---- pair bucketing (prep.cu) -----------------------------------------------------------
+// Stable counting sort of the forest-pair list by the r_perp column of the pair's first
+// pixel pair (c_first).  Keys: 0..n_perp-1 = fast-path pairs whose bins lie in columns
+// [c_first, c_first + LYA_NCOL); n_perp = pairs for the generic kernels (long forests, wide
+// column span, spacing below the bin width); n_perp+1 = pairs with nothing inside the grid.
+#define LYA_NCOL 8                  // r_perp columns of a warp-private sub-histogram
+#define LYA_FAST_TILE 80            // longest forest the fast kernels stage in one piece
+struct LyaBuckets {
+    int32_t *pq;                    // device [n][2], sorted by key (stable)
+    int64_t n;
+    int64_t n_fast, n_generic, n_skip;
+    unsigned long long visited;     // sum n_p * n_q over the whole list
+    int bad_pair;                   // a pair referred to a forest outside [0, n_forest)
+};
+lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *bp, const lya_pairs *pairs,
+                            int force_generic, LyaBuckets *out);
+void lya_buckets_free(LyaBuckets *b);
+
+// exclusive scan: in (u32 [n]) -> out (u64 [n+1], out[n] = total); tmp: ceil(n/2048)+2 u64
+cudaError_t lya_exclusive_scan(const unsigned *in, unsigned long long *out, int64_t n, unsigned long long *tmp,
+                               cudaStream_t s);
+
 #define LYA_CUDA(call)                                                          \
     do {                                                                        \
         cudaError_t e__ = (call);                                               \
@@ -125,5 +174,39 @@ __device__ __forceinline__ PairBin lya_make_pairbin(const BinParams &bp, double 
     g.cx = __dmul_rn(c, bp.inv_par);
     g.sy = __dmul_rn(s, bp.inv_perp);
     return g;
+}
+
+// r_perp column of a pixel pair with chi_i + chi_j = t, or n_perp when r_perp >= rperp_max
+// (same operations as lya_pix_bin, so the value is the column lya_pix_bin assigns).
+template <bool POW2>
+__device__ __forceinline__ int lya_col_of(const BinParams &bp, const PairBin &g, double t)
+{
+    if (POW2) {
+        unsigned by = lya_floor_u32(__dmul_rn(t, g.sy));
+        return (by < (unsigned)bp.n_perp) ? (int)by : bp.n_perp;
+    } else {
+        double rperp = __dmul_rn(t, g.s);
+        if (!(rperp < bp.rperp_max)) return bp.n_perp;
+        return (int)min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1));
+    }
+}
+
+// Can the fast kernels take this forest pair?  (warp-uniform; identical in the bucketing
+// pass and in the kernels.)  c_first: column of the pair's first pixels.  Returns the key.
+template <bool POW2>
+__device__ __forceinline__ int lya_pair_key(const BinParams &bp, const PairBin &g, const ForestHead &hp,
+                                            const ForestHead &hq, int &c_first)
+{
+    c_first = bp.n_perp;
+    if (hp.len == 0 || hq.len == 0) return bp.n_perp + 1;
+    c_first = lya_col_of<POW2>(bp, g, __dadd_rn(hp.chi0, hq.chi0));
+    if (c_first >= bp.n_perp) return bp.n_perp + 1;                 // r_perp grows with both pixels
+    int c_last = lya_col_of<POW2>(bp, g, __dadd_rn(hp.chi1, hq.chi1));
+    if (c_last >= bp.n_perp) c_last = bp.n_perp - 1;
+    bool fast = (hp.len <= LYA_FAST_TILE) && (hq.len <= LYA_FAST_TILE) && (c_last - c_first < LYA_NCOL);
+    // lanes of one flush hold pixel pairs (i, j_lane) with distinct j: their r_par bins differ
+    // when the spacing of q exceeds the bin width (margin 1e-6), see DESIGN.md "conflict-free runs"
+    fast = fast && (__dmul_rn(__dmul_rn(hq.dmin, g.c), bp.inv_par) > 1.000001);
+    return fast ? c_first : bp.n_perp;
 }
 #endif

@@ -252,6 +252,12 @@ struct Scratch {
 
 }  // namespace
 
+cudaError_t lya_exclusive_scan(const unsigned *in, unsigned long long *out, int64_t n, unsigned long long *tmp,
+                               cudaStream_t s)
+{
+    return exclusive_scan(in, out, n, tmp, s);
+}
+
 extern "C" lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                                      lya_pairs **out, int64_t *n_pairs)
 {

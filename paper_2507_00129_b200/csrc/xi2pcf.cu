@@ -4,20 +4,28 @@
 // over pixel pairs (i in p, j in q) of the listed forest pairs whose separation
 // r_par = |chi_i - chi_j| c, r_perp = (chi_i + chi_j) s falls in bin A.
 //
-// Design (B200): persistent grid, one WARP per forest pair at a time.
-//   * both forests are staged in shared memory (coalesced 8-byte loads; forest p is
-//     reused across the consecutive pairs of the list that share it);
+// Design (B200): persistent grid, one WARP per forest pair.
+//   * the forest-pair list is bucket-sorted by the r_perp column of the pair's first
+//     pixels (prep.cu); all bins of a pair lie in columns [c0, c0 + LYA_NCOL), so every
+//     warp keeps a PRIVATE (n_par x LYA_NCOL) sub-histogram in shared memory that lives
+//     across thousands of forest pairs and is merged into the global fp64/u64
+//     accumulators (red.global) only when the warp moves to another bucket;
+//   * both forests are staged in shared memory from the padded catalogue with 16-byte
+//     loads (forest p is reused across the consecutive pairs that share it);
 //   * lanes own DIAGONALS d = j - i of the (i, j) pixel-pair matrix.  Along a diagonal
 //     r_par is nearly constant and r_perp grows slowly, so consecutive pairs fall in the
-//     same bin: each lane accumulates a RUN (S, W, count) in registers and touches the
-//     histogram only when the bin changes (run-length accumulation);
-//   * only diagonals that can hold an in-grid pair are walked: chi is increasing, so
-//     the in-window j of every row i is a contiguous range found by binary search;
-//   * each lane walks D adjacent diagonals with a sliding register window over q, so a
-//     step costs one new q pixel per lane and one broadcast p pixel per warp;
-//   * runs are flushed into a per-block shared-memory histogram (u32 native atomic for
-//     N, fp64 CAS for S and W -- B200 has no native 64-bit shared atomic add), and the
-//     block histogram goes to global fp64/u64 with red.global once per launch.
+//     same bin: a lane accumulates a RUN (S, W, count) in registers and touches the
+//     sub-histogram only when the bin changes;
+//   * B200 has no native shared-memory fp64 (or 64-bit) atomic add -- they compile to a
+//     CAS loop -- so the run flush is a plain load-add-store, made safe by construction:
+//     the lanes of one flush hold pixel pairs (i, j_lane) with the same i and distinct j,
+//     and the pair is walked twice, once over chi_i >= chi_j and once over chi_i < chi_j,
+//     so two lanes can share a bin only if q's pixel spacing is below the r_par bin width;
+//     such pairs (and long forests, wide column spans) go to the generic kernel below,
+//     which uses CAS atomics on a block-level histogram;
+//   * only diagonals/rows that can hold an in-grid pair are walked: per-row binary
+//     searches on the increasing chi give the r_par window and the sign change, and a
+//     binary search along the first diagonal of each pass cuts the rows past r_perp_max.
 // Geometry is exact binary64, operation by operation (lya_internal.cuh), so N is
 // bit-identical to the oracle for any traversal order.
 #include <stdlib.h>
@@ -25,6 +33,8 @@
 
 namespace {
 
+// ======================= generic kernel: any forest length, any column span =======================
+// Block-level histogram with CAS atomics; pairs come from the ORIGINAL arrays.
 constexpr int XI_WARPS = 8;                 // warps per block
 constexpr int XI_THREADS = XI_WARPS * 32;
 constexpr int TILE = 128;                   // pixels of a forest staged per tile
@@ -254,6 +264,260 @@ cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
     return cudaGetLastError();
 }
 
+// ======================= fast kernel: warp-private sub-histograms ================================
+constexpr int FW = 8;                        // warps per block
+constexpr int FTHREADS = FW * 32;
+constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
+constexpr int FPAD = 2;                      // sentinel pixels either side of q (reads are clamped)
+constexpr int FSLOTS = 400;                  // n_par * LYA_NCOL <= FSLOTS
+constexpr int FCHUNK = 16;                   // forest pairs claimed per atomic
+
+struct XiFastParams {
+    LyaPrep prep;
+    const int32_t *pq;
+    int64_t n_pairs;
+    BinParams bp;
+    double *S, *W;
+    unsigned long long *N;
+    unsigned long long *counters;            // [4] next chunk, [2] evaluated
+};
+
+struct __align__(16) FastWarp {
+    double pc[FT], pa[FT], pw[FT];
+    double qc[FT + 2 * FPAD], qa[FT + 2 * FPAD], qw[FT + 2 * FPAD];
+    double2 SW[FSLOTS];
+    unsigned N[FSLOTS];
+};
+
+// slot of a pixel pair in the sub-histogram whose first column is c0, -1 outside the grid
+// or on the wrong side of chi_i = chi_j (sgn = 0: chi_i >= chi_j, sgn = -1: chi_i < chi_j).
+template <bool POW2>
+__device__ __forceinline__ int xi_slot(const BinParams &bp, const PairBin &g, double chi_i, double chi_j, int c0, int sgn)
+{
+    const double d = __dsub_rn(chi_i, chi_j);
+    const double t = __dadd_rn(chi_i, chi_j);
+    const bool side = ((__double2hiint(d) ^ sgn) >= 0);
+    unsigned bx, by;
+    bool ok;
+    if (POW2) {
+        bx = lya_floor_u32(__dmul_rn(fabs(d), g.cx));
+        by = lya_floor_u32(__dmul_rn(t, g.sy));
+        ok = (bx < (unsigned)bp.n_par) & (by < (unsigned)bp.n_perp);
+    } else {
+        const double rpar = __dmul_rn(fabs(d), g.c), rperp = __dmul_rn(t, g.s);
+        ok = (rpar < bp.rpar_max) & (rperp < bp.rperp_max);
+        bx = min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1));
+        by = min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1));
+    }
+    return (ok & side) ? (int)(bx * LYA_NCOL + by) - c0 : -1;
+}
+
+// Walk the diagonals [dlo, dhi] of a staged forest pair, D adjacent diagonals per lane.
+template <int D, bool POW2>
+__device__ __forceinline__ void xi_walk(FastWarp &ws, int mp, int mq, int dlo, int dhi, int sgn, double Tchi,
+                                        const BinParams &bp, const PairBin &g, int c0, int lane,
+                                        unsigned long long &evaluated)
+{
+    const double *qc = ws.qc + FPAD, *qa = ws.qa + FPAD, *qw = ws.qw + FPAD;
+    for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
+        const int dl = d0 + lane * D;                       // first diagonal of this lane
+        const int dpass_hi = min(dhi, d0 + 32 * D - 1);
+        const int i_begin = max(0, -dpass_hi);
+        int i_end = min(mp, mq - d0);                       // exclusive
+        if (i_end <= i_begin) continue;
+        {   // rows past r_perp_max: chi_p[i] + chi_q[i + d] grows with i and with d, so the first
+            // diagonal of the pass decides (Tchi is a conservative rperp_max / s)
+            int lo = i_begin, hi = i_end;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (ws.pc[mid] + qc[max(mid + d0, 0)] >= Tchi) hi = mid; else lo = mid + 1;
+            }
+            i_end = lo;
+        }
+        if (i_end <= i_begin) continue;
+        int cur[D]; double accS[D], accW[D]; unsigned cnt[D];
+        double wc[D], wa[D], ww[D];                         // sliding window over q
+#pragma unroll
+        for (int k = 0; k < D; ++k) { cur[k] = -1; accS[k] = 0.0; accW[k] = 0.0; cnt[k] = 0; }
+#pragma unroll
+        for (int k = 0; k < D - 1; ++k) {
+            const int j = min(max(i_begin + dl + k, -FPAD), mq + FPAD - 1);
+            wc[k] = qc[j]; wa[k] = qa[j]; ww[k] = qw[j];
+        }
+        evaluated += (unsigned long long)(i_end - i_begin) * D;
+        for (int ib = i_begin; ib < i_end; ib += D) {
+#pragma unroll
+            for (int u = 0; u < D; ++u) {
+                const int i = ib + u;
+                if (i < i_end) {                            // warp-uniform
+                    const double pci = ws.pc[i], pai = ws.pa[i], pwi = ws.pw[i];
+                    {   // the new q pixel of the lane's last diagonal goes into slot (u + D - 1) % D
+                        const int j = min(max(i + dl + D - 1, -FPAD), mq + FPAD - 1);
+                        wc[(u + D - 1) % D] = qc[j]; wa[(u + D - 1) % D] = qa[j]; ww[(u + D - 1) % D] = qw[j];
+                    }
+#pragma unroll
+                    for (int k = 0; k < D; ++k) {
+                        const int sl = (k + u) % D;         // slot holding q[i + dl + k]
+                        const int key = xi_slot<POW2>(bp, g, pci, wc[sl], c0, sgn);
+                        if (key != cur[k]) {
+                            if (cur[k] >= 0) {              // plain RMW: lanes of one row step hold distinct bins
+                                double2 v = ws.SW[cur[k]];
+                                v.x += accS[k]; v.y += accW[k];
+                                ws.SW[cur[k]] = v;
+                                atomicAdd(&ws.N[cur[k]], cnt[k]);
+                            }
+                            cur[k] = key; accS[k] = 0.0; accW[k] = 0.0; cnt[k] = 0;
+                        }
+                        if (key >= 0) {
+                            accS[k] = fma(pai, wa[sl], accS[k]);
+                            accW[k] = fma(pwi, ww[sl], accW[k]);
+                            cnt[k] += 1;
+                        }
+                    }
+                    __syncwarp();                           // order this row step's RMWs before the next one's
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < D; ++k)
+            if (cur[k] >= 0) {
+                double2 v = ws.SW[cur[k]];
+                v.x += accS[k]; v.y += accW[k];
+                ws.SW[cur[k]] = v;
+                atomicAdd(&ws.N[cur[k]], cnt[k]);
+            }
+        __syncwarp();
+    }
+}
+
+template <bool POW2>
+__device__ __forceinline__ void xi_walk_any(FastWarp &ws, int mp, int mq, int dlo, int dhi, int sgn, double Tchi,
+                                            const BinParams &bp, const PairBin &g, int c0, int lane,
+                                            unsigned long long &evaluated)
+{
+    if (dhi < dlo) return;
+    const int nd = dhi - dlo + 1;
+    if (nd <= 32) xi_walk<1, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
+    else if (nd <= 64) xi_walk<2, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
+    else if (nd <= 96) xi_walk<3, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
+    else xi_walk<4, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
+}
+
+// merge a warp's sub-histogram (first column c0) into the global accumulators and clear it
+__device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, int c0, int lane)
+{
+    const int n_slots = P.bp.n_par * LYA_NCOL;
+    __syncwarp();
+    for (int t = lane; t < n_slots; t += 32) {
+        const unsigned n = ws.N[t];
+        if (n) {
+            const int bx = t / LYA_NCOL, col = c0 + (t - bx * LYA_NCOL);
+            const double2 v = ws.SW[t];
+            if (col < P.bp.n_perp) {
+                const int A = bx * P.bp.n_perp + col;
+                atomicAdd(&P.N[A], (unsigned long long)n);
+                atomicAdd(&P.S[A], v.x);
+                atomicAdd(&P.W[A], v.y);
+            }
+            ws.SW[t] = make_double2(0.0, 0.0);
+            ws.N[t] = 0u;
+        }
+    }
+    __syncwarp();
+}
+
+template <bool POW2>
+__global__ void __launch_bounds__(FTHREADS, 2) k_xi_fast(XiFastParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    FastWarp &ws = ((FastWarp *)smem_raw)[wid];
+    const BinParams bp = P.bp;
+    for (int t = lane; t < FSLOTS; t += 32) { ws.SW[t] = make_double2(0.0, 0.0); ws.N[t] = 0u; }
+    if (lane < FPAD) { ws.qc[lane] = LYA_CHI_SENTINEL; ws.qa[lane] = 0.0; ws.qw[lane] = 0.0; }
+    __syncwarp();
+
+    const double *qc = ws.qc + FPAD;
+    unsigned long long evaluated = 0, since_merge = 0;
+    int cur_p = -1, head_p = -1, win_c0 = -1;
+    ForestHead hp;
+    hp.len = 0;
+    const int64_t n_chunks = (P.n_pairs + FCHUNK - 1) / FCHUNK;
+    for (;;) {
+        unsigned long long chunk = 0;
+        if (lane == 0) chunk = atomicAdd(&P.counters[4], 1ull);
+        chunk = __shfl_sync(0xffffffffu, chunk, 0);
+        if ((int64_t)chunk >= n_chunks) break;
+        const int64_t k0 = (int64_t)chunk * FCHUNK, k1 = min(k0 + FCHUNK, P.n_pairs);
+        for (int64_t k = k0; k < k1; ++k) {
+            const int2 e = ((const int2 *)P.pq)[k];
+            const int p = e.x, q = e.y;
+            if (p != head_p) { hp = P.prep.head[p]; head_p = p; }
+            const ForestHead hq = P.prep.head[q];
+            const int mp = hp.len, mq = hq.len;
+            double s, c;
+            lya_pair_sc(hp.ux, hp.uy, hp.uz, hq.ux, hq.uy, hq.uz, s, c);
+            const PairBin g = lya_make_pairbin(bp, s, c);
+            int c0;
+            const int key = lya_pair_key<POW2>(bp, g, hp, hq, c0);
+            if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
+            since_merge += (unsigned long long)mp * mq;
+            if (c0 != win_c0 || since_merge > (1ull << 31)) {
+                if (win_c0 >= 0) xi_merge(ws, P, win_c0, lane);
+                win_c0 = c0; since_merge = (unsigned long long)mp * mq;
+            }
+            __syncwarp();
+            if (p != cur_p) {
+                const double2 *sc = (const double2 *)(P.prep.chi + hp.off), *sa = (const double2 *)(P.prep.a + hp.off),
+                              *sw = (const double2 *)(P.prep.w + hp.off);
+                for (int t = lane; 2 * t < mp; t += 32) {
+                    ((double2 *)ws.pc)[t] = sc[t]; ((double2 *)ws.pa)[t] = sa[t]; ((double2 *)ws.pw)[t] = sw[t];
+                }
+                cur_p = p;
+            }
+            {
+                const double2 *sc = (const double2 *)(P.prep.chi + hq.off), *sa = (const double2 *)(P.prep.a + hq.off),
+                              *sw = (const double2 *)(P.prep.w + hq.off);
+                const int npad2 = (mq + 1) >> 1;
+                for (int t = lane; t < npad2; t += 32) {
+                    ((double2 *)qc)[t] = sc[t]; ((double2 *)(ws.qa + FPAD))[t] = sa[t]; ((double2 *)(ws.qw + FPAD))[t] = sw[t];
+                }
+                if (lane < FPAD) {                           // right sentinels (the pad pixel of an odd forest is one already)
+                    const int j = 2 * npad2 + lane;
+                    ws.qc[FPAD + j] = LYA_CHI_SENTINEL; ws.qa[FPAD + j] = 0.0; ws.qw[FPAD + j] = 0.0;
+                }
+            }
+            __syncwarp();
+            // chi window of r_par < rpar_max (conservative superset) and the sign change, per row of p
+            const double R = (c > 0.0) ? (bp.rpar_max / c) * (1.0 + 1e-12) + 1e-9 : 1e300;
+            const double Tchi = (s > 0.0) ? (bp.rperp_max / s) * (1.0 + 1e-12) + 1e-9 : 1e300;
+            int pos_lo = 1 << 20, pos_hi = -(1 << 20), neg_lo = 1 << 20, neg_hi = -(1 << 20);
+            for (int i = lane; i < mp; i += 32) {
+                const double x = ws.pc[i];
+                int lo = 0, hi = mq;                         // first j with qc[j] > x - R
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x - R) hi = mid; else lo = mid + 1; }
+                const int jlo = lo;
+                hi = mq;                                     // first j with qc[j] > x  (chi_i >= chi_j below it)
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x) hi = mid; else lo = mid + 1; }
+                const int jx = lo;
+                hi = mq;                                     // first j with qc[j] >= x + R
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] >= x + R) hi = mid; else lo = mid + 1; }
+                const int jhi = lo;
+                if (jx > jlo) { pos_lo = min(pos_lo, jlo - i); pos_hi = max(pos_hi, jx - 1 - i); }
+                if (jhi > jx) { neg_lo = min(neg_lo, jx - i); neg_hi = max(neg_hi, jhi - 1 - i); }
+            }
+            pos_lo = __reduce_min_sync(0xffffffffu, pos_lo); pos_hi = __reduce_max_sync(0xffffffffu, pos_hi);
+            neg_lo = __reduce_min_sync(0xffffffffu, neg_lo); neg_hi = __reduce_max_sync(0xffffffffu, neg_hi);
+            xi_walk_any<POW2>(ws, mp, mq, pos_lo, pos_hi, 0, Tchi, bp, g, c0, lane, evaluated);
+            xi_walk_any<POW2>(ws, mp, mq, neg_lo, neg_hi, -1, Tchi, bp, g, c0, lane, evaluated);
+        }
+    }
+    if (win_c0 >= 0) xi_merge(ws, P, win_c0, lane);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
+    if (lane == 0 && evaluated) atomicAdd(&P.counters[2], evaluated);
+}
+
 }  // namespace
 
 extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
@@ -273,50 +537,86 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
 
     const int nb = b->n_par * b->n_perp;
     cudaStream_t s = ctx->stream;
+    const BinParams bp = lya_make_binparams(b);
+    // fast path: bucketed list + warp-private sub-histograms (variant 9 forces the generic kernel)
+    const bool use_fast = pairs->n > 0 && b->n_par * LYA_NCOL <= FSLOTS && b->n_perp + 2 <= 256 && ctx->xi_variant != 9;
+    LyaPrep prep;
+    LyaBuckets bk;
+    memset(&prep, 0, sizeof(prep));
+    memset(&bk, 0, sizeof(bk));
     double *acc = NULL;                         // [S | W | N] accumulators
-    LYA_CUDA(cudaMalloc(&acc, (size_t)nb * 24));
+    auto cleanup = [&]() { cudaFree(acc); lya_prep_free(&prep); lya_buckets_free(&bk); };
+    cudaEventRecord(ctx->ev[3], s);
+    if (use_fast) {
+        st = lya_prep_build(ctx, f, true, false, &prep);
+        if (st) return st;
+        cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
+        st = lya_bucket_pairs(ctx, &prep, &bp, pairs, 0, &bk);
+        if (st) { cleanup(); return st; }
+        if (bk.bad_pair) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
+    }
+    cudaError_t e = cudaMalloc(&acc, (size_t)nb * 24);
+    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(xi accumulators)"); }
     cudaMemsetAsync(acc, 0, (size_t)nb * 24, s);
     cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
 
     XiParams P;
     P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.delta = f->delta;
     P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
-    P.pq = pairs->pq; P.n_pairs = pairs->n; P.n_forest = f->n_forest;
-    P.bp = lya_make_binparams(b);
+    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pairs->pq;
+    P.n_pairs = use_fast ? bk.n_generic : pairs->n;
+    P.n_forest = f->n_forest;
+    P.bp = bp;
     P.S = acc; P.W = acc + nb; P.N = (unsigned long long *)(acc + 2 * nb);
     P.counters = ctx->d_counters;
 
+    cudaEventRecord(ctx->ev[0], s);
+    if (use_fast && bk.n_fast > 0) {
+        XiFastParams F;
+        F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
+        F.S = P.S; F.W = P.W; F.N = P.N; F.counters = ctx->d_counters;
+        const size_t fsmem = sizeof(FastWarp) * FW;
+        const int fgrid = ctx->sm_count * 2;
+        if (bp.pow2) {
+            e = cudaFuncSetAttribute(k_xi_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
+            if (e == cudaSuccess) k_xi_fast<true><<<fgrid, FTHREADS, fsmem, s>>>(F);
+        } else {
+            e = cudaFuncSetAttribute(k_xi_fast<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
+            if (e == cudaSuccess) k_xi_fast<false><<<fgrid, FTHREADS, fsmem, s>>>(F);
+        }
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_fast launch"); }
+    }
     const size_t smem = (((size_t)nb * 20 + 15) & ~(size_t)15) + sizeof(WarpSmem) * XI_WARPS;
     const int grid = ctx->sm_count * 2;
-    const int64_t n_chunks = (pairs->n + CHUNK - 1) / CHUNK;
-    cudaEventRecord(ctx->ev[0], s);
+    const int64_t n_chunks = (P.n_pairs + CHUNK - 1) / CHUNK;
     int launches = 0;
     unsigned long long h[4] = {0, 0, 0, 0};
-    while (pairs->n > 0) {
-        cudaError_t e;
+    while (P.n_pairs > 0) {
         switch (ctx->xi_variant) {
         case 1: e = launch_xi<1>(P, grid, smem, s); break;
         case 4: e = launch_xi<4>(P, grid, smem, s); break;
         default: e = launch_xi<2>(P, grid, smem, s); break;
         }
-        if (e != cudaSuccess) { cudaFree(acc); return lya_cuda_fail(ctx, e, "k_xi launch"); }
+        if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi launch"); }
         ++launches;
         e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        if (e != cudaSuccess) { cudaFree(acc); return lya_cuda_fail(ctx, e, "k_xi"); }
+        if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi"); }
         if ((int64_t)h[0] >= n_chunks) break;      // every chunk claimed (warps stop at their u32 budget)
-        if (launches > 100000) { cudaFree(acc); return lya_fail(ctx, LYA_ERR_CUDA, "k_xi made no progress"); }
+        if (launches > 100000) { cleanup(); return lya_fail(ctx, LYA_ERR_CUDA, "k_xi made no progress"); }
     }
     cudaEventRecord(ctx->ev[1], s);
     k_xi_finalize<<<(nb + 255) / 256, 256, 0, s>>>(P.S, P.W, P.N, nb, S, W, (unsigned long long *)N, xi);
     cudaEventRecord(ctx->ev[2], s);
-    cudaError_t e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) { cudaFree(acc); return lya_cuda_fail(ctx, e, "lya_xi2pcf"); }
-    if (h[3] != 0) { cudaFree(acc); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
+    e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "lya_xi2pcf"); }
+    if (h[3] != 0) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
     if (stats) {
         memset(stats, 0, sizeof(*stats));
         stats->n_forest_pairs = (uint64_t)pairs->n;
-        stats->n_visited = h[1];
+        stats->n_visited = use_fast ? bk.visited : h[1];
         stats->n_evaluated = h[2];
         // n_binned = sum N: small D2H
         unsigned long long *hN = (unsigned long long *)malloc(sizeof(unsigned long long) * nb);
@@ -324,8 +624,8 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
             for (int k = 0; k < nb; ++k) stats->n_binned += hN[k];
         free(hN);
         cudaEventElapsedTime(&stats->ms_main, ctx->ev[0], ctx->ev[1]);
-        cudaEventElapsedTime(&stats->ms_total, ctx->ev[0], ctx->ev[2]);
+        cudaEventElapsedTime(&stats->ms_total, ctx->ev[3], ctx->ev[2]);
     }
-    cudaFree(acc);
+    cleanup();
     return LYA_OK;
 }
