@@ -74,8 +74,8 @@ void lya_prep_free(LyaPrep *p);
 // pixel pair (c_first).  Keys: 0..n_perp-1 = fast-path pairs whose bins lie in columns
 // [c_first, c_first + LYA_NCOL); n_perp = pairs for the generic kernels (long forests, wide
 // column span, spacing below the bin width); n_perp+1 = pairs with nothing inside the grid.
-#define LYA_NCOL 8                  // r_perp columns of a warp-private sub-histogram
-#define LYA_FAST_TILE 80            // longest forest the fast kernels stage in one piece
+#define LYA_NCOL 6                  // r_perp columns of a warp-private sub-histogram
+#define LYA_FAST_TILE 72            // longest forest the fast kernels stage in one piece
 struct LyaBuckets {
     int32_t *pq;                    // device [n][2], sorted by key (stable)
     int64_t n;

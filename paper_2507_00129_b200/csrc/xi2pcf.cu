@@ -265,12 +265,13 @@ cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
 }
 
 // ======================= fast kernel: warp-private sub-histograms ================================
-constexpr int FW = 8;                        // warps per block
+constexpr int FW = 6;                        // warps per block
 constexpr int FTHREADS = FW * 32;
 constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
 constexpr int FPAD = 2;                      // sentinel pixels either side of q (reads are clamped)
-constexpr int FSLOTS = 400;                  // n_par * LYA_NCOL <= FSLOTS
+constexpr int FSLOTS = 714;                  // 2 * (n_par + 1) * (LYA_NCOL + 1) <= FSLOTS
 constexpr int FCHUNK = 16;                   // forest pairs claimed per atomic
+constexpr int FROWS = 16;                    // rows of p walked per pass (keeps lanes busy: DESIGN.md)
 
 struct XiFastParams {
     LyaPrep prep;
@@ -282,146 +283,161 @@ struct XiFastParams {
     unsigned long long *counters;            // [4] next chunk, [2] evaluated
 };
 
+// Sub-histogram slot = col_rel * 2 (n_par + 1) + side * (n_par + 1) + row.
+//   side: 0 when chi_i >= chi_j, 1 otherwise (the two sides of a bin are added when the warp merges);
+//   row n_par and col_rel LYA_NCOL are GARBAGE (pixel pair outside the grid / a sentinel pixel), so
+//   the pair loop needs no validity test; garbage slots are dropped by the merge.
 struct __align__(16) FastWarp {
+    double2 SW[FSLOTS];                      // (S, W) per slot
+    unsigned N[(FSLOTS + 3) & ~3];           // (padded: the arrays below need 16-byte alignment)
     double pc[FT], pa[FT], pw[FT];
     double qc[FT + 2 * FPAD], qa[FT + 2 * FPAD], qw[FT + 2 * FPAD];
-    double2 SW[FSLOTS];
-    unsigned N[FSLOTS];
+    unsigned char jlo[FT], jhi[FT];          // per row of p: window [jlo, jhi) of q that can be in the grid
 };
 
-// slot of a pixel pair in the sub-histogram whose first column is c0, -1 outside the grid
-// or on the wrong side of chi_i = chi_j (sgn = 0: chi_i >= chi_j, sgn = -1: chi_i < chi_j).
+// ---- predicated shared-memory accesses (no divergence in the pair loop) ----
+__device__ __forceinline__ void sts_v2_if(bool p, unsigned addr, double x, double y)
+{
+    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q st.shared.v2.f64 [%1], {%2, %3};\n}"
+                 :: "r"((unsigned)p), "r"(addr), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void lds_v2_if(bool p, unsigned addr, double &x, double &y)
+{
+    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %2, 0;\n @q ld.shared.v2.f64 {%0, %1}, [%3];\n}"
+                 : "+d"(x), "+d"(y) : "r"((unsigned)p), "r"(addr) : "memory");
+}
+__device__ __forceinline__ void red_u32_if(bool p, unsigned addr, unsigned v)
+{
+    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q red.shared.add.u32 [%1], %2;\n}"
+                 :: "r"((unsigned)p), "r"(addr), "r"(v) : "memory");
+}
+
+// byte offset (16 * slot) of a pixel pair's sub-histogram entry
 template <bool POW2>
-__device__ __forceinline__ int xi_slot(const BinParams &bp, const PairBin &g, double chi_i, double chi_j, int c0, int sgn)
+__device__ __forceinline__ unsigned xi_key(const BinParams &bp, const PairBin &g, double chi_i, double chi_j, unsigned c0,
+                                           unsigned np1)
 {
     const double d = __dsub_rn(chi_i, chi_j);
     const double t = __dadd_rn(chi_i, chi_j);
-    const bool side = ((__double2hiint(d) ^ sgn) >= 0);
     unsigned bx, by;
-    bool ok;
     if (POW2) {
         bx = lya_floor_u32(__dmul_rn(fabs(d), g.cx));
         by = lya_floor_u32(__dmul_rn(t, g.sy));
-        ok = (bx < (unsigned)bp.n_par) & (by < (unsigned)bp.n_perp);
     } else {
         const double rpar = __dmul_rn(fabs(d), g.c), rperp = __dmul_rn(t, g.s);
-        ok = (rpar < bp.rpar_max) & (rperp < bp.rperp_max);
-        bx = min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1));
-        by = min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1));
+        bx = (rpar < bp.rpar_max) ? min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1)) : (unsigned)bp.n_par;
+        by = (rperp < bp.rperp_max) ? min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1)) : 0x7fffffffu;
     }
-    return (ok & side) ? (int)(bx * LYA_NCOL + by) - c0 : -1;
+    bx = min(bx, np1 - 1u);
+    const unsigned col = min(by - c0, (unsigned)LYA_NCOL);
+    const unsigned side = (unsigned)__double2hiint(d) >> 31;
+    return (col * (2u * np1) + side * np1 + bx) * 16u;
 }
 
-// Walk the diagonals [dlo, dhi] of a staged forest pair, D adjacent diagonals per lane.
+// Walk rows [r0, r1] of p against the diagonals [dlo, dhi], D adjacent diagonals per lane.
+// Each lane HOLDS the sub-histogram entry of its current run in registers: when the key changes it
+// stores the entry back (release) and loads the new one (acquire), both predicated.  The lanes of a
+// row hold pixel pairs (i, j_lane) with distinct j on their side of chi_i = chi_j, hence distinct
+// entries (lya_pair_key: q's spacing exceeds the r_par bin width), so an entry has one holder at a
+// time; all releases of a row come before its acquires (warp barrier in between).
 template <int D, bool POW2>
-__device__ __forceinline__ void xi_walk(FastWarp &ws, int mp, int mq, int dlo, int dhi, int sgn, double Tchi,
-                                        const BinParams &bp, const PairBin &g, int c0, int lane,
-                                        unsigned long long &evaluated)
+__device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
+                                        int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
+                                        unsigned np1, int lane, unsigned long long &evaluated)
 {
     const double *qc = ws.qc + FPAD, *qa = ws.qa + FPAD, *qw = ws.qw + FPAD;
+    const unsigned garbage = (LYA_NCOL * 2u * np1 + np1 - 1u) * 16u;  // what a sentinel pixel maps to
     for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
         const int dl = d0 + lane * D;                       // first diagonal of this lane
-        const int dpass_hi = min(dhi, d0 + 32 * D - 1);
-        const int i_begin = max(0, -dpass_hi);
-        int i_end = min(mp, mq - d0);                       // exclusive
-        if (i_end <= i_begin) continue;
-        {   // rows past r_perp_max: chi_p[i] + chi_q[i + d] grows with i and with d, so the first
-            // diagonal of the pass decides (Tchi is a conservative rperp_max / s)
-            int lo = i_begin, hi = i_end;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (ws.pc[mid] + qc[max(mid + d0, 0)] >= Tchi) hi = mid; else lo = mid + 1;
-            }
-            i_end = lo;
-        }
-        if (i_end <= i_begin) continue;
-        int cur[D]; double accS[D], accW[D]; unsigned cnt[D];
+        unsigned cur[D];
+        int i0[D];
+        double accS[D], accW[D];
         double wc[D], wa[D], ww[D];                         // sliding window over q
 #pragma unroll
-        for (int k = 0; k < D; ++k) { cur[k] = -1; accS[k] = 0.0; accW[k] = 0.0; cnt[k] = 0; }
+        for (int k = 0; k < D; ++k) { cur[k] = garbage; i0[k] = r0; accS[k] = 0.0; accW[k] = 0.0; }
 #pragma unroll
         for (int k = 0; k < D - 1; ++k) {
-            const int j = min(max(i_begin + dl + k, -FPAD), mq + FPAD - 1);
+            const int j = min(max(r0 + dl + k, -FPAD), mq + FPAD - 1);
             wc[k] = qc[j]; wa[k] = qa[j]; ww[k] = qw[j];
         }
-        evaluated += (unsigned long long)(i_end - i_begin) * D;
-        for (int ib = i_begin; ib < i_end; ib += D) {
+        evaluated += (unsigned long long)(r1 - r0 + 1) * D;
+        for (int ib = r0; ib <= r1; ib += D) {
 #pragma unroll
             for (int u = 0; u < D; ++u) {
                 const int i = ib + u;
-                if (i < i_end) {                            // warp-uniform
+                if (i <= r1) {                              // warp-uniform
                     const double pci = ws.pc[i], pai = ws.pa[i], pwi = ws.pw[i];
                     {   // the new q pixel of the lane's last diagonal goes into slot (u + D - 1) % D
                         const int j = min(max(i + dl + D - 1, -FPAD), mq + FPAD - 1);
                         wc[(u + D - 1) % D] = qc[j]; wa[(u + D - 1) % D] = qa[j]; ww[(u + D - 1) % D] = qw[j];
                     }
+                    unsigned key[D];
+                    bool ch[D];
+#pragma unroll
+                    for (int k = 0; k < D; ++k) {
+                        key[k] = xi_key<POW2>(bp, g, pci, wc[(k + u) % D], c0, np1);
+                        ch[k] = key[k] != cur[k];
+                        sts_v2_if(ch[k], sw_base + cur[k], accS[k], accW[k]);                 // release
+                        red_u32_if(ch[k], n_base + (cur[k] >> 2), (unsigned)(i - i0[k]));
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int k = 0; k < D; ++k) {
+                        lds_v2_if(ch[k], sw_base + key[k], accS[k], accW[k]);                 // acquire
+                        cur[k] = key[k];
+                        i0[k] = ch[k] ? i : i0[k];
+                    }
 #pragma unroll
                     for (int k = 0; k < D; ++k) {
                         const int sl = (k + u) % D;         // slot holding q[i + dl + k]
-                        const int key = xi_slot<POW2>(bp, g, pci, wc[sl], c0, sgn);
-                        if (key != cur[k]) {
-                            if (cur[k] >= 0) {              // plain RMW: lanes of one row step hold distinct bins
-                                double2 v = ws.SW[cur[k]];
-                                v.x += accS[k]; v.y += accW[k];
-                                ws.SW[cur[k]] = v;
-                                atomicAdd(&ws.N[cur[k]], cnt[k]);
-                            }
-                            cur[k] = key; accS[k] = 0.0; accW[k] = 0.0; cnt[k] = 0;
-                        }
-                        if (key >= 0) {
-                            accS[k] = fma(pai, wa[sl], accS[k]);
-                            accW[k] = fma(pwi, ww[sl], accW[k]);
-                            cnt[k] += 1;
-                        }
+                        accS[k] = fma(pai, wa[sl], accS[k]);
+                        accW[k] = fma(pwi, ww[sl], accW[k]);
                     }
-                    __syncwarp();                           // order this row step's RMWs before the next one's
                 }
             }
         }
+        // release what the lanes still hold
 #pragma unroll
-        for (int k = 0; k < D; ++k)
-            if (cur[k] >= 0) {
-                double2 v = ws.SW[cur[k]];
-                v.x += accS[k]; v.y += accW[k];
-                ws.SW[cur[k]] = v;
-                atomicAdd(&ws.N[cur[k]], cnt[k]);
-            }
+        for (int k = 0; k < D; ++k) {
+            sts_v2_if(true, sw_base + cur[k], accS[k], accW[k]);
+            red_u32_if(true, n_base + (cur[k] >> 2), (unsigned)(r1 + 1 - i0[k]));
+        }
         __syncwarp();
     }
 }
 
 template <bool POW2>
-__device__ __forceinline__ void xi_walk_any(FastWarp &ws, int mp, int mq, int dlo, int dhi, int sgn, double Tchi,
-                                            const BinParams &bp, const PairBin &g, int c0, int lane,
-                                            unsigned long long &evaluated)
+__device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
+                                            int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
+                                            unsigned np1, int lane, unsigned long long &evaluated)
 {
-    if (dhi < dlo) return;
     const int nd = dhi - dlo + 1;
-    if (nd <= 32) xi_walk<1, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
-    else if (nd <= 64) xi_walk<2, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
-    else if (nd <= 96) xi_walk<3, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
-    else xi_walk<4, POW2>(ws, mp, mq, dlo, dhi, sgn, Tchi, bp, g, c0, lane, evaluated);
+    if (nd <= 32) xi_walk<1, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
+    else if (nd <= 64) xi_walk<2, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
+    else if (nd <= 96) xi_walk<3, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
+    else xi_walk<4, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
 }
 
 // merge a warp's sub-histogram (first column c0) into the global accumulators and clear it
 __device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, int c0, int lane)
 {
-    const int n_slots = P.bp.n_par * LYA_NCOL;
+    const int np1 = P.bp.n_par + 1;
     __syncwarp();
-    for (int t = lane; t < n_slots; t += 32) {
-        const unsigned n = ws.N[t];
+    for (int t = lane; t < np1 * (LYA_NCOL + 1); t += 32) {      // t = col_rel * np1 + row
+        const int cr = t / np1, bx = t - cr * np1, col = c0 + cr;
+        const int s0 = cr * 2 * np1 + bx, s1 = s0 + np1;          // the two sides of the bin
+        const unsigned n = ws.N[s0] + ws.N[s1];
         if (n) {
-            const int bx = t / LYA_NCOL, col = c0 + (t - bx * LYA_NCOL);
-            const double2 v = ws.SW[t];
-            if (col < P.bp.n_perp) {
+            if (bx < P.bp.n_par && cr < LYA_NCOL && col < P.bp.n_perp) {
+                const double2 v0 = ws.SW[s0], v1 = ws.SW[s1];
                 const int A = bx * P.bp.n_perp + col;
                 atomicAdd(&P.N[A], (unsigned long long)n);
-                atomicAdd(&P.S[A], v.x);
-                atomicAdd(&P.W[A], v.y);
+                atomicAdd(&P.S[A], v0.x + v1.x);
+                atomicAdd(&P.W[A], v0.y + v1.y);
             }
-            ws.SW[t] = make_double2(0.0, 0.0);
-            ws.N[t] = 0u;
+            ws.N[s0] = 0u; ws.N[s1] = 0u;
         }
+        ws.SW[s0] = make_double2(0.0, 0.0); ws.SW[s1] = make_double2(0.0, 0.0);
     }
     __syncwarp();
 }
@@ -433,11 +449,13 @@ __global__ void __launch_bounds__(FTHREADS, 2) k_xi_fast(XiFastParams P)
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     FastWarp &ws = ((FastWarp *)smem_raw)[wid];
     const BinParams bp = P.bp;
+    const unsigned np1 = (unsigned)bp.n_par + 1u;
     for (int t = lane; t < FSLOTS; t += 32) { ws.SW[t] = make_double2(0.0, 0.0); ws.N[t] = 0u; }
     if (lane < FPAD) { ws.qc[lane] = LYA_CHI_SENTINEL; ws.qa[lane] = 0.0; ws.qw[lane] = 0.0; }
     __syncwarp();
 
     const double *qc = ws.qc + FPAD;
+    const unsigned sw_base = (unsigned)__cvta_generic_to_shared(ws.SW), n_base = (unsigned)__cvta_generic_to_shared(ws.N);
     unsigned long long evaluated = 0, since_merge = 0;
     int cur_p = -1, head_p = -1, win_c0 = -1;
     ForestHead hp;
@@ -488,28 +506,33 @@ __global__ void __launch_bounds__(FTHREADS, 2) k_xi_fast(XiFastParams P)
                 }
             }
             __syncwarp();
-            // chi window of r_par < rpar_max (conservative superset) and the sign change, per row of p
+            // per row of p: the window of q with r_par < rpar_max and r_perp < rperp_max (conservative superset)
             const double R = (c > 0.0) ? (bp.rpar_max / c) * (1.0 + 1e-12) + 1e-9 : 1e300;
             const double Tchi = (s > 0.0) ? (bp.rperp_max / s) * (1.0 + 1e-12) + 1e-9 : 1e300;
-            int pos_lo = 1 << 20, pos_hi = -(1 << 20), neg_lo = 1 << 20, neg_hi = -(1 << 20);
             for (int i = lane; i < mp; i += 32) {
                 const double x = ws.pc[i];
                 int lo = 0, hi = mq;                         // first j with qc[j] > x - R
                 while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x - R) hi = mid; else lo = mid + 1; }
                 const int jlo = lo;
-                hi = mq;                                     // first j with qc[j] > x  (chi_i >= chi_j below it)
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x) hi = mid; else lo = mid + 1; }
-                const int jx = lo;
-                hi = mq;                                     // first j with qc[j] >= x + R
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] >= x + R) hi = mid; else lo = mid + 1; }
-                const int jhi = lo;
-                if (jx > jlo) { pos_lo = min(pos_lo, jlo - i); pos_hi = max(pos_hi, jx - 1 - i); }
-                if (jhi > jx) { neg_lo = min(neg_lo, jx - i); neg_hi = max(neg_hi, jhi - 1 - i); }
+                const double top = fmin(x + R, Tchi - x);    // first j with qc[j] >= top
+                hi = mq;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] >= top) hi = mid; else lo = mid + 1; }
+                ws.jlo[i] = (unsigned char)jlo;
+                ws.jhi[i] = (unsigned char)lo;
             }
-            pos_lo = __reduce_min_sync(0xffffffffu, pos_lo); pos_hi = __reduce_max_sync(0xffffffffu, pos_hi);
-            neg_lo = __reduce_min_sync(0xffffffffu, neg_lo); neg_hi = __reduce_max_sync(0xffffffffu, neg_hi);
-            xi_walk_any<POW2>(ws, mp, mq, pos_lo, pos_hi, 0, Tchi, bp, g, c0, lane, evaluated);
-            xi_walk_any<POW2>(ws, mp, mq, neg_lo, neg_hi, -1, Tchi, bp, g, c0, lane, evaluated);
+            __syncwarp();
+            // walk FROWS rows at a time over exactly the diagonals those rows need
+            for (int i0 = 0; i0 < mp; i0 += FROWS) {
+                const int i = i0 + lane;
+                int dlo = 1 << 20, dhi = -(1 << 20), r0 = 1 << 20, r1 = -1;
+                if (lane < FROWS && i < mp) {
+                    const int jl = ws.jlo[i], jh = ws.jhi[i];
+                    if (jh > jl) { dlo = jl - i; dhi = jh - 1 - i; r0 = i; r1 = i; }
+                }
+                dlo = __reduce_min_sync(0xffffffffu, dlo); dhi = __reduce_max_sync(0xffffffffu, dhi);
+                r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
+                if (r1 >= r0) xi_walk_any<POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated);
+            }
         }
     }
     if (win_c0 >= 0) xi_merge(ws, P, win_c0, lane);
@@ -539,7 +562,7 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
     cudaStream_t s = ctx->stream;
     const BinParams bp = lya_make_binparams(b);
     // fast path: bucketed list + warp-private sub-histograms (variant 9 forces the generic kernel)
-    const bool use_fast = pairs->n > 0 && b->n_par * LYA_NCOL <= FSLOTS && b->n_perp + 2 <= 256 && ctx->xi_variant != 9;
+    const bool use_fast = pairs->n > 0 && 2 * (b->n_par + 1) * (LYA_NCOL + 1) <= FSLOTS && b->n_perp + 2 <= 256 && ctx->xi_variant != 9;
     LyaPrep prep;
     LyaBuckets bk;
     memset(&prep, 0, sizeof(prep));
