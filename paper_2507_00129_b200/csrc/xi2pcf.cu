@@ -268,10 +268,11 @@ cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
 constexpr int FW = 6;                        // warps per block
 constexpr int FTHREADS = FW * 32;
 constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
+constexpr int FROWS = 16;                    // rows of p walked per pass (keeps lanes busy: DESIGN.md)
+constexpr int FTP = ((FT + FROWS - 1) / FROWS) * FROWS + 2;   // p rows incl. sentinel rows
 constexpr int FPAD = 2;                      // sentinel pixels either side of q (reads are clamped)
 constexpr int FSLOTS = 714;                  // 2 * (n_par + 1) * (LYA_NCOL + 1) <= FSLOTS
 constexpr int FCHUNK = 16;                   // forest pairs claimed per atomic
-constexpr int FROWS = 16;                    // rows of p walked per pass (keeps lanes busy: DESIGN.md)
 
 struct XiFastParams {
     LyaPrep prep;
@@ -290,7 +291,7 @@ struct XiFastParams {
 struct __align__(16) FastWarp {
     double2 SW[FSLOTS];                      // (S, W) per slot
     unsigned N[(FSLOTS + 3) & ~3];           // (padded: the arrays below need 16-byte alignment)
-    double pc[FT], pa[FT], pw[FT];
+    double pc[FTP], pa[FTP], pw[FTP];        // rows >= len are sentinels (walks cover whole row groups)
     double qc[FT + 2 * FPAD], qa[FT + 2 * FPAD], qw[FT + 2 * FPAD];
     unsigned char jlo[FT], jhi[FT];          // per row of p: window [jlo, jhi) of q that can be in the grid
 };
@@ -306,10 +307,15 @@ __device__ __forceinline__ void lds_v2_if(bool p, unsigned addr, double &x, doub
     asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %2, 0;\n @q ld.shared.v2.f64 {%0, %1}, [%3];\n}"
                  : "+d"(x), "+d"(y) : "r"((unsigned)p), "r"(addr) : "memory");
 }
-__device__ __forceinline__ void red_u32_if(bool p, unsigned addr, unsigned v)
+__device__ __forceinline__ void sts_u32_if(bool p, unsigned addr, unsigned v)
 {
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q red.shared.add.u32 [%1], %2;\n}"
+    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q st.shared.u32 [%1], %2;\n}"
                  :: "r"((unsigned)p), "r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void lds_u32_if(bool p, unsigned addr, unsigned &v)
+{
+    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %1, 0;\n @q ld.shared.u32 %0, [%2];\n}"
+                 : "+r"(v) : "r"((unsigned)p), "r"(addr) : "memory");
 }
 
 // byte offset (16 * slot) of a pixel pair's sub-histogram entry
@@ -335,11 +341,13 @@ __device__ __forceinline__ unsigned xi_key(const BinParams &bp, const PairBin &g
 }
 
 // Walk rows [r0, r1] of p against the diagonals [dlo, dhi], D adjacent diagonals per lane.
-// Each lane HOLDS the sub-histogram entry of its current run in registers: when the key changes it
-// stores the entry back (release) and loads the new one (acquire), both predicated.  The lanes of a
-// row hold pixel pairs (i, j_lane) with distinct j on their side of chi_i = chi_j, hence distinct
-// entries (lya_pair_key: q's spacing exceeds the r_par bin width), so an entry has one holder at a
-// time; all releases of a row come before its acquires (warp barrier in between).
+// Each lane HOLDS the sub-histogram entry (S, W, N) of its current run in registers: when the key
+// changes it stores the entry back (release) and loads the new one (acquire), both predicated, so the
+// loop has no divergent branch.  The lanes of a row hold pixel pairs (i, j_lane) with distinct j on
+// their side of chi_i = chi_j, hence distinct entries (lya_pair_key: q's spacing exceeds the r_par bin
+// width), so an entry has one holder at a time; all releases of a row come before its acquires (warp
+// barrier in between).  The keys of row i+1 are computed between the acquire of row i and the FMAs
+// that need it.  r1 - r0 + 1 is a multiple of D; rows >= mp of p are sentinels.
 template <int D, bool POW2>
 __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
                                         int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
@@ -349,58 +357,71 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
     const unsigned garbage = (LYA_NCOL * 2u * np1 + np1 - 1u) * 16u;  // what a sentinel pixel maps to
     for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
         const int dl = d0 + lane * D;                       // first diagonal of this lane
-        unsigned cur[D];
-        int i0[D];
-        double accS[D], accW[D];
+        unsigned cur[D], cnt[D], key[D];
+        double accS[D], accW[D], fa[D], fw[D];
         double wc[D], wa[D], ww[D];                         // sliding window over q
+        double pa_c, pw_c;
 #pragma unroll
-        for (int k = 0; k < D; ++k) { cur[k] = garbage; i0[k] = r0; accS[k] = 0.0; accW[k] = 0.0; }
+        for (int k = 0; k < D; ++k) { cur[k] = garbage; cnt[k] = 0u; accS[k] = 0.0; accW[k] = 0.0; }
+        {   // prologue: window and keys of row r0
 #pragma unroll
-        for (int k = 0; k < D - 1; ++k) {
-            const int j = min(max(r0 + dl + k, -FPAD), mq + FPAD - 1);
-            wc[k] = qc[j]; wa[k] = qa[j]; ww[k] = qw[j];
+            for (int k = 0; k < D; ++k) {
+                const int j = min(max(r0 + dl + k, -FPAD), mq + FPAD - 1);
+                wc[k] = qc[j]; wa[k] = qa[j]; ww[k] = qw[j];
+            }
+            const double pci = ws.pc[r0];
+            pa_c = ws.pa[r0]; pw_c = ws.pw[r0];
+#pragma unroll
+            for (int k = 0; k < D; ++k) { key[k] = xi_key<POW2>(bp, g, pci, wc[k], c0, np1); fa[k] = wa[k]; fw[k] = ww[k]; }
         }
         evaluated += (unsigned long long)(r1 - r0 + 1) * D;
         for (int ib = r0; ib <= r1; ib += D) {
 #pragma unroll
             for (int u = 0; u < D; ++u) {
-                const int i = ib + u;
-                if (i <= r1) {                              // warp-uniform
-                    const double pci = ws.pc[i], pai = ws.pa[i], pwi = ws.pw[i];
-                    {   // the new q pixel of the lane's last diagonal goes into slot (u + D - 1) % D
-                        const int j = min(max(i + dl + D - 1, -FPAD), mq + FPAD - 1);
-                        wc[(u + D - 1) % D] = qc[j]; wa[(u + D - 1) % D] = qa[j]; ww[(u + D - 1) % D] = qw[j];
-                    }
-                    unsigned key[D];
-                    bool ch[D];
+                const int i = ib + u;                       // window slot of q[i + dl + k] is (k + u) % D
+                bool ch[D];
+#pragma unroll
+                for (int k = 0; k < D; ++k) {
+                    ch[k] = key[k] != cur[k];
+                    sts_v2_if(ch[k], sw_base + cur[k], accS[k], accW[k]);                 // release
+                    sts_u32_if(ch[k], n_base + (cur[k] >> 2), cnt[k]);
+                }
+                __syncwarp();
+#pragma unroll
+                for (int k = 0; k < D; ++k) {
+                    lds_v2_if(ch[k], sw_base + key[k], accS[k], accW[k]);                 // acquire
+                    lds_u32_if(ch[k], n_base + (key[k] >> 2), cnt[k]);
+                    cur[k] = key[k];
+                }
+                // row i + 1: its new q pixel replaces q[i + dl] in window slot u
+                double fa_n[D], fw_n[D];
+                unsigned key_n[D];
+                {
+                    const int j = min(max(i + dl + D, -FPAD), mq + FPAD - 1);
+                    wc[u] = qc[j]; wa[u] = qa[j]; ww[u] = qw[j];
+                    const double pci = ws.pc[i + 1];
 #pragma unroll
                     for (int k = 0; k < D; ++k) {
-                        key[k] = xi_key<POW2>(bp, g, pci, wc[(k + u) % D], c0, np1);
-                        ch[k] = key[k] != cur[k];
-                        sts_v2_if(ch[k], sw_base + cur[k], accS[k], accW[k]);                 // release
-                        red_u32_if(ch[k], n_base + (cur[k] >> 2), (unsigned)(i - i0[k]));
-                    }
-                    __syncwarp();
-#pragma unroll
-                    for (int k = 0; k < D; ++k) {
-                        lds_v2_if(ch[k], sw_base + key[k], accS[k], accW[k]);                 // acquire
-                        cur[k] = key[k];
-                        i0[k] = ch[k] ? i : i0[k];
-                    }
-#pragma unroll
-                    for (int k = 0; k < D; ++k) {
-                        const int sl = (k + u) % D;         // slot holding q[i + dl + k]
-                        accS[k] = fma(pai, wa[sl], accS[k]);
-                        accW[k] = fma(pwi, ww[sl], accW[k]);
+                        const int sl = (k + u + 1) % D;
+                        key_n[k] = xi_key<POW2>(bp, g, pci, wc[sl], c0, np1);
+                        fa_n[k] = wa[sl]; fw_n[k] = ww[sl];
                     }
                 }
+#pragma unroll
+                for (int k = 0; k < D; ++k) {
+                    accS[k] = fma(pa_c, fa[k], accS[k]);
+                    accW[k] = fma(pw_c, fw[k], accW[k]);
+                    cnt[k] += 1u;
+                    fa[k] = fa_n[k]; fw[k] = fw_n[k]; key[k] = key_n[k];
+                }
+                pa_c = ws.pa[i + 1]; pw_c = ws.pw[i + 1];
             }
         }
         // release what the lanes still hold
 #pragma unroll
         for (int k = 0; k < D; ++k) {
             sts_v2_if(true, sw_base + cur[k], accS[k], accW[k]);
-            red_u32_if(true, n_base + (cur[k] >> 2), (unsigned)(r1 + 1 - i0[k]));
+            sts_u32_if(true, n_base + (cur[k] >> 2), cnt[k]);
         }
         __syncwarp();
     }
@@ -414,7 +435,6 @@ __device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsi
     const int nd = dhi - dlo + 1;
     if (nd <= 32) xi_walk<1, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
     else if (nd <= 64) xi_walk<2, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
-    else if (nd <= 96) xi_walk<3, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
     else xi_walk<4, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
 }
 
@@ -491,6 +511,10 @@ __global__ void __launch_bounds__(FTHREADS, 2) k_xi_fast(XiFastParams P)
                 for (int t = lane; 2 * t < mp; t += 32) {
                     ((double2 *)ws.pc)[t] = sc[t]; ((double2 *)ws.pa)[t] = sa[t]; ((double2 *)ws.pw)[t] = sw[t];
                 }
+                __syncwarp();
+                for (int t = mp + lane; t < FTP; t += 32) {              // sentinel rows (!= q's sentinel: r_par never 0)
+                    ws.pc[t] = 2.0 * LYA_CHI_SENTINEL; ws.pa[t] = 0.0; ws.pw[t] = 0.0;
+                }
                 cur_p = p;
             }
             {
@@ -531,7 +555,7 @@ __global__ void __launch_bounds__(FTHREADS, 2) k_xi_fast(XiFastParams P)
                 }
                 dlo = __reduce_min_sync(0xffffffffu, dlo); dhi = __reduce_max_sync(0xffffffffu, dhi);
                 r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
-                if (r1 >= r0) xi_walk_any<POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated);
+                if (r1 >= r0) xi_walk_any<POW2>(ws, sw_base, n_base, r0 & ~3, r1 | 3, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated);
             }
         }
     }
