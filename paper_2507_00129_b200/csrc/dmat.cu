@@ -68,7 +68,7 @@ struct DmParams {
     BinParams bp;
     unsigned long long seed, thr;
     double *Dn, *Wd;
-    unsigned long long *counters;   // [0] next chunk, [1] visited, [2] evaluated, [3] error, [4] kept, [5] binned
+    unsigned long long *counters;   // [0] next chunk, [1] visited, [2] evaluated, [3] error, [5] kept, [6] binned
     int LC;                         // columns per local table
 };
 
@@ -304,8 +304,401 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
     if (lane == 0) {
         atomicAdd(&P.counters[1], visited);
         atomicAdd(&P.counters[2], evaluated);
-        atomicAdd(&P.counters[4], kept_total);
-        atomicAdd(&P.counters[5], binned);
+        atomicAdd(&P.counters[5], kept_total);
+        atomicAdd(&P.counters[6], binned);
+    }
+}
+
+// ======================= fast kernel ======================================
+// One warp per forest pair of the bucket-sorted list, forests staged from the padded catalogue.
+//  pass A  diagonal walk (the xi kernel's traversal): the four H tables of the pair, each lane
+//          holding the table entry of its current run in registers (predicated release/acquire, no
+//          atomics: the walk is done once per side of chi_i = chi_j, so entries have one holder);
+//          every in-grid pair is hashed on the fly (stage 4) and the kept ones are queued;
+//  pass B  the non-zero table entries are compacted into a list;
+//  pass C  the kept pairs are drained: T1..T3 per kept pair, T4 with lanes over the table entries and
+//          an inner loop over the kept pairs (the entry stays in registers); every update is one
+//          red.global.add.f64 into the L2-resident Dn.
+constexpr int FD_WARPS = 5;
+constexpr int FD_THREADS = FD_WARPS * 32;
+constexpr int FD_T = LYA_FAST_TILE;
+constexpr int FD_ROWS = 16;
+constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
+constexpr int FD_PAD = 2;
+constexpr int FD_SLOTS = 360;                // (n_par + 1) * (LYA_NCOL + 1) <= FD_SLOTS
+constexpr int FD_KCAP = 128;                 // kept pairs queued per drain
+constexpr int FD_CHUNK = 8;
+
+struct DmFastParams {
+    LyaPrep prep;
+    const int32_t *pq;
+    int64_t n_pairs;
+    BinParams bp;
+    unsigned long long seed, thr;
+    double *Dn, *Wd;
+    unsigned long long *counters;   // [4] next chunk, [2] evaluated, [3] error, [5] kept, [6] binned
+};
+
+struct __align__(16) DmFastWarp {
+    double2 H01[FD_SLOTS], H23[FD_SLOTS];    // (H_aa, H_ag), (H_ga, H_gg) per slot = col_rel * (n_par + 1) + row
+    double pc[FD_TP], pw[FD_TP], pu[FD_TP], pea[FD_TP], peg[FD_TP];
+    double qc[FD_T + 2 * FD_PAD], qw[FD_T + 2 * FD_PAD], qu[FD_T + 2 * FD_PAD], qea[FD_T + 2 * FD_PAD], qeg[FD_T + 2 * FD_PAD];
+    unsigned long long pk[FD_T], qk[FD_T];   // stage-4 keys of the pixels
+    unsigned kept[FD_KCAP];                  // (i << 20) | (j << 12) | A
+    unsigned short nz[FD_SLOTS];             // non-zero slots
+    unsigned char jlo[FD_T], jx[FD_T], jhi[FD_T];
+    unsigned nkept, pad_[3];
+};
+
+__device__ __forceinline__ void dsts_v2_if(bool p, unsigned addr, double x, double y)
+{
+    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q st.shared.v2.f64 [%1], {%2, %3};\n}"
+                 :: "r"((unsigned)p), "r"(addr), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void dlds_v2_if(bool p, unsigned addr, double &x, double &y)
+{
+    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %2, 0;\n @q ld.shared.v2.f64 {%0, %1}, [%3];\n}"
+                 : "+d"(x), "+d"(y) : "r"((unsigned)p), "r"(addr) : "memory");
+}
+
+// byte offset (16 * slot) of a pixel pair in the H tables and whether it is a pair of THIS walk
+// (inside the grid and on the walk's side of chi_i = chi_j: sgn = 0 for chi_i >= chi_j, -1 otherwise);
+// A = its bin.  Pairs outside get the garbage row / column.
+template <bool POW2>
+__device__ __forceinline__ unsigned dm_key(const BinParams &bp, const PairBin &g, double chi_i, double chi_j, unsigned c0,
+                                           unsigned np1, int sgn, bool &valid, unsigned &A)
+{
+    const double d = __dsub_rn(chi_i, chi_j);
+    const double t = __dadd_rn(chi_i, chi_j);
+    unsigned bx, by;
+    if (POW2) {
+        bx = lya_floor_u32(__dmul_rn(fabs(d), g.cx));
+        by = lya_floor_u32(__dmul_rn(t, g.sy));
+    } else {
+        const double rpar = __dmul_rn(fabs(d), g.c), rperp = __dmul_rn(t, g.s);
+        bx = (rpar < bp.rpar_max) ? min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1)) : (unsigned)bp.n_par;
+        by = (rperp < bp.rperp_max) ? min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1)) : 0x7fffffffu;
+    }
+    const bool side = ((__double2hiint(d) ^ sgn) >= 0);
+    valid = side & (bx < (unsigned)bp.n_par) & (by < (unsigned)bp.n_perp);
+    A = bx * (unsigned)bp.n_perp + by;
+    bx = valid ? bx : np1 - 1u;
+    const unsigned col = min(by - c0, (unsigned)LYA_NCOL);
+    return (col * np1 + bx) * 16u;
+}
+
+// stage-4 keep mask on precomputed pixel keys (same integer function as keep_pair above)
+__device__ __forceinline__ bool dm_keep(unsigned long long klo, unsigned long long khi, unsigned long long thr)
+{
+    return keep_pair(klo, khi, thr);
+}
+
+// pass A over rows [r0, r1] (a multiple of D rows; rows >= len are sentinels) and diagonals [dlo, dhi]
+template <int D, bool POW2>
+__device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h23, int r0, int r1, int mq, int dlo, int dhi,
+                                        int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned np1,
+                                        unsigned long long thr, int lane, unsigned &binned, unsigned &kept_n,
+                                        unsigned long long &evaluated)
+{
+    const double *qc = ws.qc + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
+    const unsigned garbage = (LYA_NCOL * np1 + np1 - 1u) * 16u;
+    for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
+        const int dl = d0 + lane * D;
+        unsigned cur[D];
+        double h0[D], h1[D], h2[D], h3[D];
+        double wc[D], wa[D], wg[D];                         // sliding window over q: chi, ea, eg
+#pragma unroll
+        for (int k = 0; k < D; ++k) { cur[k] = garbage; h0[k] = 0.0; h1[k] = 0.0; h2[k] = 0.0; h3[k] = 0.0; }
+#pragma unroll
+        for (int k = 0; k < D - 1; ++k) {
+            const int j = min(max(r0 + dl + k, -FD_PAD), mq + FD_PAD - 1);
+            wc[k] = qc[j]; wa[k] = qea[j]; wg[k] = qeg[j];
+        }
+        evaluated += (unsigned long long)(r1 - r0 + 1) * D;
+        for (int ib = r0; ib <= r1; ib += D) {
+#pragma unroll
+            for (int u = 0; u < D; ++u) {
+                const int i = ib + u;
+                const double pci = ws.pc[i], pai = ws.pea[i], pgi = ws.peg[i];
+                const unsigned long long pki = ws.pk[min(i, FD_T - 1)];
+                const int jn = i + dl + D - 1;              // the lane's newest q pixel
+                {
+                    const int j = min(max(jn, -FD_PAD), mq + FD_PAD - 1);
+                    wc[(u + D - 1) % D] = qc[j]; wa[(u + D - 1) % D] = qea[j]; wg[(u + D - 1) % D] = qeg[j];
+                }
+                unsigned key[D];
+                bool ch[D];
+#pragma unroll
+                for (int k = 0; k < D; ++k) {
+                    const int sl = (k + u) % D;
+                    bool valid; unsigned A;
+                    key[k] = dm_key<POW2>(bp, g, pci, wc[sl], c0, np1, sgn, valid, A);
+                    const int j = jn - (D - 1) + k;
+                    const bool kp = valid && dm_keep(pki, ws.qk[min(max(j, 0), FD_T - 1)], thr);
+                    binned += valid ? 1u : 0u;
+                    if (kp) {                                // ~1 % of the pairs at f = 0.99
+                        const unsigned idx = atomicAdd(&ws.nkept, 1u);
+                        if (idx < FD_KCAP) ws.kept[idx] = ((unsigned)i << 20) | ((unsigned)j << 12) | A;
+                        kept_n += 1u;
+                    }
+                    ch[k] = key[k] != cur[k];
+                    dsts_v2_if(ch[k], h01 + cur[k], h0[k], h1[k]);                      // release
+                    dsts_v2_if(ch[k], h23 + cur[k], h2[k], h3[k]);
+                }
+                __syncwarp();
+#pragma unroll
+                for (int k = 0; k < D; ++k) {
+                    const int sl = (k + u) % D;
+                    dlds_v2_if(ch[k], h01 + key[k], h0[k], h1[k]);                      // acquire
+                    dlds_v2_if(ch[k], h23 + key[k], h2[k], h3[k]);
+                    cur[k] = key[k];
+                    h0[k] = fma(pai, wa[sl], h0[k]); h1[k] = fma(pai, wg[sl], h1[k]);
+                    h2[k] = fma(pgi, wa[sl], h2[k]); h3[k] = fma(pgi, wg[sl], h3[k]);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < D; ++k) {
+            dsts_v2_if(true, h01 + cur[k], h0[k], h1[k]);
+            dsts_v2_if(true, h23 + cur[k], h2[k], h3[k]);
+        }
+        __syncwarp();
+    }
+}
+
+template <bool POW2>
+__device__ __forceinline__ void dm_walk_any(DmFastWarp &ws, unsigned h01, unsigned h23, int r0, int r1, int mq, int dlo, int dhi,
+                                            int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned np1,
+                                            unsigned long long thr, int lane, unsigned &binned, unsigned &kept_n,
+                                            unsigned long long &evaluated)
+{
+    if (dhi < dlo) return;
+    const int nd = dhi - dlo + 1;
+    if (nd <= 32) dm_walk<1, POW2>(ws, h01, h23, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, np1, thr, lane, binned, kept_n, evaluated);
+    else dm_walk<2, POW2>(ws, h01, h23, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, np1, thr, lane, binned, kept_n, evaluated);
+}
+
+// pass C: drain n queued kept pairs.  do_t123: also T1..T3 (false when only T4 is wanted).
+template <bool POW2>
+__device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp, int mq, const DmFastParams &P,
+                                         const PairBin &g, int c0, int lane)
+{
+    const BinParams &bp = P.bp;
+    const int nb = bp.n_par * bp.n_perp, np1 = bp.n_par + 1;
+    const double *qc = ws.qc + FD_PAD, *qw = ws.qw + FD_PAD, *qu = ws.qu + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
+    // T1: Dn[A][A] += om, Wd[A] += om (lanes over kept pairs)
+    for (int e = lane; e < n; e += 32) {
+        const unsigned rec = ws.kept[e];
+        const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
+        const double om = ws.pw[i] * qw[j];
+        atomicAdd(P.Dn + (size_t)A * nb + A, om);
+        atomicAdd(P.Wd + A, om);
+    }
+    // T2, T3 (lanes over the pixels of q resp. p)
+    for (int e = 0; e < n; ++e) {
+        const unsigned rec = ws.kept[e];
+        const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
+        const double om = ws.pw[i] * qw[j], ui = ws.pu[i], uj = qu[j];
+        double *row = P.Dn + (size_t)A * nb;
+        const double pci = ws.pc[i], qcj = qc[j];
+        for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {          // T2: (i, j') inside row i's window
+            const int B = lya_pix_bin<POW2>(bp, g, pci, qc[j2]);
+            if (B >= 0) atomicAdd(row + B, -om * (qea[j2] + uj * qeg[j2]));
+        }
+        for (int i2 = lane; i2 < mp; i2 += 32) {                             // T3: (i', j)
+            const int B = lya_pix_bin<POW2>(bp, g, ws.pc[i2], qcj);
+            if (B >= 0) atomicAdd(row + B, -om * (ws.pea[i2] + ui * ws.peg[i2]));
+        }
+    }
+    // T4: lanes over the non-zero table entries, inner loop over the kept pairs
+    for (int t = lane; t < nnz; t += 32) {
+        const int slot = ws.nz[t];
+        const int cr = slot / np1, bx = slot - cr * np1;
+        const int B = bx * bp.n_perp + c0 + cr;
+        const double2 a = ws.H01[slot], b = ws.H23[slot];
+        for (int e = 0; e < n; ++e) {
+            const unsigned rec = ws.kept[e];
+            const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
+            const double om = ws.pw[i] * qw[j], ui = ws.pu[i], uj = qu[j];
+            const double v = (a.x + uj * a.y) + ui * (b.x + uj * b.y);
+            atomicAdd(P.Dn + (size_t)A * nb + B, om * v);
+        }
+    }
+}
+
+template <bool POW2>
+__global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    DmFastWarp &ws = ((DmFastWarp *)smem_raw)[wid];
+    const BinParams bp = P.bp;
+    const unsigned np1 = (unsigned)bp.n_par + 1u;
+    const int n_slots = (int)np1 * (LYA_NCOL + 1);
+    for (int t = lane; t < FD_SLOTS; t += 32) { ws.H01[t] = make_double2(0.0, 0.0); ws.H23[t] = make_double2(0.0, 0.0); }
+    if (lane < FD_PAD) { ws.qc[lane] = LYA_CHI_SENTINEL; ws.qw[lane] = 0.0; ws.qu[lane] = 0.0; ws.qea[lane] = 0.0; ws.qeg[lane] = 0.0; }
+    if (lane == 0) ws.nkept = 0u;
+    __syncwarp();
+    const double *qc = ws.qc + FD_PAD;
+    const unsigned h01 = (unsigned)__cvta_generic_to_shared(ws.H01), h23 = (unsigned)__cvta_generic_to_shared(ws.H23);
+    unsigned long long evaluated = 0, kept_total = 0, binned_total = 0;
+    int cur_p = -1, head_p = -1;
+    ForestHead hp;
+    hp.len = 0;
+    const int64_t n_chunks = (P.n_pairs + FD_CHUNK - 1) / FD_CHUNK;
+    for (;;) {
+        unsigned long long chunk = 0;
+        if (lane == 0) chunk = atomicAdd(&P.counters[4], 1ull);
+        chunk = __shfl_sync(0xffffffffu, chunk, 0);
+        if ((int64_t)chunk >= n_chunks) break;
+        const int64_t k0 = (int64_t)chunk * FD_CHUNK, k1 = min(k0 + FD_CHUNK, P.n_pairs);
+        for (int64_t k = k0; k < k1; ++k) {
+            const int2 e = ((const int2 *)P.pq)[k];
+            const int p = e.x, q = e.y;
+            if (p != head_p) { hp = P.prep.head[p]; head_p = p; }
+            const ForestHead hq = P.prep.head[q];
+            const int mp = hp.len, mq = hq.len;
+            if ((hp.flags | hq.flags) & 1) {
+                if (lane == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_DEGENERATE);
+                continue;
+            }
+            double s, c;
+            lya_pair_sc(hp.ux, hp.uy, hp.uz, hq.ux, hq.uy, hq.uz, s, c);
+            const PairBin g = lya_make_pairbin(bp, s, c);
+            int c0;
+            const int key = lya_pair_key<POW2>(bp, g, hp, hq, c0);
+            if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
+            __syncwarp();
+            if (p != cur_p) {
+                const double2 *s0 = (const double2 *)(P.prep.chi + hp.off), *s1 = (const double2 *)(P.prep.w + hp.off),
+                              *s2 = (const double2 *)(P.prep.u + hp.off), *s3 = (const double2 *)(P.prep.ea + hp.off),
+                              *s4 = (const double2 *)(P.prep.eg + hp.off);
+                for (int t = lane; 2 * t < mp; t += 32) {
+                    ((double2 *)ws.pc)[t] = s0[t]; ((double2 *)ws.pw)[t] = s1[t]; ((double2 *)ws.pu)[t] = s2[t];
+                    ((double2 *)ws.pea)[t] = s3[t]; ((double2 *)ws.peg)[t] = s4[t];
+                }
+                for (int t = lane; t < mp; t += 32) ws.pk[t] = key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
+                __syncwarp();
+                for (int t = mp + lane; t < FD_TP; t += 32) {            // sentinel rows (!= q's sentinel: r_par never 0)
+                    ws.pc[t] = 2.0 * LYA_CHI_SENTINEL; ws.pw[t] = 0.0; ws.pu[t] = 0.0; ws.pea[t] = 0.0; ws.peg[t] = 0.0;
+                }
+                cur_p = p;
+            }
+            {
+                const double2 *s0 = (const double2 *)(P.prep.chi + hq.off), *s1 = (const double2 *)(P.prep.w + hq.off),
+                              *s2 = (const double2 *)(P.prep.u + hq.off), *s3 = (const double2 *)(P.prep.ea + hq.off),
+                              *s4 = (const double2 *)(P.prep.eg + hq.off);
+                const int npad2 = (mq + 1) >> 1;
+                for (int t = lane; t < npad2; t += 32) {
+                    ((double2 *)qc)[t] = s0[t]; ((double2 *)(ws.qw + FD_PAD))[t] = s1[t]; ((double2 *)(ws.qu + FD_PAD))[t] = s2[t];
+                    ((double2 *)(ws.qea + FD_PAD))[t] = s3[t]; ((double2 *)(ws.qeg + FD_PAD))[t] = s4[t];
+                }
+                for (int t = lane; t < mq; t += 32) ws.qk[t] = key_hi(P.seed, (unsigned long long)(hq.pix0 + t));
+                if (lane < FD_PAD) {
+                    const int j = FD_PAD + 2 * npad2 + lane;
+                    ws.qc[j] = LYA_CHI_SENTINEL; ws.qw[j] = 0.0; ws.qu[j] = 0.0; ws.qea[j] = 0.0; ws.qeg[j] = 0.0;
+                }
+            }
+            __syncwarp();
+            // per row of p: in-grid window [jlo, jhi) of q and the sign change jx (chi_i >= chi_j below it)
+            const double R = (c > 0.0) ? (bp.rpar_max / c) * (1.0 + 1e-12) + 1e-9 : 1e300;
+            const double Tchi = (s > 0.0) ? (bp.rperp_max / s) * (1.0 + 1e-12) + 1e-9 : 1e300;
+            for (int i = lane; i < mp; i += 32) {
+                const double x = ws.pc[i];
+                int lo = 0, hi = mq;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x - R) hi = mid; else lo = mid + 1; }
+                const int jlo = lo;
+                const double top = fmin(x + R, Tchi - x);
+                hi = mq;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] >= top) hi = mid; else lo = mid + 1; }
+                const int jhi = lo;
+                lo = jlo; hi = jhi;
+                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x) hi = mid; else lo = mid + 1; }
+                ws.jlo[i] = (unsigned char)jlo; ws.jhi[i] = (unsigned char)jhi; ws.jx[i] = (unsigned char)lo;
+            }
+            __syncwarp();
+            // ---- pass A ----
+            unsigned binned = 0, kept_n = 0;
+            for (int i0 = 0; i0 < mp; i0 += FD_ROWS) {
+                const int i = i0 + lane;
+                int plo = 1 << 20, phi = -(1 << 20), nlo = 1 << 20, nhi = -(1 << 20), r0 = 1 << 20, r1 = -1;
+                if (lane < FD_ROWS && i < mp) {
+                    const int jl = ws.jlo[i], jh = ws.jhi[i], jx = ws.jx[i];
+                    if (jx > jl) { plo = jl - i; phi = jx - 1 - i; }
+                    if (jh > jx) { nlo = jx - i; nhi = jh - 1 - i; }
+                    if (jh > jl) { r0 = i; r1 = i; }
+                }
+                plo = __reduce_min_sync(0xffffffffu, plo); phi = __reduce_max_sync(0xffffffffu, phi);
+                nlo = __reduce_min_sync(0xffffffffu, nlo); nhi = __reduce_max_sync(0xffffffffu, nhi);
+                r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
+                if (r1 < r0) continue;
+                dm_walk_any<POW2>(ws, h01, h23, r0 & ~1, r1 | 1, mq, plo, phi, 0, bp, g, (unsigned)c0, np1, P.thr, lane, binned, kept_n, evaluated);
+                dm_walk_any<POW2>(ws, h01, h23, r0 & ~1, r1 | 1, mq, nlo, nhi, -1, bp, g, (unsigned)c0, np1, P.thr, lane, binned, kept_n, evaluated);
+            }
+            binned_total += binned; kept_total += kept_n;
+            __syncwarp();
+            // ---- pass B: compact the non-zero entries (H_aa > 0 wherever a pair with weight fell) ----
+            int nnz = 0;
+            for (int t0 = 0; t0 < n_slots; t0 += 32) {
+                const int t = t0 + lane;
+                bool nzf = false;
+                if (t < n_slots) {
+                    const int cr = t / (int)np1, bx = t - cr * (int)np1;
+                    const double2 a = ws.H01[t], b = ws.H23[t];
+                    nzf = (bx < bp.n_par) && (cr < LYA_NCOL) && (a.x != 0.0 || a.y != 0.0 || b.x != 0.0 || b.y != 0.0);
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, nzf);
+                if (nzf) ws.nz[nnz + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)t;
+                nnz += __popc(bal);
+            }
+            __syncwarp();
+            // ---- pass C ----
+            const unsigned nk = ws.nkept;
+            if (nk <= FD_KCAP) {
+                dm_drain<POW2>(ws, (int)nk, nnz, mp, mq, P, g, c0, lane);
+            } else {
+                // more kept pairs than the queue holds (small reject fractions): redo the mask row by row
+                int n_q = 0;
+                for (int i = 0; i < mp; ++i) {
+                    const double pci = ws.pc[i];
+                    const unsigned long long ki = ws.pk[i];
+                    for (int j0 = ws.jlo[i]; j0 < ws.jhi[i]; j0 += 32) {
+                        const int j = j0 + lane;
+                        int A = -1;
+                        if (j < ws.jhi[i]) A = lya_pix_bin<POW2>(bp, g, pci, qc[j]);
+                        const bool kp = (A >= 0) && keep_pair(ki, ws.qk[min(j, FD_T - 1)], P.thr);
+                        const unsigned bal = __ballot_sync(0xffffffffu, kp);
+                        if (bal) {
+                            if (n_q + __popc(bal) > FD_KCAP) {
+                                __syncwarp();
+                                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane);
+                                __syncwarp();
+                                n_q = 0;
+                            }
+                            if (kp) ws.kept[n_q + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)i << 20) | ((unsigned)j << 12) | (unsigned)A;
+                            n_q += __popc(bal);
+                        }
+                    }
+                }
+                __syncwarp();
+                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane);
+            }
+            __syncwarp();
+            // clear the table and the queue for the next pair
+            for (int t = lane; t < n_slots; t += 32) { ws.H01[t] = make_double2(0.0, 0.0); ws.H23[t] = make_double2(0.0, 0.0); }
+            if (lane == 0) ws.nkept = 0u;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
+        kept_total += __shfl_xor_sync(0xffffffffu, kept_total, o);
+        binned_total += __shfl_xor_sync(0xffffffffu, binned_total, o);
+    }
+    if (lane == 0) {
+        atomicAdd(&P.counters[2], evaluated);
+        atomicAdd(&P.counters[5], kept_total);
+        atomicAdd(&P.counters[6], binned_total);
     }
 }
 
@@ -340,45 +733,81 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     int max_len = 0;
     st = lya_validate_forests(ctx, f, false, true, &max_len);
     if (st) return st;
-    if (max_len > 255) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: forests longer than 255 pixels are not supported yet");
 
     const int nb = b->n_par * b->n_perp;
     cudaStream_t s = ctx->stream;
+    const BinParams bp = lya_make_binparams(b);
+    const bool use_fast = pairs->n > 0 && (b->n_par + 1) * (LYA_NCOL + 1) <= FD_SLOTS && b->n_perp + 2 <= 256 &&
+                          ctx->dmat_variant != 9;
+    if (!use_fast && max_len > DTILE)
+        return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: forests longer than %d pixels are not supported with this binning", DTILE);
     double *scal = NULL, *Dn = Dn_out, *Wd = Wd_out;
     bool own_Dn = false, own_Wd = false;
     const int64_t nf = f->n_forest;
-    LYA_CUDA(cudaMalloc(&scal, sizeof(double) * 3 * (size_t)(nf ? nf : 1)));
-    if (!Dn) { cudaError_t e = cudaMalloc(&Dn, sizeof(double) * (size_t)nb * nb); if (e != cudaSuccess) { cudaFree(scal); return lya_cuda_fail(ctx, e, "cudaMalloc(Dn)"); } own_Dn = true; }
-    if (!Wd) { cudaError_t e = cudaMalloc(&Wd, sizeof(double) * (size_t)nb); if (e != cudaSuccess) { cudaFree(scal); if (own_Dn) cudaFree(Dn); return lya_cuda_fail(ctx, e, "cudaMalloc(Wd)"); } own_Wd = true; }
-    auto cleanup = [&]() { cudaFree(scal); if (own_Dn) cudaFree(Dn); if (own_Wd) cudaFree(Wd); };
+    LyaPrep prep;
+    LyaBuckets bk;
+    memset(&prep, 0, sizeof(prep));
+    memset(&bk, 0, sizeof(bk));
+    auto cleanup = [&]() { cudaFree(scal); if (own_Dn) cudaFree(Dn); if (own_Wd) cudaFree(Wd); lya_prep_free(&prep); lya_buckets_free(&bk); };
+    cudaEventRecord(ctx->ev[3], s);
+    if (use_fast) {
+        st = lya_prep_build(ctx, f, false, true, &prep);
+        if (st) return st;
+        cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
+        st = lya_bucket_pairs(ctx, &prep, &bp, pairs, 0, &bk);
+        if (st) { cleanup(); return st; }
+        if (bk.bad_pair == LYA_DEV_DEGENERATE) { cleanup(); return lya_fail(ctx, LYA_ERR_DEGENERATE_FOREST, "a listed forest has sum w == 0 or sum w (L-Lbar)^2 == 0"); }
+        if (bk.bad_pair) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
+    }
+    cudaError_t e = cudaMalloc(&scal, sizeof(double) * 3 * (size_t)(nf ? nf : 1));
+    if (e == cudaSuccess && !Dn) { e = cudaMalloc(&Dn, sizeof(double) * (size_t)nb * nb); own_Dn = (e == cudaSuccess); if (!own_Dn) Dn = NULL; }
+    if (e == cudaSuccess && !Wd) { e = cudaMalloc(&Wd, sizeof(double) * (size_t)nb); own_Wd = (e == cudaSuccess); if (!own_Wd) Wd = NULL; }
+    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_dmat)"); }
     cudaMemsetAsync(Dn, 0, sizeof(double) * (size_t)nb * nb, s);
     cudaMemsetAsync(Wd, 0, sizeof(double) * (size_t)nb, s);
     cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
-    if (nf > 0)
-        k_forest_scalars<<<(unsigned)((nf + 127) / 128), 128, 0, s>>>(f->pix_off, f->w, f->loglam, nf, scal, scal + nf, scal + 2 * nf);
-
-    DmParams P;
-    P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.loglam = f->loglam;
-    P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
-    P.f_invS = scal; P.f_lbar = scal + nf; P.f_invV = scal + 2 * nf;
-    P.pq = pairs->pq; P.n_pairs = pairs->n; P.n_forest = nf;
-    P.bp = lya_make_binparams(b);
-    P.seed = seed;
+    unsigned long long thr;
     {
         double t = floor(reject_fraction * 4294967296.0 + 0.5);
         if (t < 0) t = 0;
         if (t > 4294967296.0) t = 4294967296.0;
-        P.thr = (unsigned long long)t;
+        thr = (unsigned long long)t;
     }
+    // generic kernel (long forests, wide column span, fine pixel spacing): original arrays
+    DmParams P;
+    P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.loglam = f->loglam;
+    P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
+    P.f_invS = scal; P.f_lbar = scal + nf; P.f_invV = scal + 2 * nf;
+    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pairs->pq;
+    P.n_pairs = use_fast ? bk.n_generic : pairs->n;
+    P.n_forest = nf;
+    P.bp = bp;
+    P.seed = seed; P.thr = thr;
     P.Dn = Dn; P.Wd = Wd; P.counters = ctx->d_counters;
     P.LC = H_SLOTS / b->n_par;
     if (P.LC > 8) P.LC = 8;
     if (P.LC > b->n_perp) P.LC = b->n_perp;
 
-    const size_t smem = sizeof(DmWarpSmem) * DM_WARPS;
     cudaEventRecord(ctx->ev[0], s);
-    if (pairs->n > 0) {
-        cudaError_t e;
+    if (use_fast && bk.n_fast > 0) {
+        DmFastParams F;
+        F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp; F.seed = seed; F.thr = thr;
+        F.Dn = Dn; F.Wd = Wd; F.counters = ctx->d_counters;
+        const size_t fsmem = sizeof(DmFastWarp) * FD_WARPS;
+        const int fgrid = ctx->sm_count * 2;
+        if (bp.pow2) {
+            e = cudaFuncSetAttribute(k_dmat_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
+            if (e == cudaSuccess) k_dmat_fast<true><<<fgrid, FD_THREADS, fsmem, s>>>(F);
+        } else {
+            e = cudaFuncSetAttribute(k_dmat_fast<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
+            if (e == cudaSuccess) k_dmat_fast<false><<<fgrid, FD_THREADS, fsmem, s>>>(F);
+        }
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_dmat_fast launch"); }
+    }
+    if (P.n_pairs > 0) {
+        k_forest_scalars<<<(unsigned)((nf + 127) / 128), 128, 0, s>>>(f->pix_off, f->w, f->loglam, nf, scal, scal + nf, scal + 2 * nf);
+        const size_t smem = sizeof(DmWarpSmem) * DM_WARPS;
         int grid = ctx->sm_count * 2;
         if (P.bp.pow2) {
             e = cudaFuncSetAttribute(k_dmat<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -394,9 +823,10 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     if (D) k_dmat_normalise<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, s>>>(Dn, Wd, nb, D);
     cudaEventRecord(ctx->ev[2], s);
     unsigned long long h[8];
-    cudaError_t e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
+    e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "lya_dmat"); }
+    const unsigned long long visited = use_fast ? bk.visited : h[1];
     cleanup();
     switch ((unsigned)h[3]) {
     case LYA_DEV_OK: break;
@@ -407,12 +837,12 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     if (stats) {
         memset(stats, 0, sizeof(*stats));
         stats->n_forest_pairs = (uint64_t)pairs->n;
-        stats->n_visited = h[1];
+        stats->n_visited = visited;
         stats->n_evaluated = h[2];
-        stats->n_kept = h[4];
-        stats->n_binned = h[5];
+        stats->n_kept = h[5];
+        stats->n_binned = h[6];
         cudaEventElapsedTime(&stats->ms_main, ctx->ev[0], ctx->ev[1]);
-        cudaEventElapsedTime(&stats->ms_total, ctx->ev[0], ctx->ev[2]);
+        cudaEventElapsedTime(&stats->ms_total, ctx->ev[3], ctx->ev[2]);
     }
     return LYA_OK;
 }

@@ -47,11 +47,12 @@ struct BinParams;
 // Every forest starts at an even offset and is padded to an even length, so each
 // sub-array of a forest can be moved with 16-byte vector loads.  Pad pixels hold
 // chi = LYA_CHI_SENTINEL and 0 elsewhere (never inside any grid).
-struct __align__(16) ForestHead {   // 64 bytes, one per forest
+struct __align__(16) ForestHead {   // 80 bytes, one per forest
     double ux, uy, uz;              // sightline unit vector
     double dmin;                    // smallest chi spacing inside the forest (1e300 if < 2 pixels)
     double chi0, chi1;              // first / last pixel (valid when len > 0)
     long long off;                  // offset of the forest in the packed arrays (even)
+    long long pix0;                 // offset of the forest in the caller's flat arrays (stage-4 pixel ids)
     int len;                        // pixels
     int flags;                      // bit 0: degenerate for eq. 2.7 (sum w == 0 or sum w u^2 == 0)
 };
@@ -81,7 +82,7 @@ struct LyaBuckets {
     int64_t n;
     int64_t n_fast, n_generic, n_skip;
     unsigned long long visited;     // sum n_p * n_q over the whole list
-    int bad_pair;                   // a pair referred to a forest outside [0, n_forest)
+    int bad_pair;                   // LYA_DEV_BAD_PAIR: a pair outside [0, n_forest); LYA_DEV_DEGENERATE: a listed degenerate forest
 };
 lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *bp, const lya_pairs *pairs,
                             int force_generic, LyaBuckets *out);

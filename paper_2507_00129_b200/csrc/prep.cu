@@ -62,7 +62,9 @@ __global__ void k_pack(lya_forests f, const unsigned long long *off2, LyaPrep P)
         double v = 0.0;
         for (int t = lane; t < n; t += 32) { double u = f.loglam[a + t] - lbar; v += f.w[a + t] * u * u; }
         v = warp_sum(v);
-        const bool ok = (sw > 0.0) && (v > 0.0);
+        // degenerate (reading R-7): no weight, or all weighted L equal up to rounding of L - Lbar
+        const double tiny = 1e-12 * fabs(lbar);
+        const bool ok = (sw > 0.0) && (v > sw * tiny * tiny);
         invS = ok ? 1.0 / sw : 0.0;
         invV = ok ? 1.0 / v : 0.0;
         flags = ok ? 0 : 1;
@@ -87,7 +89,7 @@ __global__ void k_pack(lya_forests f, const unsigned long long *off2, LyaPrep P)
         h.dmin = dmin;
         h.chi0 = n ? f.chi[a] : 0.0;
         h.chi1 = n ? f.chi[a + n - 1] : 0.0;
-        h.off = o; h.len = n; h.flags = flags;
+        h.off = o; h.pix0 = (long long)a; h.len = n; h.flags = flags;
         P.head[p] = h;
     }
 }
@@ -100,8 +102,9 @@ template <bool POW2>
 __device__ __forceinline__ int pair_key(const ForestHead *head, int64_t n_forest, const BinParams &bp, int p, int q,
                                         unsigned long long &visited, int &bad)
 {
-    if ((unsigned)p >= (unsigned)n_forest || (unsigned)q >= (unsigned)n_forest) { bad = 1; return bp.n_perp + 1; }
+    if ((unsigned)p >= (unsigned)n_forest || (unsigned)q >= (unsigned)n_forest) { bad = max(bad, (int)LYA_DEV_BAD_PAIR); return bp.n_perp + 1; }
     const ForestHead hp = head[p], hq = head[q];
+    if ((hp.flags | hq.flags) & 1) bad = max(bad, (int)LYA_DEV_DEGENERATE);   // (only set by a dmat catalogue)
     visited += (unsigned long long)hp.len * (unsigned long long)hq.len;
     double s, c;
     lya_pair_sc(hp.ux, hp.uy, hp.uz, hq.ux, hq.uy, hq.uz, s, c);
@@ -139,10 +142,10 @@ __global__ void k_bucket_count(const ForestHead *head, int64_t n_forest, BinPara
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) visited += __shfl_xor_sync(0xffffffffu, visited, o);
-    bad = __any_sync(0xffffffffu, bad);
+    bad = __reduce_max_sync(0xffffffffu, bad);
     if (lane == 0) {
         if (visited) atomicAdd(&counters[1], visited);
-        if (bad) atomicMax(&counters[3], (unsigned long long)LYA_DEV_BAD_PAIR);
+        if (bad) atomicMax(&counters[3], (unsigned long long)bad);
     }
 }
 
@@ -274,6 +277,6 @@ lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *
     out->n_generic = (int64_t)(h_start[1] - h_start[0]);
     out->n_skip = n - (int64_t)h_start[1];
     out->visited = h_cnt[1];
-    out->bad_pair = h_cnt[3] != 0;
+    out->bad_pair = (int)h_cnt[3];
     return LYA_OK;
 }
