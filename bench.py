@@ -232,11 +232,11 @@ def main():
         x, dm = step()
         ms_xi.append(x["stats"]["ms_main"])
         pairs_total += x["stats"]["n_binned"]
-        launches += 12 + 3           # neighbour pipeline kernels + xi (main, finalize) + validation
+        launches += 15 + 13          # lya_neighbours: 15 kernels; lya_xi2pcf: validate, prep (5), bucketing (5), k_xi_fast, finalize
         if dm is not None:
             ms_dm.append(dm["stats"]["ms_main"])
             pairs_total += dm["stats"]["n_binned"]
-            launches += 4
+            launches += 13           # lya_dmat: validate, prep (5), bucketing (5), k_dmat_fast, normalise
     ev1.record()
     barrier()
     clocks = sampler.stop() if rank == 0 else None
@@ -294,30 +294,35 @@ def main():
         t_xi = float(np.mean(ms_xi)) * 1e-3
         t_dm = float(np.mean(ms_dm)) * 1e-3 if ms_dm else 0.0
         sm_clk = (clocks.get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)) * 1e6
-        # roofline: algorithmic fp64-pipe instructions per launch
-        #   xi: 6 per visited pixel pair (sub, add, 2 mul, 2 floor) + 2 per binned pair (2 FMA)
-        alg_xi = 6.0 * sx["n_visited"] + 2.0 * sx["n_binned"]
+        # roofline: ALGORITHMIC fp64 lane-operations per launch / measured launch time,
+        # against the fp64 pipe: SMs x 64 lanes x sm_max_mhz.
+        #   xi: 8 per binned pixel pair (sub, add, 2 mul, 2 floor-adds, 2 FMA); out-of-grid evaluations are waste
+        #   D : 10 per scanned (in-grid) pair (6 geometry + 4 H FMAs) + 4 per scatter-add of the drain
         peak_alu = ctx.sm_count() * FP64_LANES_PER_SM * peaks.get("sm_max_mhz", 1965.0) * 1e6
-        roof_xi = {"bound": "alu", "kernel": "k_xi", "achieved": alg_xi / t_xi / 1e12, "peak": peak_alu / 1e12,
-                   "unit": "Tinst/s (fp64 lane-instructions)", "frac": alg_xi / t_xi / peak_alu, "traffic": None,
-                   "peak_source": f"derived: {ctx.sm_count()} SMs x {FP64_LANES_PER_SM} fp64 lanes x sm_max_mhz ({peak_kind} MEASURED_PEAKS.json)",
-                   "frac_at_sampled_clock": alg_xi / t_xi / (ctx.sm_count() * FP64_LANES_PER_SM * sm_clk),
-                   "measured_peaks": {k: ctx.lya_measure_peak(k) for k in ("fp64_fma", "fp64_add", "smem_cas64", "smem_add32", "l2_red64")}}
+        peak_src = (f"derived: {ctx.sm_count()} SMs x {FP64_LANES_PER_SM} fp64 lanes x sm_max_mhz "
+                    f"({peak_kind} MEASURED_PEAKS.json); DFMA/DADD microbenchmarks in measured_peaks")
+        mp = {k: ctx.lya_measure_peak(k) for k in ("fp64_fma", "fp64_add", "smem_cas64", "smem_add32", "l2_red64")}
+        alg_xi = 8.0 * sx["n_binned"]
+        roof_xi = {"bound": "alu", "kernel": "k_xi_fast", "achieved": alg_xi / t_xi / 1e12, "peak": peak_alu / 1e12,
+                   "unit": "Tops/s (fp64 lane-operations)", "frac": alg_xi / t_xi / peak_alu, "traffic": None,
+                   "peak_source": peak_src, "frac_at_sampled_clock": alg_xi / t_xi / (ctx.sm_count() * FP64_LANES_PER_SM * sm_clk),
+                   "evaluated_per_binned": sx["n_evaluated"] / max(sx["n_binned"], 1)}
         roof = roof_xi
         extra = {"xi": {"binned_pairs_per_s": sx["n_binned"] / t_xi, "visited_pairs_per_s": sx["n_visited"] / t_xi,
                         "evaluated_pairs_per_s": sx["n_evaluated"] / t_xi, "ms": t_xi * 1e3,
-                        "forest_pairs": sx["n_forest_pairs"], "roofline": roof_xi}}
+                        "forest_pairs": sx["n_forest_pairs"], "roofline": roof_xi},
+                 "measured_peaks": mp}
         if sd is not None:
-            # D: algorithmic fp64 instructions = H pass (6 per visited + 4 FMA per binned) + per kept pair
-            # (n_p + n_q) x (6 geometry + 2) for T2/T3 and 4 per support bin for T4 -- reported as scatter rate
+            alg_d = 10.0 * sd["n_binned"] + 4.0 * sd["n_scatter"]
+            roof_d = {"bound": "alu", "kernel": "k_dmat_fast", "achieved": alg_d / t_dm / 1e12, "peak": peak_alu / 1e12,
+                      "unit": "Tops/s (fp64 lane-operations)", "frac": alg_d / t_dm / peak_alu, "traffic": None,
+                      "peak_source": peak_src,
+                      "scatter_adds_per_s": sd["n_scatter"] / t_dm,
+                      "frac_of_measured_l2_red_peak": sd["n_scatter"] / t_dm / mp["l2_red64"]}
             extra["dmat"] = {"scanned_pairs_per_s": sd["n_binned"] / t_dm, "kept_pairs_per_s": sd["n_kept"] / t_dm,
-                             "ms": t_dm * 1e3, "n_kept": sd["n_kept"]}
+                             "ms": t_dm * 1e3, "n_kept": sd["n_kept"], "n_scatter": sd["n_scatter"], "roofline": roof_d}
             if t_dm > t_xi:
-                alg_d = 6.0 * sd["n_visited"] + 4.0 * sd["n_binned"]
-                roof = {"bound": "alu", "kernel": "k_dmat", "achieved": alg_d / t_dm / 1e12, "peak": peak_alu / 1e12,
-                        "unit": "Tinst/s (fp64 lane-instructions)", "frac": alg_d / t_dm / peak_alu, "traffic": None,
-                        "note": "H-table pass only; the per-kept-pair scatter is bounded by L2 fp64 red throughput, see dmat.red_per_s",
-                        "peak_source": roof_xi["peak_source"]}
+                roof = roof_d
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

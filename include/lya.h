@@ -90,6 +90,7 @@ typedef struct {
     uint64_t n_evaluated;      /* pixel pairs whose separation was actually computed */
     uint64_t n_binned;         /* pixel pairs inside the grid (= sum_A N_A) */
     uint64_t n_kept;           /* lya_dmat: in-grid pixel pairs that passed the keep mask */
+    uint64_t n_scatter;        /* lya_dmat: fp64 scatter-adds into Dn/Wd issued by the fast kernel (0 for generic pairs) */
     float    ms_main;          /* device time of the dominant kernel (CUDA events on the ctx stream) */
     float    ms_total;         /* device time of the whole call */
 } lya_stats;

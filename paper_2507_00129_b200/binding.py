@@ -43,7 +43,7 @@ class CBinning(C.Structure):
 
 class CStats(C.Structure):
     _fields_ = [("n_forest_pairs", C.c_uint64), ("n_visited", C.c_uint64), ("n_evaluated", C.c_uint64),
-                ("n_binned", C.c_uint64), ("n_kept", C.c_uint64), ("ms_main", C.c_float), ("ms_total", C.c_float)]
+                ("n_binned", C.c_uint64), ("n_kept", C.c_uint64), ("n_scatter", C.c_uint64), ("ms_main", C.c_float), ("ms_total", C.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -336,7 +336,7 @@ struct DmFastParams {
     BinParams bp;
     unsigned long long seed, thr;
     double *Dn, *Wd;
-    unsigned long long *counters;   // [4] next chunk, [2] evaluated, [3] error, [5] kept, [6] binned
+    unsigned long long *counters;   // [4] next chunk, [2] evaluated, [3] error, [5] kept, [6] binned, [7] scatter-adds
 };
 
 struct __align__(16) DmFastWarp {
@@ -481,7 +481,7 @@ __device__ __forceinline__ void dm_walk_any(DmFastWarp &ws, unsigned h01, unsign
 // pass C: drain n queued kept pairs.  do_t123: also T1..T3 (false when only T4 is wanted).
 template <bool POW2>
 __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp, int mq, const DmFastParams &P,
-                                         const PairBin &g, int c0, int lane)
+                                         const PairBin &g, int c0, int lane, unsigned long long &n_red)
 {
     const BinParams &bp = P.bp;
     const int nb = bp.n_par * bp.n_perp, np1 = bp.n_par + 1;
@@ -493,6 +493,7 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
         const double om = ws.pw[i] * qw[j];
         atomicAdd(P.Dn + (size_t)A * nb + A, om);
         atomicAdd(P.Wd + A, om);
+        n_red += 2;
     }
     // T2, T3 (lanes over the pixels of q resp. p)
     for (int e = 0; e < n; ++e) {
@@ -503,11 +504,11 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
         const double pci = ws.pc[i], qcj = qc[j];
         for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {          // T2: (i, j') inside row i's window
             const int B = lya_pix_bin<POW2>(bp, g, pci, qc[j2]);
-            if (B >= 0) atomicAdd(row + B, -om * (qea[j2] + uj * qeg[j2]));
+            if (B >= 0) { atomicAdd(row + B, -om * (qea[j2] + uj * qeg[j2])); n_red += 1; }
         }
         for (int i2 = lane; i2 < mp; i2 += 32) {                             // T3: (i', j)
             const int B = lya_pix_bin<POW2>(bp, g, ws.pc[i2], qcj);
-            if (B >= 0) atomicAdd(row + B, -om * (ws.pea[i2] + ui * ws.peg[i2]));
+            if (B >= 0) { atomicAdd(row + B, -om * (ws.pea[i2] + ui * ws.peg[i2])); n_red += 1; }
         }
     }
     // T4: lanes over the non-zero table entries, inner loop over the kept pairs
@@ -523,6 +524,7 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
             const double v = (a.x + uj * a.y) + ui * (b.x + uj * b.y);
             atomicAdd(P.Dn + (size_t)A * nb + B, om * v);
         }
+        n_red += (unsigned long long)n;
     }
 }
 
@@ -541,7 +543,7 @@ __global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
     __syncwarp();
     const double *qc = ws.qc + FD_PAD;
     const unsigned h01 = (unsigned)__cvta_generic_to_shared(ws.H01), h23 = (unsigned)__cvta_generic_to_shared(ws.H23);
-    unsigned long long evaluated = 0, kept_total = 0, binned_total = 0;
+    unsigned long long evaluated = 0, kept_total = 0, binned_total = 0, n_red = 0;
     int cur_p = -1, head_p = -1;
     ForestHead hp;
     hp.len = 0;
@@ -655,7 +657,7 @@ __global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
             // ---- pass C ----
             const unsigned nk = ws.nkept;
             if (nk <= FD_KCAP) {
-                dm_drain<POW2>(ws, (int)nk, nnz, mp, mq, P, g, c0, lane);
+                dm_drain<POW2>(ws, (int)nk, nnz, mp, mq, P, g, c0, lane, n_red);
             } else {
                 // more kept pairs than the queue holds (small reject fractions): redo the mask row by row
                 int n_q = 0;
@@ -671,7 +673,7 @@ __global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
                         if (bal) {
                             if (n_q + __popc(bal) > FD_KCAP) {
                                 __syncwarp();
-                                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane);
+                                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane, n_red);
                                 __syncwarp();
                                 n_q = 0;
                             }
@@ -681,7 +683,7 @@ __global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
                     }
                 }
                 __syncwarp();
-                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane);
+                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane, n_red);
             }
             __syncwarp();
             // clear the table and the queue for the next pair
@@ -694,11 +696,13 @@ __global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
         evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
         kept_total += __shfl_xor_sync(0xffffffffu, kept_total, o);
         binned_total += __shfl_xor_sync(0xffffffffu, binned_total, o);
+        n_red += __shfl_xor_sync(0xffffffffu, n_red, o);
     }
     if (lane == 0) {
         atomicAdd(&P.counters[2], evaluated);
         atomicAdd(&P.counters[5], kept_total);
         atomicAdd(&P.counters[6], binned_total);
+        atomicAdd(&P.counters[7], n_red);
     }
 }
 
@@ -841,6 +845,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         stats->n_evaluated = h[2];
         stats->n_kept = h[5];
         stats->n_binned = h[6];
+        stats->n_scatter = h[7];
         cudaEventElapsedTime(&stats->ms_main, ctx->ev[0], ctx->ev[1]);
         cudaEventElapsedTime(&stats->ms_total, ctx->ev[3], ctx->ev[2]);
     }

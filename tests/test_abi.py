@@ -35,7 +35,7 @@ def test_struct_layouts_match_header():
     from paper_2507_00129_b200 import binding
     assert C.sizeof(binding.CForests) == 12 * 8
     assert C.sizeof(binding.CBinning) == 24
-    assert C.sizeof(binding.CStats) == 5 * 8 + 2 * 4
+    assert C.sizeof(binding.CStats) == 6 * 8 + 2 * 4
 
 
 def test_no_cpu_fallback(lib):
