@@ -169,9 +169,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-dmat", action="store_true")
-    ap.add_argument("--ref-forests", type=int, default=3000)
+    ap.add_argument("--ref-forests", type=int, default=8000)
     ap.add_argument("--ref-dmat-div", type=int, default=50)
-    ap.add_argument("--cpu-forests", type=int, default=3000)
+    ap.add_argument("--cpu-forests", type=int, default=12000)
     ap.add_argument("--forests", type=int, default=0,
                     help="profiling only: a shaped sub-catalogue of this many forests (same sky density)")
     args = ap.parse_args()
@@ -180,7 +180,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2507_00129_b200 import binding as B, build, gen
+    from paper_2507_00129_b200 import binding as B, build, gen, shard
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -199,7 +199,7 @@ def main():
     mseed = gen.mask_seed(wl["mask_cfg"])
     # weak scaling: every rank owns an independent catalogue of the same shape (seed + rank)
     f = gen.make_config(wl["cfg"], n_forest=args.forests or None,
-                        seed=None if rank == 0 else gen.SEED_BASE + wl["cfg"] + 1000 * rank)
+                        seed=shard.rank_seed(gen.SEED_BASE + wl["cfg"], rank))
     ctx = B.Context(f"cuda:{local}")
     d = B.DeviceForests(f, device=f"cuda:{local}")
     b = B.binning()
@@ -241,13 +241,7 @@ def main():
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     ms = ev0.elapsed_time(ev1)
-    t = torch.tensor([ms, float(pairs_total)], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        tmax = t.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms, pairs_all = float(tmax[0]), float(tsum[1])
-    else:
-        pairs_all = float(pairs_total)
+    ms, pairs_all = shard.aggregate(ms, float(pairs_total), device=f"cuda:{local}")
     value = pairs_all / (ms * 1e-3)
 
     # ---- e2e: host buffers through lya_run_host (pinned), copies inside the timed region ----
@@ -280,11 +274,7 @@ def main():
             pe += r["stats_xi"]["n_binned"] + (r["stats_dmat"]["n_binned"] if do_d else 0)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        te = torch.tensor([dt, float(pe)], dtype=torch.float64, device=f"cuda:{local}")
-        if world > 1:
-            tm = te.clone(); dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-            ts = te.clone(); dist.all_reduce(ts, op=dist.ReduceOp.SUM)
-            dt, pe = float(tm[0]), float(ts[1])
+        dt, pe = shard.aggregate(dt, float(pe), device=f"cuda:{local}")
         e2e = {"value": pe / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3}
 
