@@ -326,7 +326,7 @@ constexpr int FD_ROWS = 16;
 constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
 constexpr int FD_PAD = 2;
 constexpr int FD_SLOTS = 360;                // (n_par + 1) * (LYA_NCOL + 1) <= FD_SLOTS
-constexpr int FD_KCAP = 128;                 // kept pairs queued per drain
+constexpr int FD_KCAP = 48;                  // kept pairs queued per drain
 constexpr int FD_CHUNK = 8;
 
 struct DmFastParams {
@@ -345,6 +345,8 @@ struct __align__(16) DmFastWarp {
     double qc[FD_T + 2 * FD_PAD], qw[FD_T + 2 * FD_PAD], qu[FD_T + 2 * FD_PAD], qea[FD_T + 2 * FD_PAD], qeg[FD_T + 2 * FD_PAD];
     unsigned long long pk[FD_T], qk[FD_T];   // stage-4 keys of the pixels
     unsigned kept[FD_KCAP];                  // (i << 20) | (j << 12) | A
+    double2 kc01[FD_KCAP], kc23[FD_KCAP];    // per kept pair: om (1, u_j), om (u_i, u_i u_j)
+    double2 kgeo[FD_KCAP];                   // per kept pair: chi_i, chi_j
     unsigned short nz[FD_SLOTS];             // non-zero slots
     unsigned char jlo[FD_T], jx[FD_T], jhi[FD_T];
     unsigned nkept, pad_[3];
@@ -393,7 +395,10 @@ __device__ __forceinline__ bool dm_keep(unsigned long long klo, unsigned long lo
     return keep_pair(klo, khi, thr);
 }
 
-// pass A over rows [r0, r1] (a multiple of D rows; rows >= len are sentinels) and diagonals [dlo, dhi]
+// pass A over rows [r0, r1] (a multiple of D rows; rows >= len are sentinels) and diagonals [dlo, dhi].
+// Same scheme as k_xi_fast: a lane holds the H entry of its current run in registers (predicated
+// release / acquire around a warp barrier); the keys, mask and queueing of row i+1 are computed
+// between the acquire of row i and the FMAs that need it.
 template <int D, bool POW2>
 __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h23, int r0, int r1, int mq, int dlo, int dhi,
                                         int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned np1,
@@ -404,43 +409,48 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h
     const unsigned garbage = (LYA_NCOL * np1 + np1 - 1u) * 16u;
     for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
         const int dl = d0 + lane * D;
-        unsigned cur[D];
-        double h0[D], h1[D], h2[D], h3[D];
+        unsigned cur[D], key[D];
+        double h0[D], h1[D], h2[D], h3[D], fa[D], fg[D];
         double wc[D], wa[D], wg[D];                         // sliding window over q: chi, ea, eg
+        double pa_c, pg_c;
 #pragma unroll
         for (int k = 0; k < D; ++k) { cur[k] = garbage; h0[k] = 0.0; h1[k] = 0.0; h2[k] = 0.0; h3[k] = 0.0; }
+        // keys, mask and queueing of one row (i, window slot of diagonal k = (k + u) % D)
+        auto row_keys = [&](int i, int u, bool live, unsigned *key_o, double *fa_o, double *fg_o) {
+            const double pci = ws.pc[i];
+            const unsigned long long pki = ws.pk[min(i, FD_T - 1)];
 #pragma unroll
-        for (int k = 0; k < D - 1; ++k) {
+            for (int k = 0; k < D; ++k) {
+                const int sl = (k + u) % D;
+                bool valid; unsigned A;
+                key_o[k] = dm_key<POW2>(bp, g, pci, wc[sl], c0, np1, sgn, valid, A);
+                fa_o[k] = wa[sl]; fg_o[k] = wg[sl];
+                valid = valid && live;
+                const int j = i + dl + k;
+                const bool kp = valid && keep_pair(pki, ws.qk[min(max(j, 0), FD_T - 1)], thr);
+                binned += valid ? 1u : 0u;
+                if (kp) {                                    // ~1 % of the pairs at f = 0.99
+                    const unsigned idx = atomicAdd(&ws.nkept, 1u);
+                    if (idx < FD_KCAP) ws.kept[idx] = ((unsigned)i << 20) | ((unsigned)j << 12) | A;
+                    kept_n += 1u;
+                }
+            }
+        };
+#pragma unroll
+        for (int k = 0; k < D; ++k) {
             const int j = min(max(r0 + dl + k, -FD_PAD), mq + FD_PAD - 1);
             wc[k] = qc[j]; wa[k] = qea[j]; wg[k] = qeg[j];
         }
+        row_keys(r0, 0, true, key, fa, fg);
+        pa_c = ws.pea[r0]; pg_c = ws.peg[r0];
         evaluated += (unsigned long long)(r1 - r0 + 1) * D;
         for (int ib = r0; ib <= r1; ib += D) {
 #pragma unroll
             for (int u = 0; u < D; ++u) {
                 const int i = ib + u;
-                const double pci = ws.pc[i], pai = ws.pea[i], pgi = ws.peg[i];
-                const unsigned long long pki = ws.pk[min(i, FD_T - 1)];
-                const int jn = i + dl + D - 1;              // the lane's newest q pixel
-                {
-                    const int j = min(max(jn, -FD_PAD), mq + FD_PAD - 1);
-                    wc[(u + D - 1) % D] = qc[j]; wa[(u + D - 1) % D] = qea[j]; wg[(u + D - 1) % D] = qeg[j];
-                }
-                unsigned key[D];
                 bool ch[D];
 #pragma unroll
                 for (int k = 0; k < D; ++k) {
-                    const int sl = (k + u) % D;
-                    bool valid; unsigned A;
-                    key[k] = dm_key<POW2>(bp, g, pci, wc[sl], c0, np1, sgn, valid, A);
-                    const int j = jn - (D - 1) + k;
-                    const bool kp = valid && dm_keep(pki, ws.qk[min(max(j, 0), FD_T - 1)], thr);
-                    binned += valid ? 1u : 0u;
-                    if (kp) {                                // ~1 % of the pairs at f = 0.99
-                        const unsigned idx = atomicAdd(&ws.nkept, 1u);
-                        if (idx < FD_KCAP) ws.kept[idx] = ((unsigned)i << 20) | ((unsigned)j << 12) | A;
-                        kept_n += 1u;
-                    }
                     ch[k] = key[k] != cur[k];
                     dsts_v2_if(ch[k], h01 + cur[k], h0[k], h1[k]);                      // release
                     dsts_v2_if(ch[k], h23 + cur[k], h2[k], h3[k]);
@@ -448,13 +458,25 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h
                 __syncwarp();
 #pragma unroll
                 for (int k = 0; k < D; ++k) {
-                    const int sl = (k + u) % D;
                     dlds_v2_if(ch[k], h01 + key[k], h0[k], h1[k]);                      // acquire
                     dlds_v2_if(ch[k], h23 + key[k], h2[k], h3[k]);
                     cur[k] = key[k];
-                    h0[k] = fma(pai, wa[sl], h0[k]); h1[k] = fma(pai, wg[sl], h1[k]);
-                    h2[k] = fma(pgi, wa[sl], h2[k]); h3[k] = fma(pgi, wg[sl], h3[k]);
                 }
+                // row i + 1: its new q pixel replaces q[i + dl] in window slot u
+                unsigned key_n[D];
+                double fa_n[D], fg_n[D];
+                {
+                    const int j = min(max(i + dl + D, -FD_PAD), mq + FD_PAD - 1);
+                    wc[u] = qc[j]; wa[u] = qea[j]; wg[u] = qeg[j];
+                    row_keys(i + 1, u + 1, i + 1 <= r1, key_n, fa_n, fg_n);
+                }
+#pragma unroll
+                for (int k = 0; k < D; ++k) {
+                    h0[k] = fma(pa_c, fa[k], h0[k]); h1[k] = fma(pa_c, fg[k], h1[k]);
+                    h2[k] = fma(pg_c, fa[k], h2[k]); h3[k] = fma(pg_c, fg[k], h3[k]);
+                    fa[k] = fa_n[k]; fg[k] = fg_n[k]; key[k] = key_n[k];
+                }
+                pa_c = ws.pea[i + 1]; pg_c = ws.peg[i + 1];
             }
         }
 #pragma unroll
@@ -478,7 +500,7 @@ __device__ __forceinline__ void dm_walk_any(DmFastWarp &ws, unsigned h01, unsign
     else dm_walk<2, POW2>(ws, h01, h23, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, np1, thr, lane, binned, kept_n, evaluated);
 }
 
-// pass C: drain n queued kept pairs.  do_t123: also T1..T3 (false when only T4 is wanted).
+// pass C: drain n queued kept pairs.
 template <bool POW2>
 __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp, int mq, const DmFastParams &P,
                                          const PairBin &g, int c0, int lane, unsigned long long &n_red)
@@ -486,43 +508,47 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
     const BinParams &bp = P.bp;
     const int nb = bp.n_par * bp.n_perp, np1 = bp.n_par + 1;
     const double *qc = ws.qc + FD_PAD, *qw = ws.qw + FD_PAD, *qu = ws.qu + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
-    // T1: Dn[A][A] += om, Wd[A] += om (lanes over kept pairs)
+    // coefficients of every kept pair (lanes over kept pairs) and T1: Dn[A][A] += om, Wd[A] += om
     for (int e = lane; e < n; e += 32) {
         const unsigned rec = ws.kept[e];
         const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
-        const double om = ws.pw[i] * qw[j];
+        const double om = ws.pw[i] * qw[j], ui = ws.pu[i], uj = qu[j];
+        const double omi = om * ui;
+        ws.kc01[e] = make_double2(om, om * uj);
+        ws.kc23[e] = make_double2(omi, omi * uj);
+        ws.kgeo[e] = make_double2(ws.pc[i], qc[j]);
         atomicAdd(P.Dn + (size_t)A * nb + A, om);
         atomicAdd(P.Wd + A, om);
         n_red += 2;
     }
-    // T2, T3 (lanes over the pixels of q resp. p)
+    __syncwarp();
+    // T2: -(om ea_j' + om u_j eg_j') over row i's window;  T3: -(om ea_i' + om u_i eg_i') over p
     for (int e = 0; e < n; ++e) {
         const unsigned rec = ws.kept[e];
-        const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
-        const double om = ws.pw[i] * qw[j], ui = ws.pu[i], uj = qu[j];
+        const int i = rec >> 20, A = rec & 0xfff;
+        const double2 c01 = ws.kc01[e], c23 = ws.kc23[e], geo = ws.kgeo[e];
         double *row = P.Dn + (size_t)A * nb;
-        const double pci = ws.pc[i], qcj = qc[j];
-        for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {          // T2: (i, j') inside row i's window
-            const int B = lya_pix_bin<POW2>(bp, g, pci, qc[j2]);
-            if (B >= 0) { atomicAdd(row + B, -om * (qea[j2] + uj * qeg[j2])); n_red += 1; }
+        for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {
+            const int B = lya_pix_bin<POW2>(bp, g, geo.x, qc[j2]);
+            if (B >= 0) { atomicAdd(row + B, -fma(c01.y, qeg[j2], c01.x * qea[j2])); n_red += 1; }
         }
-        for (int i2 = lane; i2 < mp; i2 += 32) {                             // T3: (i', j)
-            const int B = lya_pix_bin<POW2>(bp, g, ws.pc[i2], qcj);
-            if (B >= 0) { atomicAdd(row + B, -om * (ws.pea[i2] + ui * ws.peg[i2])); n_red += 1; }
+        for (int i2 = lane; i2 < mp; i2 += 32) {
+            const int B = lya_pix_bin<POW2>(bp, g, ws.pc[i2], geo.y);
+            if (B >= 0) { atomicAdd(row + B, -fma(c23.x, ws.peg[i2], c01.x * ws.pea[i2])); n_red += 1; }
         }
     }
     // T4: lanes over the non-zero table entries, inner loop over the kept pairs
     for (int t = lane; t < nnz; t += 32) {
         const int slot = ws.nz[t];
         const int cr = slot / np1, bx = slot - cr * np1;
-        const int B = bx * bp.n_perp + c0 + cr;
+        double *colB = P.Dn + (bx * bp.n_perp + c0 + cr);
         const double2 a = ws.H01[slot], b = ws.H23[slot];
+#pragma unroll 2
         for (int e = 0; e < n; ++e) {
-            const unsigned rec = ws.kept[e];
-            const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
-            const double om = ws.pw[i] * qw[j], ui = ws.pu[i], uj = qu[j];
-            const double v = (a.x + uj * a.y) + ui * (b.x + uj * b.y);
-            atomicAdd(P.Dn + (size_t)A * nb + B, om * v);
+            const int A = ws.kept[e] & 0xfff;
+            const double2 c01 = ws.kc01[e], c23 = ws.kc23[e];
+            const double v = fma(c23.y, b.y, fma(c23.x, b.x, fma(c01.y, a.y, c01.x * a.x)));
+            atomicAdd(colB + (size_t)A * nb, v);
         }
         n_red += (unsigned long long)n;
     }
