@@ -115,18 +115,19 @@ __device__ void drain_kept(DmWarpSmem &ws, int n_kept, int mp, int mq, const DmP
         const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
         const double om = ws.pw[i] * qw[j];
         const double ui = ws.pu[i], uj = qu[j];
-        double *row = P.Dn + (size_t)A * nb;
+        const int At = lya_bin_tr(bp, A);                                  // Dn, Wd are accumulated in transposed bin order
+        double *row = P.Dn + (size_t)At * nb;
         if (first_chunk) {
-            if (lane == 0) { red_add(row + A, om); red_add(P.Wd + A, om); }
+            if (lane == 0) { red_add(row + At, om); red_add(P.Wd + At, om); }
             for (int j2 = lane; j2 < mq; j2 += 32) {                       // T2
-                int B = lya_pix_bin<POW2>(bp, g, ws.pc[i], qc[j2]);
+                int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i], qc[j2]);
                 if (B >= 0) {
                     double aj = qw[j2] * invSq, gj = qw[j2] * qu[j2] * invVq;
                     red_add(row + B, -om * (aj + uj * gj));
                 }
             }
             for (int i2 = lane; i2 < mp; i2 += 32) {                       // T3
-                int B = lya_pix_bin<POW2>(bp, g, ws.pc[i2], qc[j]);
+                int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i2], qc[j]);
                 if (B >= 0) {
                     double ai = ws.pw[i2] * invSp, gi = ws.pw[i2] * ws.pu[i2] * invVp;
                     red_add(row + B, -om * (ai + ui * gi));
@@ -138,7 +139,7 @@ __device__ void drain_kept(DmWarpSmem &ws, int n_kept, int mp, int mq, const DmP
             double haa = ws.H[0][t];
             if (haa != 0.0 || ws.H[3][t] != 0.0 || ws.H[1][t] != 0.0 || ws.H[2][t] != 0.0) {
                 int bx = t / ncol, lc = t - bx * ncol;
-                int B = bx * bp.n_perp + c0 + lc;
+                int B = (c0 + lc) * bp.n_par + bx;
                 double v = haa + uj * ws.H[1][t] + ui * ws.H[2][t] + ui * uj * ws.H[3][t];
                 red_add(row + B, om * v);
             }
@@ -319,13 +320,13 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
 //  pass C  the kept pairs are drained: T1..T3 per kept pair, T4 with lanes over the table entries and
 //          an inner loop over the kept pairs (the entry stays in registers); every update is one
 //          red.global.add.f64 into the L2-resident Dn.
-constexpr int FD_WARPS = 5;
+constexpr int FD_WARPS = 11;                 // one CTA per SM (shared memory: 20.3 KB per warp)
 constexpr int FD_THREADS = FD_WARPS * 32;
 constexpr int FD_T = LYA_FAST_TILE;
 constexpr int FD_ROWS = 16;
 constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
 constexpr int FD_PAD = 2;
-constexpr int FD_SLOTS = 360;                // (n_par + 1) * (LYA_NCOL + 1) <= FD_SLOTS
+constexpr int FD_SLOTS = 306;                // (n_par + 1) * LYA_NCOL <= FD_SLOTS
 constexpr int FD_KCAP = 48;                  // kept pairs queued per drain
 constexpr int FD_CHUNK = 8;
 
@@ -383,9 +384,9 @@ __device__ __forceinline__ unsigned dm_key(const BinParams &bp, const PairBin &g
     }
     const bool side = ((__double2hiint(d) ^ sgn) >= 0);
     valid = side & (bx < (unsigned)bp.n_par) & (by < (unsigned)bp.n_perp);
-    A = bx * (unsigned)bp.n_perp + by;
-    bx = valid ? bx : np1 - 1u;
-    const unsigned col = min(by - c0, (unsigned)LYA_NCOL);
+    A = by * (unsigned)bp.n_par + bx;                   // transposed bin order (see lya_pix_bin_t)
+    bx = valid ? bx : np1 - 1u;                          // everything else -> the garbage entry (0, n_par)
+    const unsigned col = valid ? by - c0 : 0u;
     return (col * np1 + bx) * 16u;
 }
 
@@ -406,7 +407,7 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h
                                         unsigned long long &evaluated)
 {
     const double *qc = ws.qc + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
-    const unsigned garbage = (LYA_NCOL * np1 + np1 - 1u) * 16u;
+    const unsigned garbage = (np1 - 1u) * 16u;
     for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
         const int dl = d0 + lane * D;
         unsigned cur[D], key[D];
@@ -529,11 +530,11 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
         const double2 c01 = ws.kc01[e], c23 = ws.kc23[e], geo = ws.kgeo[e];
         double *row = P.Dn + (size_t)A * nb;
         for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {
-            const int B = lya_pix_bin<POW2>(bp, g, geo.x, qc[j2]);
+            const int B = lya_pix_bin_t<POW2>(bp, g, geo.x, qc[j2]);
             if (B >= 0) { atomicAdd(row + B, -fma(c01.y, qeg[j2], c01.x * qea[j2])); n_red += 1; }
         }
         for (int i2 = lane; i2 < mp; i2 += 32) {
-            const int B = lya_pix_bin<POW2>(bp, g, ws.pc[i2], geo.y);
+            const int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i2], geo.y);
             if (B >= 0) { atomicAdd(row + B, -fma(c23.x, ws.peg[i2], c01.x * ws.pea[i2])); n_red += 1; }
         }
     }
@@ -541,7 +542,7 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
     for (int t = lane; t < nnz; t += 32) {
         const int slot = ws.nz[t];
         const int cr = slot / np1, bx = slot - cr * np1;
-        double *colB = P.Dn + (bx * bp.n_perp + c0 + cr);
+        double *colB = P.Dn + ((c0 + cr) * bp.n_par + bx);
         const double2 a = ws.H01[slot], b = ws.H23[slot];
 #pragma unroll 2
         for (int e = 0; e < n; ++e) {
@@ -555,14 +556,14 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
 }
 
 template <bool POW2>
-__global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
+__global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     DmFastWarp &ws = ((DmFastWarp *)smem_raw)[wid];
     const BinParams bp = P.bp;
     const unsigned np1 = (unsigned)bp.n_par + 1u;
-    const int n_slots = (int)np1 * (LYA_NCOL + 1);
+    const int n_slots = (int)np1 * LYA_NCOL;
     for (int t = lane; t < FD_SLOTS; t += 32) { ws.H01[t] = make_double2(0.0, 0.0); ws.H23[t] = make_double2(0.0, 0.0); }
     if (lane < FD_PAD) { ws.qc[lane] = LYA_CHI_SENTINEL; ws.qw[lane] = 0.0; ws.qu[lane] = 0.0; ws.qea[lane] = 0.0; ws.qeg[lane] = 0.0; }
     if (lane == 0) ws.nkept = 0u;
@@ -693,7 +694,7 @@ __global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
                     for (int j0 = ws.jlo[i]; j0 < ws.jhi[i]; j0 += 32) {
                         const int j = j0 + lane;
                         int A = -1;
-                        if (j < ws.jhi[i]) A = lya_pix_bin<POW2>(bp, g, pci, qc[j]);
+                        if (j < ws.jhi[i]) A = lya_pix_bin_t<POW2>(bp, g, pci, qc[j]);
                         const bool kp = (A >= 0) && keep_pair(ki, ws.qk[min(j, FD_T - 1)], P.thr);
                         const unsigned bal = __ballot_sync(0xffffffffu, kp);
                         if (bal) {
@@ -732,12 +733,20 @@ __global__ void __launch_bounds__(FD_THREADS, 2) k_dmat_fast(DmFastParams P)
     }
 }
 
-__global__ void k_dmat_normalise(const double *Dn, const double *Wd, int nb, double *D)
+// Dn_t, Wd_t: accumulators in transposed bin order.  Writes the API-order outputs (any may be NULL):
+// D[A][B] = Dn[A][B] / Wd[A] (row 0 where Wd[A] == 0), Dn, Wd.
+__global__ void k_dmat_normalise(const double *Dn_t, const double *Wd_t, BinParams bp, double *D, double *Dn, double *Wd)
 {
+    const int nb = bp.n_par * bp.n_perp;
     int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (idx >= (int64_t)nb * nb) return;
-    double wd = Wd[idx / nb];
-    D[idx] = (wd != 0.0) ? Dn[idx] / wd : 0.0;
+    const int A = (int)(idx / nb), B = (int)(idx - (int64_t)A * nb);
+    const int ax = A / bp.n_perp, ay = A - ax * bp.n_perp, bx = B / bp.n_perp, by = B - bx * bp.n_perp;
+    const int At = ay * bp.n_par + ax, Bt = by * bp.n_par + bx;
+    const double wd = Wd_t[At], v = Dn_t[(size_t)At * nb + Bt];
+    if (D) D[idx] = (wd != 0.0) ? v / wd : 0.0;
+    if (Dn) Dn[idx] = v;
+    if (Wd && B == 0) Wd[A] = wd;
 }
 
 }  // namespace
@@ -767,11 +776,11 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     const int nb = b->n_par * b->n_perp;
     cudaStream_t s = ctx->stream;
     const BinParams bp = lya_make_binparams(b);
-    const bool use_fast = pairs->n > 0 && (b->n_par + 1) * (LYA_NCOL + 1) <= FD_SLOTS && b->n_perp + 2 <= 256 &&
+    const bool use_fast = pairs->n > 0 && (b->n_par + 1) * LYA_NCOL <= FD_SLOTS && b->n_perp + 2 <= 256 &&
                           ctx->dmat_variant != 9;
     if (!use_fast && max_len > DTILE)
         return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: forests longer than %d pixels are not supported with this binning", DTILE);
-    double *scal = NULL, *Dn = Dn_out, *Wd = Wd_out;
+    double *scal = NULL, *Dn = NULL, *Wd = NULL;          // internal accumulators (transposed bin order)
     bool own_Dn = false, own_Wd = false;
     const int64_t nf = f->n_forest;
     LyaPrep prep;
@@ -824,7 +833,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp; F.seed = seed; F.thr = thr;
         F.Dn = Dn; F.Wd = Wd; F.counters = ctx->d_counters;
         const size_t fsmem = sizeof(DmFastWarp) * FD_WARPS;
-        const int fgrid = ctx->sm_count * 2;
+        const int fgrid = ctx->sm_count;
         if (bp.pow2) {
             e = cudaFuncSetAttribute(k_dmat_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
             if (e == cudaSuccess) k_dmat_fast<true><<<fgrid, FD_THREADS, fsmem, s>>>(F);
@@ -850,7 +859,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_dmat launch"); }
     }
     cudaEventRecord(ctx->ev[1], s);
-    if (D) k_dmat_normalise<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, s>>>(Dn, Wd, nb, D);
+    k_dmat_normalise<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, s>>>(Dn, Wd, bp, D, Dn_out, Wd_out);
     cudaEventRecord(ctx->ev[2], s);
     unsigned long long h[8];
     e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);

@@ -168,6 +168,35 @@ __device__ __forceinline__ int lya_pix_bin(const BinParams &bp, const PairBin &g
     }
 }
 
+// Same bin test, TRANSPOSED index b_perp * n_par + b_par (the internal order of the D accumulator:
+// the bins a forest pair touches are then contiguous runs of b_par inside <= 6 columns).
+template <bool POW2>
+__device__ __forceinline__ int lya_pix_bin_t(const BinParams &bp, const PairBin &g, double chi_i, double chi_j)
+{
+    double d = __dsub_rn(chi_i, chi_j);
+    double t = __dadd_rn(chi_i, chi_j);
+    unsigned bx, by;
+    bool ok;
+    if (POW2) {
+        bx = lya_floor_u32(__dmul_rn(fabs(d), g.cx));
+        by = lya_floor_u32(__dmul_rn(t, g.sy));
+        ok = (bx < (unsigned)bp.n_par) & (by < (unsigned)bp.n_perp);
+    } else {
+        double rpar = __dmul_rn(fabs(d), g.c);
+        double rperp = __dmul_rn(t, g.s);
+        ok = (rpar < bp.rpar_max) & (rperp < bp.rperp_max);
+        bx = min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1));
+        by = min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1));
+    }
+    return ok ? (int)(by * (unsigned)bp.n_par + bx) : -1;
+}
+// API bin index (b_par * n_perp + b_perp) -> transposed
+__device__ __forceinline__ int lya_bin_tr(const BinParams &bp, int A)
+{
+    const int bx = A / bp.n_perp;
+    return (A - bx * bp.n_perp) * bp.n_par + bx;
+}
+
 __device__ __forceinline__ PairBin lya_make_pairbin(const BinParams &bp, double s, double c)
 {
     PairBin g;
