@@ -320,14 +320,15 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
 //  pass C  the kept pairs are drained: T1..T3 per kept pair, T4 with lanes over the table entries and
 //          an inner loop over the kept pairs (the entry stays in registers); every update is one
 //          red.global.add.f64 into the L2-resident Dn.
-constexpr int FD_WARPS = 11;                 // one CTA per SM (shared memory: 20.3 KB per warp)
+constexpr int FD_WARPS = 13;                 // one CTA per SM (shared memory: 17.2 KB per warp)
 constexpr int FD_THREADS = FD_WARPS * 32;
 constexpr int FD_T = LYA_FAST_TILE;
 constexpr int FD_ROWS = 16;
 constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
 constexpr int FD_PAD = 2;
 constexpr int FD_SLOTS = 306;                // (n_par + 1) * LYA_NCOL <= FD_SLOTS
-constexpr int FD_KCAP = 48;                  // kept pairs queued per drain
+constexpr int FD_KCAP = 96;                  // kept pairs queued per forest pair
+constexpr int FD_KBATCH = 32;                // kept pairs drained together (coefficient tables)
 constexpr int FD_CHUNK = 8;
 
 struct DmFastParams {
@@ -342,12 +343,12 @@ struct DmFastParams {
 
 struct __align__(16) DmFastWarp {
     double2 H01[FD_SLOTS], H23[FD_SLOTS];    // (H_aa, H_ag), (H_ga, H_gg) per slot = col_rel * (n_par + 1) + row
-    double pc[FD_TP], pw[FD_TP], pu[FD_TP], pea[FD_TP], peg[FD_TP];
-    double qc[FD_T + 2 * FD_PAD], qw[FD_T + 2 * FD_PAD], qu[FD_T + 2 * FD_PAD], qea[FD_T + 2 * FD_PAD], qeg[FD_T + 2 * FD_PAD];
+    double pc[FD_TP], pea[FD_TP], peg[FD_TP];            // (w and u of the kept pairs are read from HBM/L2 in the drain)
+    double qc[FD_T + 2 * FD_PAD], qea[FD_T + 2 * FD_PAD], qeg[FD_T + 2 * FD_PAD];
     unsigned long long pk[FD_T], qk[FD_T];   // stage-4 keys of the pixels
     unsigned kept[FD_KCAP];                  // (i << 20) | (j << 12) | A
-    double2 kc01[FD_KCAP], kc23[FD_KCAP];    // per kept pair: om (1, u_j), om (u_i, u_i u_j)
-    double2 kgeo[FD_KCAP];                   // per kept pair: chi_i, chi_j
+    double2 kc01[FD_KBATCH], kc23[FD_KBATCH]; // per kept pair of a batch: om (1, u_j), om (u_i, u_i u_j)
+    double2 kgeo[FD_KBATCH];                 // per kept pair of a batch: chi_i, chi_j
     unsigned short nz[FD_SLOTS];             // non-zero slots
     unsigned char jlo[FD_T], jx[FD_T], jhi[FD_T];
     unsigned nkept, pad_[3];
@@ -503,17 +504,18 @@ __device__ __forceinline__ void dm_walk_any(DmFastWarp &ws, unsigned h01, unsign
 
 // pass C: drain n queued kept pairs.
 template <bool POW2>
-__device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp, int mq, const DmFastParams &P,
-                                         const PairBin &g, int c0, int lane, unsigned long long &n_red)
+__device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, const unsigned *kept, int n, int nnz, int mp, int mq, const DmFastParams &P,
+                                         const PairBin &g, int c0, long long offp, long long offq, int lane,
+                                         unsigned long long &n_red)
 {
     const BinParams &bp = P.bp;
     const int nb = bp.n_par * bp.n_perp, np1 = bp.n_par + 1;
-    const double *qc = ws.qc + FD_PAD, *qw = ws.qw + FD_PAD, *qu = ws.qu + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
+    const double *qc = ws.qc + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
     // coefficients of every kept pair (lanes over kept pairs) and T1: Dn[A][A] += om, Wd[A] += om
     for (int e = lane; e < n; e += 32) {
-        const unsigned rec = ws.kept[e];
+        const unsigned rec = kept[e];
         const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
-        const double om = ws.pw[i] * qw[j], ui = ws.pu[i], uj = qu[j];
+        const double om = P.prep.w[offp + i] * P.prep.w[offq + j], ui = P.prep.u[offp + i], uj = P.prep.u[offq + j];
         const double omi = om * ui;
         ws.kc01[e] = make_double2(om, om * uj);
         ws.kc23[e] = make_double2(omi, omi * uj);
@@ -525,7 +527,7 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
     __syncwarp();
     // T2: -(om ea_j' + om u_j eg_j') over row i's window;  T3: -(om ea_i' + om u_i eg_i') over p
     for (int e = 0; e < n; ++e) {
-        const unsigned rec = ws.kept[e];
+        const unsigned rec = kept[e];
         const int i = rec >> 20, A = rec & 0xfff;
         const double2 c01 = ws.kc01[e], c23 = ws.kc23[e], geo = ws.kgeo[e];
         double *row = P.Dn + (size_t)A * nb;
@@ -546,12 +548,23 @@ __device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp,
         const double2 a = ws.H01[slot], b = ws.H23[slot];
 #pragma unroll 2
         for (int e = 0; e < n; ++e) {
-            const int A = ws.kept[e] & 0xfff;
+            const int A = kept[e] & 0xfff;
             const double2 c01 = ws.kc01[e], c23 = ws.kc23[e];
             const double v = fma(c23.y, b.y, fma(c23.x, b.x, fma(c01.y, a.y, c01.x * a.x)));
             atomicAdd(colB + (size_t)A * nb, v);
         }
         n_red += (unsigned long long)n;
+    }
+}
+
+template <bool POW2>
+__device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp, int mq, const DmFastParams &P,
+                                         const PairBin &g, int c0, long long offp, long long offq, int lane,
+                                         unsigned long long &n_red)
+{
+    for (int e0 = 0; e0 < n; e0 += FD_KBATCH) {
+        dm_drain_batch<POW2>(ws, ws.kept + e0, min(FD_KBATCH, n - e0), nnz, mp, mq, P, g, c0, offp, offq, lane, n_red);
+        __syncwarp();
     }
 }
 
@@ -565,7 +578,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
     const unsigned np1 = (unsigned)bp.n_par + 1u;
     const int n_slots = (int)np1 * LYA_NCOL;
     for (int t = lane; t < FD_SLOTS; t += 32) { ws.H01[t] = make_double2(0.0, 0.0); ws.H23[t] = make_double2(0.0, 0.0); }
-    if (lane < FD_PAD) { ws.qc[lane] = LYA_CHI_SENTINEL; ws.qw[lane] = 0.0; ws.qu[lane] = 0.0; ws.qea[lane] = 0.0; ws.qeg[lane] = 0.0; }
+    if (lane < FD_PAD) { ws.qc[lane] = LYA_CHI_SENTINEL; ws.qea[lane] = 0.0; ws.qeg[lane] = 0.0; }
     if (lane == 0) ws.nkept = 0u;
     __syncwarp();
     const double *qc = ws.qc + FD_PAD;
@@ -599,33 +612,29 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
             __syncwarp();
             if (p != cur_p) {
-                const double2 *s0 = (const double2 *)(P.prep.chi + hp.off), *s1 = (const double2 *)(P.prep.w + hp.off),
-                              *s2 = (const double2 *)(P.prep.u + hp.off), *s3 = (const double2 *)(P.prep.ea + hp.off),
+                const double2 *s0 = (const double2 *)(P.prep.chi + hp.off), *s3 = (const double2 *)(P.prep.ea + hp.off),
                               *s4 = (const double2 *)(P.prep.eg + hp.off);
                 for (int t = lane; 2 * t < mp; t += 32) {
-                    ((double2 *)ws.pc)[t] = s0[t]; ((double2 *)ws.pw)[t] = s1[t]; ((double2 *)ws.pu)[t] = s2[t];
-                    ((double2 *)ws.pea)[t] = s3[t]; ((double2 *)ws.peg)[t] = s4[t];
+                    ((double2 *)ws.pc)[t] = s0[t]; ((double2 *)ws.pea)[t] = s3[t]; ((double2 *)ws.peg)[t] = s4[t];
                 }
                 for (int t = lane; t < mp; t += 32) ws.pk[t] = key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
                 __syncwarp();
                 for (int t = mp + lane; t < FD_TP; t += 32) {            // sentinel rows (!= q's sentinel: r_par never 0)
-                    ws.pc[t] = 2.0 * LYA_CHI_SENTINEL; ws.pw[t] = 0.0; ws.pu[t] = 0.0; ws.pea[t] = 0.0; ws.peg[t] = 0.0;
+                    ws.pc[t] = 2.0 * LYA_CHI_SENTINEL; ws.pea[t] = 0.0; ws.peg[t] = 0.0;
                 }
                 cur_p = p;
             }
             {
-                const double2 *s0 = (const double2 *)(P.prep.chi + hq.off), *s1 = (const double2 *)(P.prep.w + hq.off),
-                              *s2 = (const double2 *)(P.prep.u + hq.off), *s3 = (const double2 *)(P.prep.ea + hq.off),
+                const double2 *s0 = (const double2 *)(P.prep.chi + hq.off), *s3 = (const double2 *)(P.prep.ea + hq.off),
                               *s4 = (const double2 *)(P.prep.eg + hq.off);
                 const int npad2 = (mq + 1) >> 1;
                 for (int t = lane; t < npad2; t += 32) {
-                    ((double2 *)qc)[t] = s0[t]; ((double2 *)(ws.qw + FD_PAD))[t] = s1[t]; ((double2 *)(ws.qu + FD_PAD))[t] = s2[t];
-                    ((double2 *)(ws.qea + FD_PAD))[t] = s3[t]; ((double2 *)(ws.qeg + FD_PAD))[t] = s4[t];
+                    ((double2 *)qc)[t] = s0[t]; ((double2 *)(ws.qea + FD_PAD))[t] = s3[t]; ((double2 *)(ws.qeg + FD_PAD))[t] = s4[t];
                 }
                 for (int t = lane; t < mq; t += 32) ws.qk[t] = key_hi(P.seed, (unsigned long long)(hq.pix0 + t));
                 if (lane < FD_PAD) {
                     const int j = FD_PAD + 2 * npad2 + lane;
-                    ws.qc[j] = LYA_CHI_SENTINEL; ws.qw[j] = 0.0; ws.qu[j] = 0.0; ws.qea[j] = 0.0; ws.qeg[j] = 0.0;
+                    ws.qc[j] = LYA_CHI_SENTINEL; ws.qea[j] = 0.0; ws.qeg[j] = 0.0;
                 }
             }
             __syncwarp();
@@ -684,7 +693,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             // ---- pass C ----
             const unsigned nk = ws.nkept;
             if (nk <= FD_KCAP) {
-                dm_drain<POW2>(ws, (int)nk, nnz, mp, mq, P, g, c0, lane, n_red);
+                dm_drain<POW2>(ws, (int)nk, nnz, mp, mq, P, g, c0, hp.off, hq.off, lane, n_red);
             } else {
                 // more kept pairs than the queue holds (small reject fractions): redo the mask row by row
                 int n_q = 0;
@@ -700,7 +709,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                         if (bal) {
                             if (n_q + __popc(bal) > FD_KCAP) {
                                 __syncwarp();
-                                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane, n_red);
+                                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, hp.off, hq.off, lane, n_red);
                                 __syncwarp();
                                 n_q = 0;
                             }
@@ -710,7 +719,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                     }
                 }
                 __syncwarp();
-                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, lane, n_red);
+                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, hp.off, hq.off, lane, n_red);
             }
             __syncwarp();
             // clear the table and the queue for the next pair
