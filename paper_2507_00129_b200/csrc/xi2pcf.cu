@@ -265,13 +265,13 @@ cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
 }
 
 // ======================= fast kernel: warp-private sub-histograms ================================
-constexpr int FW = 6;                        // warps per block
+constexpr int FW = 14;                       // warps per block, one block per SM (16.2 KB of shared memory per warp)
 constexpr int FTHREADS = FW * 32;
 constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
 constexpr int FROWS = 16;                    // rows of p walked per pass (keeps lanes busy: DESIGN.md)
 constexpr int FTP = ((FT + FROWS - 1) / FROWS) * FROWS + 2;   // p rows incl. sentinel rows
 constexpr int FPAD = 2;                      // sentinel pixels either side of q (reads are clamped)
-constexpr int FSLOTS = 714;                  // 2 * (n_par + 1) * (LYA_NCOL + 1) <= FSLOTS
+constexpr int FSLOTS = 612;                  // 2 * (n_par + 1) * LYA_NCOL <= FSLOTS
 constexpr int FCHUNK = 16;                   // forest pairs claimed per atomic
 
 struct XiFastParams {
@@ -286,8 +286,8 @@ struct XiFastParams {
 
 // Sub-histogram slot = col_rel * 2 (n_par + 1) + side * (n_par + 1) + row.
 //   side: 0 when chi_i >= chi_j, 1 otherwise (the two sides of a bin are added when the warp merges);
-//   row n_par and col_rel LYA_NCOL are GARBAGE (pixel pair outside the grid / a sentinel pixel), so
-//   the pair loop needs no validity test; garbage slots are dropped by the merge.
+//   row n_par is GARBAGE: a pixel pair outside the grid (or a sentinel pixel) maps to entry
+//   (column 0, side 0, row n_par), so the pair loop has no validity branch; the merge drops that row.
 struct __align__(16) FastWarp {
     double2 SW[FSLOTS];                      // (S, W) per slot
     unsigned N[(FSLOTS + 3) & ~3];           // (padded: the arrays below need 16-byte alignment)
@@ -334,8 +334,9 @@ __device__ __forceinline__ unsigned xi_key(const BinParams &bp, const PairBin &g
         bx = (rpar < bp.rpar_max) ? min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1)) : (unsigned)bp.n_par;
         by = (rperp < bp.rperp_max) ? min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1)) : 0x7fffffffu;
     }
-    bx = min(bx, np1 - 1u);
-    const unsigned col = min(by - c0, (unsigned)LYA_NCOL);
+    const bool valid = (bx < np1 - 1u) & (by - c0 < (unsigned)LYA_NCOL);   // else -> the garbage entry (0, n_par)
+    bx = valid ? bx : np1 - 1u;
+    const unsigned col = valid ? by - c0 : 0u;
     const unsigned side = (unsigned)__double2hiint(d) >> 31;
     return (col * (2u * np1) + side * np1 + bx) * 16u;
 }
@@ -354,7 +355,7 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
                                         unsigned np1, int lane, unsigned long long &evaluated)
 {
     const double *qc = ws.qc + FPAD, *qa = ws.qa + FPAD, *qw = ws.qw + FPAD;
-    const unsigned garbage = (LYA_NCOL * 2u * np1 + np1 - 1u) * 16u;  // what a sentinel pixel maps to
+    const unsigned garbage = (np1 - 1u) * 16u;              // entry (column 0, side 0, row n_par)
     for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
         const int dl = d0 + lane * D;                       // first diagonal of this lane
         unsigned cur[D], cnt[D], key[D];
@@ -443,7 +444,7 @@ __device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, in
 {
     const int np1 = P.bp.n_par + 1;
     __syncwarp();
-    for (int t = lane; t < np1 * (LYA_NCOL + 1); t += 32) {      // t = col_rel * np1 + row
+    for (int t = lane; t < np1 * LYA_NCOL; t += 32) {            // t = col_rel * np1 + row
         const int cr = t / np1, bx = t - cr * np1, col = c0 + cr;
         const int s0 = cr * 2 * np1 + bx, s1 = s0 + np1;          // the two sides of the bin
         const unsigned n = ws.N[s0] + ws.N[s1];
@@ -463,7 +464,7 @@ __device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, in
 }
 
 template <bool POW2>
-__global__ void __launch_bounds__(FTHREADS, 2) k_xi_fast(XiFastParams P)
+__global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -586,7 +587,7 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
     cudaStream_t s = ctx->stream;
     const BinParams bp = lya_make_binparams(b);
     // fast path: bucketed list + warp-private sub-histograms (variant 9 forces the generic kernel)
-    const bool use_fast = pairs->n > 0 && 2 * (b->n_par + 1) * (LYA_NCOL + 1) <= FSLOTS && b->n_perp + 2 <= 256 && ctx->xi_variant != 9;
+    const bool use_fast = pairs->n > 0 && 2 * (b->n_par + 1) * LYA_NCOL <= FSLOTS && b->n_perp + 2 <= 256 && ctx->xi_variant != 9;
     LyaPrep prep;
     LyaBuckets bk;
     memset(&prep, 0, sizeof(prep));
@@ -623,7 +624,7 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
         F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
         F.S = P.S; F.W = P.W; F.N = P.N; F.counters = ctx->d_counters;
         const size_t fsmem = sizeof(FastWarp) * FW;
-        const int fgrid = ctx->sm_count * 2;
+        const int fgrid = ctx->sm_count;
         if (bp.pow2) {
             e = cudaFuncSetAttribute(k_xi_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
             if (e == cudaSuccess) k_xi_fast<true><<<fgrid, FTHREADS, fsmem, s>>>(F);
