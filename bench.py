@@ -146,7 +146,7 @@ def cpu_baseline(wl, budget_forests):
     t0 = time.perf_counter()
     x = orc.xi(cat, pq)
     t_xi = time.perf_counter() - t0
-    pq_d = pq[: max(1, len(pq) // 50)]
+    pq_d = pq[: max(1, len(pq) // 8)]
     frac = 0.0 if wl["cfg"] == 0 else 0.99
     t0 = time.perf_counter()
     orc.dmat(cat, pq_d, frac, gen.mask_seed(wl["mask_cfg"]), want_D=False)
