@@ -201,6 +201,42 @@ def test_long_and_ragged_forests_tiles(ctx, B, orc):
     check_xi(ctx.lya_xi2pcf(d, B.binning(), pairs), orc.xi(f, ref), "long forests")
 
 
+def test_kernel_routes_fast_and_generic(B, orc, monkeypatch):
+    """The same catalogue through (a) the fast kernels (bucketed list, warp-private tables), (b) the
+    generic kernels forced for the whole list, (c) a grid whose 8 Mpc/h r_par bins exceed the pixel
+    spacing, so that the bucketing pass itself routes every pair to the generic kernels, and (d) a grid
+    with more r_par rows than a sub-histogram holds.  All match the oracle; (a) and (b) agree exactly
+    on the integers."""
+    f = gen.make_config(4, n_forest=400)
+    pq = orc.pairs_window(f)
+    pq_d = pq[:400]
+    seed = gen.mask_seed(4)
+    ox, od = orc.xi(f, pq), orc.dmat(f, pq_d, 0.9, seed)
+    res = {}
+    for variant in ("0", "9"):
+        monkeypatch.setenv("LYA_XI_VARIANT", variant)
+        monkeypatch.setenv("LYA_DMAT_VARIANT", variant)
+        c = B.Context("cuda:0")
+        d = B.DeviceForests(f)
+        gx = c.lya_xi2pcf(d, B.binning(), c.lya_pairs_import(pq))
+        gd = c.lya_dmat(d, B.binning(), c.lya_pairs_import(pq_d), 0.9, seed)
+        check_xi(gx, ox, f"variant {variant}")
+        check_dmat(gd, od, f"variant {variant} D")
+        res[variant] = (gx["N"].cpu().numpy().copy(), gd["stats"]["n_kept"], gd["stats"]["n_binned"], gd["stats"]["n_scatter"])
+        c.close()
+    assert np.array_equal(res["0"][0], res["9"][0]) and res["0"][1:3] == res["9"][1:3]
+    assert res["0"][3] > 0 and res["9"][3] == 0            # scatter-adds are counted by the fast kernel only
+    monkeypatch.delenv("LYA_XI_VARIANT"); monkeypatch.delenv("LYA_DMAT_VARIANT")
+    c = B.Context("cuda:0")
+    d = B.DeviceForests(f)
+    for (rp, rt, n_par, n_perp) in ((200.0, 200.0, 25, 25), (200.0, 200.0, 64, 50)):
+        b, ob = B.binning(rp, rt, n_par, n_perp), orc.binning(rp, rt, n_par, n_perp)
+        check_xi(c.lya_xi2pcf(d, b, c.lya_pairs_import(pq)), orc.xi(f, pq, ob), f"grid {n_par}x{n_perp}")
+        check_dmat(c.lya_dmat(d, b, c.lya_pairs_import(pq_d), 0.9, seed), orc.dmat(f, pq_d, 0.9, seed, b=ob),
+                   f"grid {n_par}x{n_perp} D")
+    c.close()
+
+
 # ------------------------------------------------------------------ invariances and edge cases
 def test_P7_pair_order_and_swap(ctx, B, orc, cfg0):
     d = B.DeviceForests(cfg0)
