@@ -670,8 +670,10 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 nlo = __reduce_min_sync(0xffffffffu, nlo); nhi = __reduce_max_sync(0xffffffffu, nhi);
                 r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
                 if (r1 < r0) continue;
-                dm_walk_any<POW2>(ws, h01, h23, r0 & ~1, r1 | 1, mq, plo, phi, 0, bp, g, (unsigned)c0, np1, P.thr, lane, binned, kept_n, evaluated);
-                dm_walk_any<POW2>(ws, h01, h23, r0 & ~1, r1 | 1, mq, nlo, nhi, -1, bp, g, (unsigned)c0, np1, P.thr, lane, binned, kept_n, evaluated);
+#pragma unroll 1
+                for (int sgn = 0; sgn >= -1; --sgn)         // one call site: chi_i >= chi_j, then chi_i < chi_j
+                    dm_walk_any<POW2>(ws, h01, h23, r0 & ~1, r1 | 1, mq, sgn ? nlo : plo, sgn ? nhi : phi, sgn, bp, g,
+                                      (unsigned)c0, np1, P.thr, lane, binned, kept_n, evaluated);
             }
             binned_total += binned; kept_total += kept_n;
             __syncwarp();
@@ -690,36 +692,36 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 nnz += __popc(bal);
             }
             __syncwarp();
-            // ---- pass C ----
+            // ---- pass C (one drain call site: the kernel's code has to stay small for the instruction cache) ----
+            // Normally the queue holds every kept pair.  With more kept pairs than the queue holds (small
+            // reject fractions) the mask is redone row by row and the queue drained each time it fills.
             const unsigned nk = ws.nkept;
-            if (nk <= FD_KCAP) {
-                dm_drain<POW2>(ws, (int)nk, nnz, mp, mq, P, g, c0, hp.off, hq.off, lane, n_red);
-            } else {
-                // more kept pairs than the queue holds (small reject fractions): redo the mask row by row
-                int n_q = 0;
-                for (int i = 0; i < mp; ++i) {
-                    const double pci = ws.pc[i];
-                    const unsigned long long ki = ws.pk[i];
-                    for (int j0 = ws.jlo[i]; j0 < ws.jhi[i]; j0 += 32) {
-                        const int j = j0 + lane;
+            const bool overflow = nk > FD_KCAP;
+            int n_q = overflow ? 0 : (int)nk;
+            int si = 0, sj = (overflow && mp > 0) ? (int)ws.jlo[0] : 0;
+            for (;;) {
+                bool done = true;
+                if (overflow) {
+                    while (si < mp) {
+                        const int jh = ws.jhi[si];
+                        if (sj >= jh) { ++si; sj = (si < mp) ? (int)ws.jlo[si] : 0; continue; }
+                        const int j = sj + lane;
                         int A = -1;
-                        if (j < ws.jhi[i]) A = lya_pix_bin_t<POW2>(bp, g, pci, qc[j]);
-                        const bool kp = (A >= 0) && keep_pair(ki, ws.qk[min(j, FD_T - 1)], P.thr);
+                        if (j < jh) A = lya_pix_bin_t<POW2>(bp, g, ws.pc[si], qc[j]);
+                        const bool kp = (A >= 0) && keep_pair(ws.pk[si], ws.qk[min(j, FD_T - 1)], P.thr);
                         const unsigned bal = __ballot_sync(0xffffffffu, kp);
-                        if (bal) {
-                            if (n_q + __popc(bal) > FD_KCAP) {
-                                __syncwarp();
-                                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, hp.off, hq.off, lane, n_red);
-                                __syncwarp();
-                                n_q = 0;
-                            }
-                            if (kp) ws.kept[n_q + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)i << 20) | ((unsigned)j << 12) | (unsigned)A;
-                            n_q += __popc(bal);
-                        }
+                        if (n_q + __popc(bal) > FD_KCAP) break;          // drain first, then redo these 32 pixels
+                        if (kp) ws.kept[n_q + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)si << 20) | ((unsigned)j << 12) | (unsigned)A;
+                        n_q += __popc(bal);
+                        sj += 32;
                     }
+                    done = si >= mp;
                 }
                 __syncwarp();
                 dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, hp.off, hq.off, lane, n_red);
+                __syncwarp();
+                if (done) break;
+                n_q = 0;
             }
             __syncwarp();
             // clear the table and the queue for the next pair
