@@ -120,6 +120,14 @@ lya_status lya_pairs_export(lya_ctx *ctx, const lya_pairs *pairs, int32_t *pq);
 /* Builds a list from caller pairs (device int32 [n_pairs][2]); entries must be
  * distinct forests, either order; no criterion is applied (tests, sharding). */
 lya_status lya_pairs_import(lya_ctx *ctx, const int32_t *pq, int64_t n_pairs, lya_pairs **out);
+/* Forest-pair subsampling, the paper's own wording for the distortion matrix ("In practice D_AB is
+ * computed only with a small subset of forest pairs"; DESIGN.md NEXT-2): keeps the forest
+ * pair (p<q) iff keep(seed, p, q) of the stage-4 integer mask (with the FOREST indices
+ * in place of pixel offsets) is true for reject_fraction.  The order of the kept pairs is preserved.
+ * lya_dmat on the result with reject_fraction = 0 is the distortion matrix of that subset.
+ * *out is library-owned; n_kept: host out.  Synchronises the ctx stream. */
+lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, double reject_fraction, uint64_t seed,
+                               lya_pairs **out, int64_t *n_kept);
 int64_t    lya_pairs_count(const lya_pairs *pairs);
 void       lya_pairs_free(lya_ctx *ctx, lya_pairs *pairs);
 

@@ -183,3 +183,12 @@ def dmat(f, pairs, reject_fraction=0.0, seed=0, b=None, want_D=True, collapsed=F
         with np.errstate(divide="ignore", invalid="ignore"):
             out["D"] = np.where(Wd[:, None] != 0.0, Dn / np.where(Wd == 0, 1.0, Wd)[:, None], 0.0)
     return out
+
+
+def subsample_forest_pairs(pairs, reject_fraction: float, seed: int):
+    """The paper's forest-pair subsampling (DESIGN.md NEXT-2): keep (p, q) iff
+    keep(seed, p, q) of the stage-4 integer mask with the forest indices as ids.  Order preserved."""
+    pq = _pq(pairs)
+    thr = mask_threshold(reject_fraction)
+    sel = np.fromiter((keep(seed, int(p), int(q), thr) for p, q in pq), dtype=bool, count=len(pq))
+    return pq[sel]

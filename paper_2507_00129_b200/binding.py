@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblya.so")
 
 EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_neighbours",
-           "lya_pairs_export", "lya_pairs_import", "lya_pairs_count", "lya_pairs_free",
+           "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
            "lya_xi2pcf", "lya_dmat", "lya_run_host", "lya_measure_peak"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
@@ -72,6 +72,8 @@ def load():
         lib.lya_pairs_export.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.lya_pairs_import.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_void_p)]
         lib.lya_pairs_free.argtypes = [C.c_void_p, C.c_void_p]
+        lib.lya_pairs_subsample.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_uint64,
+                                            C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
         lib.lya_xi2pcf.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
         lib.lya_dmat.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
@@ -195,6 +197,13 @@ class Context:
         h = C.c_void_p()
         self._check(load().lya_pairs_import(self.h, _ptr(pq) if len(pq) else None, len(pq), C.byref(h)))
         return Pairs(self, h, len(pq))
+
+    def lya_pairs_subsample(self, pairs: Pairs, reject_fraction: float, seed: int) -> Pairs:
+        h = C.c_void_p()
+        n = C.c_int64()
+        self._check(load().lya_pairs_subsample(self.h, pairs.handle, float(reject_fraction), C.c_uint64(seed),
+                                               C.byref(h), C.byref(n)))
+        return Pairs(self, h, n.value)
 
     # ---- lya_xi2pcf ----
     def lya_xi2pcf(self, forests: DeviceForests, b: CBinning, pairs: Pairs):

@@ -762,6 +762,70 @@ __global__ void k_dmat_normalise(const double *Dn_t, const double *Wd_t, BinPara
 
 }  // namespace
 
+namespace {
+__global__ void k_fp_flag(const int32_t *pq, int64_t n, unsigned long long seed, unsigned long long thr, unsigned *flag)
+{
+    const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int2 e = ((const int2 *)pq)[k];
+    const unsigned long long lo = (unsigned long long)min(e.x, e.y), hi = (unsigned long long)max(e.x, e.y);
+    flag[k] = keep_pair(key_lo(seed, lo), key_hi(seed, hi), thr) ? 1u : 0u;
+}
+__global__ void k_fp_compact(const int32_t *pq, int64_t n, const unsigned *flag, const unsigned long long *pos, int32_t *out)
+{
+    const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (k >= n || !flag[k]) return;
+    ((int2 *)out)[pos[k]] = ((const int2 *)pq)[k];
+}
+}  // namespace
+
+extern "C" lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, double reject_fraction, uint64_t seed,
+                                          lya_pairs **out, int64_t *n_kept)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (!pairs || !out || !n_kept) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_pairs_subsample: NULL argument");
+    if (!(reject_fraction >= 0.0 && reject_fraction <= 1.0))
+        return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_pairs_subsample: reject_fraction must be in [0,1]");
+    *out = NULL; *n_kept = 0;
+    LYA_CUDA(cudaSetDevice(ctx->device));
+    lya_pairs *pl = (lya_pairs *)calloc(1, sizeof(lya_pairs));
+    if (!pl) return lya_fail(ctx, LYA_ERR_OOM, "host allocation failed");
+    const int64_t n = pairs->n;
+    if (n == 0) { *out = pl; return LYA_OK; }
+    double t = floor(reject_fraction * 4294967296.0 + 0.5);
+    if (t < 0) t = 0;
+    if (t > 4294967296.0) t = 4294967296.0;
+    const unsigned long long thr = (unsigned long long)t;
+    cudaStream_t s = ctx->stream;
+    unsigned *flag = NULL;
+    unsigned long long *pos = NULL, *tmp = NULL;
+    cudaError_t e = cudaMalloc(&flag, sizeof(unsigned) * (size_t)n);
+    if (e == cudaSuccess) e = cudaMalloc(&pos, sizeof(unsigned long long) * (size_t)(n + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&tmp, sizeof(unsigned long long) * (size_t)(n / 2048 + 4));
+    auto drop = [&]() { cudaFree(flag); cudaFree(pos); cudaFree(tmp); };
+    if (e != cudaSuccess) { drop(); free(pl); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_pairs_subsample)"); }
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    k_fp_flag<<<blocks, 256, 0, s>>>(pairs->pq, n, seed, thr, flag);
+    e = lya_exclusive_scan(flag, pos, n, tmp, s);
+    unsigned long long total = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&total, pos + n, sizeof(total), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { drop(); free(pl); return lya_cuda_fail(ctx, e, "lya_pairs_subsample"); }
+    pl->n = (int64_t)total;
+    if (total > 0) {
+        e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)total);
+        if (e == cudaSuccess) {
+            k_fp_compact<<<blocks, 256, 0, s>>>(pairs->pq, n, flag, pos, pl->pq);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        }
+        if (e != cudaSuccess) { if (pl->pq) cudaFree(pl->pq); drop(); free(pl); return lya_cuda_fail(ctx, e, "lya_pairs_subsample"); }
+    }
+    drop();
+    *out = pl; *n_kept = pl->n;
+    return LYA_OK;
+}
+
 extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
                                double reject_fraction, uint64_t seed, double *D, double *Dn_out, double *Wd_out,
                                lya_stats *stats)

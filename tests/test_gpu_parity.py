@@ -237,6 +237,20 @@ def test_kernel_routes_fast_and_generic(B, orc, monkeypatch):
     c.close()
 
 
+def test_forest_pair_subsampling_next2(ctx, B, orc):
+    """D from a subset of FOREST pairs = lya_pairs_subsample + lya_dmat(f = 0)."""
+    f = gen.make_config(1, n_forest=150, density_scale=4.0)
+    d = B.DeviceForests(f)
+    pairs = ctx.lya_neighbours(d, B.binning())
+    pq = pairs.export().cpu().numpy()
+    for frac, seed in ((0.9, 11), (0.5, 12)):
+        sub = ctx.lya_pairs_subsample(pairs, frac, seed)
+        want = orc.subsample_forest_pairs(pq, frac, seed)
+        assert sub.n == len(want) and np.array_equal(sub.export().cpu().numpy(), want)      # same set, same order
+        check_dmat(ctx.lya_dmat(d, B.binning(), sub, 0.0, 0), orc.dmat(f, want, 0.0, 0), f"forest-pair subset f={frac}")
+    assert ctx.lya_pairs_subsample(pairs, 1.0, 3).n == 0 and ctx.lya_pairs_subsample(pairs, 0.0, 3).n == pairs.n
+
+
 # ------------------------------------------------------------------ invariances and edge cases
 def test_P7_pair_order_and_swap(ctx, B, orc, cfg0):
     d = B.DeviceForests(cfg0)
@@ -330,7 +344,7 @@ def test_run_host_end_to_end(ctx, B, orc, cfg0):
 
 
 # ------------------------------------------------------------------ full-size configs, bench launch configuration
-@pytest.mark.parametrize("cfg", [2, 4])
+@pytest.mark.parametrize("cfg", [1, 2, 4])
 def test_full_size_properties_and_sampled_parity(ctx, B, orc, cfg):
     """At BASELINE.json's full sizes the oracle cannot run everything: check the neighbour list
     on sampled forests against a numpy brute force over ALL forests, the exact bookkeeping
@@ -362,6 +376,6 @@ def test_full_size_properties_and_sampled_parity(ctx, B, orc, cfg):
     sub = pq[sel].cpu().numpy()
     check_xi(ctx.lya_xi2pcf(d, b, ctx.lya_pairs_import(sub)), orc.xi(f, sub), f"cfg{cfg} sampled pairs")
     subd = sub[:1500]
-    seed = gen.mask_seed(3 if cfg == 2 else 4)
+    seed = gen.mask_seed(3 if cfg == 2 else cfg)
     check_dmat(ctx.lya_dmat(d, b, ctx.lya_pairs_import(subd), 0.99, seed), orc.dmat(f, subd, 0.99, seed),
                f"cfg{cfg} sampled pairs D")

@@ -381,3 +381,26 @@ def test_PD8_normalisation_sanity(cfg0, d0):
     db = orc.dmat(cfg0, pq[:400], 0.0, 0, b=big)
     assert np.abs(db["Dover"]).max() == 0.0
     assert np.all(np.abs(db["Dn"].sum(1)) <= 1e-11 * np.abs(db["Dn"]).sum(1) + 1e-300)
+
+
+# ---------------------------------------------------------------- NEXT-2: forest-pair subsampling
+def test_forest_pair_subsample_statistics_and_linearity(cfg0):
+    """The forest-pair subset is a deterministic ~(1-f) fraction of the list, keeps the order, and
+    D of a union of disjoint forest-pair subsets is the Wd-weighted combination of their Dn
+    (Dn and Wd are additive over forest pairs, eq. 2.6)."""
+    pq = orc.pairs_all(cfg0.n_forest)
+    sub = orc.subsample_forest_pairs(pq, 0.7, 77)
+    n = len(pq)
+    assert abs(len(sub) - 0.3 * n) < 4 * np.sqrt(0.21 * n)
+    assert np.array_equal(sub, orc.subsample_forest_pairs(pq, 0.7, 77))
+    idx = {(int(a), int(b)): k for k, (a, b) in enumerate(pq)}
+    pos = [idx[(int(a), int(b))] for a, b in sub]
+    assert pos == sorted(pos)
+    assert len(orc.subsample_forest_pairs(pq, 0.0, 5)) == n and len(orc.subsample_forest_pairs(pq, 1.0, 5)) == 0
+    keep_set = set(map(tuple, sub.tolist()))
+    rest = np.array([e for e in pq.tolist() if tuple(e) not in keep_set], dtype=np.int32)
+    some = sub[:60]; other = rest[:60]
+    d1, d2 = orc.dmat(cfg0, some, 0.0, 0), orc.dmat(cfg0, other, 0.0, 0)
+    d12 = orc.dmat(cfg0, np.concatenate([some, other]), 0.0, 0)
+    assert np.allclose(d12["Dn"], d1["Dn"] + d2["Dn"], rtol=0, atol=1e-9 * np.abs(d12["Dn"]).max())
+    assert np.allclose(d12["Wd"], d1["Wd"] + d2["Wd"], rtol=1e-12)
