@@ -101,10 +101,13 @@ struct DmWarpSmem {
 
 __device__ __forceinline__ void red_add(double *addr, double v) { atomicAdd(addr, v); }
 
-// Drain the kept-pair queue: T1..T3 (first column chunk only) and T4 (this chunk's columns).
+// Drain the kept-pair queue of one staged tile pair: T1..T3 (first column chunk only) and T4 (this
+// chunk's columns).  T2 / T3 run over the WHOLE forests q / p, read from global memory (forests can
+// be longer than a tile); op, oq = offsets of the forests, np, nq = their lengths.
 template <bool POW2>
-__device__ void drain_kept(DmWarpSmem &ws, int n_kept, int mp, int mq, const DmParams &P, const PairBin &g,
-                           double invSp, double invVp, double invSq, double invVq,
+__device__ void drain_kept(DmWarpSmem &ws, int n_kept, const DmParams &P, const PairBin &g,
+                           int64_t op, int np, double lbp, double invSp, double invVp,
+                           int64_t oq, int nq, double lbq, double invSq, double invVq,
                            int c0, int ncol, bool first_chunk, int lane)
 {
     const BinParams &bp = P.bp;
@@ -119,18 +122,18 @@ __device__ void drain_kept(DmWarpSmem &ws, int n_kept, int mp, int mq, const DmP
         double *row = P.Dn + (size_t)At * nb;
         if (first_chunk) {
             if (lane == 0) { red_add(row + At, om); red_add(P.Wd + At, om); }
-            for (int j2 = lane; j2 < mq; j2 += 32) {                       // T2
-                int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i], qc[j2]);
+            for (int j2 = lane; j2 < nq; j2 += 32) {                       // T2
+                int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i], P.chi[oq + j2]);
                 if (B >= 0) {
-                    double aj = qw[j2] * invSq, gj = qw[j2] * qu[j2] * invVq;
-                    red_add(row + B, -om * (aj + uj * gj));
+                    const double w2 = P.w[oq + j2], u2 = P.loglam[oq + j2] - lbq;
+                    red_add(row + B, -om * (w2 * invSq + uj * (w2 * u2 * invVq)));
                 }
             }
-            for (int i2 = lane; i2 < mp; i2 += 32) {                       // T3
-                int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i2], qc[j]);
+            for (int i2 = lane; i2 < np; i2 += 32) {                       // T3
+                int B = lya_pix_bin_t<POW2>(bp, g, P.chi[op + i2], qc[j]);
                 if (B >= 0) {
-                    double ai = ws.pw[i2] * invSp, gi = ws.pw[i2] * ws.pu[i2] * invVp;
-                    red_add(row + B, -om * (ai + ui * gi));
+                    const double w2 = P.w[op + i2], u2 = P.loglam[op + i2] - lbp;
+                    red_add(row + B, -om * (w2 * invSp + ui * (w2 * u2 * invVp)));
                 }
             }
         }
@@ -157,8 +160,8 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
     const int LC = P.LC;
     unsigned long long visited = 0, evaluated = 0, kept_total = 0, binned = 0;
     const int64_t n_chunks = (P.n_pairs + DCHUNK - 1) / DCHUNK;
-    int cur_p = -1;
-    double invSp = 0, invVp = 0;
+    int cur_p = -1, cur_ip0 = -1, scal_p = -1;
+    double invSp = 0, invVp = 0, lbp = 0;
     const double *qc = ws.qc + DQPAD, *qw = ws.qw + DQPAD, *qu = ws.qu + DQPAD;
 
     for (;;) {
@@ -174,125 +177,142 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
                 continue;
             }
             const int64_t op = P.pix_off[p], oq = P.pix_off[q];
-            const int mp = (int)(P.pix_off[p + 1] - op), mq = (int)(P.pix_off[q + 1] - oq);
-            if (mp == 0 || mq == 0) continue;
-            if (mp > DTILE || mq > DTILE) {
-                if (lane == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_TOO_LONG);
-                continue;
-            }
+            const int np = (int)(P.pix_off[p + 1] - op), nq = (int)(P.pix_off[q + 1] - oq);
+            if (np == 0 || nq == 0) continue;
             const double invSq = P.f_invS[q], invVq = P.f_invV[q], lbq = P.f_lbar[q];
-            __syncwarp();
-            if (p != cur_p) {
-                invSp = P.f_invS[p]; invVp = P.f_invV[p];
-                const double lbp = P.f_lbar[p];
-                for (int t = lane; t < mp; t += 32) {
-                    ws.pc[t] = P.chi[op + t];
-                    ws.pw[t] = P.w[op + t];
-                    ws.pu[t] = P.loglam[op + t] - lbp;
-                    ws.pk[t] = key_lo(P.seed, (unsigned long long)(op + t));
-                }
-                cur_p = p;
-            }
+            if (p != scal_p) { invSp = P.f_invS[p]; invVp = P.f_invV[p]; lbp = P.f_lbar[p]; scal_p = p; }
             if (isnan(invSp) || isnan(invVp) || isnan(invSq) || isnan(invVq)) {
                 if (lane == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_DEGENERATE);
                 continue;
             }
-            for (int t = lane; t < mq + 2 * DQPAD; t += 32) {
-                int j = t - DQPAD;
-                bool in = (j >= 0) && (j < mq);
-                ws.qc[t] = in ? P.chi[oq + j] : LYA_CHI_SENTINEL;
-                ws.qw[t] = in ? P.w[oq + j] : 0.0;
-                ws.qu[t] = in ? P.loglam[oq + j] - lbq : 0.0;
-                if (in) ws.qk[j] = key_hi(P.seed, (unsigned long long)(oq + j));
-            }
-            __syncwarp();
-            visited += (unsigned long long)mp * mq;
+            visited += (unsigned long long)np * nq;
             double s, c;
             lya_pair_sc(P.ux[p], P.uy[p], P.uz[p], P.ux[q], P.uy[q], P.uz[q], s, c);
             const PairBin g = lya_make_pairbin(bp, s, c);
-
             // r_perp column range of this forest pair: r_perp is increasing in both pixels
             int c_first, c_last;
             {
-                double t0 = __dmul_rn(__dadd_rn(ws.pc[0], qc[0]), g.s);
-                double t1 = __dmul_rn(__dadd_rn(ws.pc[mp - 1], qc[mq - 1]), g.s);
+                double t0 = __dmul_rn(__dadd_rn(P.chi[op], P.chi[oq]), g.s);
+                double t1 = __dmul_rn(__dadd_rn(P.chi[op + np - 1], P.chi[oq + nq - 1]), g.s);
                 if (!(t0 < bp.rperp_max)) continue;                        // nothing in the grid
                 c_first = min((int)lya_floor_u32(__dmul_rn(t0, bp.inv_perp)), bp.n_perp - 1);
                 c_last = (t1 < bp.rperp_max) ? min((int)lya_floor_u32(__dmul_rn(t1, bp.inv_perp)), bp.n_perp - 1)
                                              : bp.n_perp - 1;
             }
+            // stage one DTILE-pixel tile of p / q (forests of any length are walked tile by tile)
+            auto stage_p = [&](int ip0, int mp) {
+                if (p == cur_p && ip0 == cur_ip0) return;
+                __syncwarp();
+                for (int t = lane; t < mp; t += 32) {
+                    ws.pc[t] = P.chi[op + ip0 + t];
+                    ws.pw[t] = P.w[op + ip0 + t];
+                    ws.pu[t] = P.loglam[op + ip0 + t] - lbp;
+                    ws.pk[t] = key_lo(P.seed, (unsigned long long)(op + ip0 + t));
+                }
+                cur_p = p; cur_ip0 = ip0;
+                __syncwarp();
+            };
+            auto stage_q = [&](int jq0, int mq) {
+                __syncwarp();
+                for (int t = lane; t < mq + 2 * DQPAD; t += 32) {
+                    int j = t - DQPAD;
+                    bool in = (j >= 0) && (j < mq);
+                    ws.qc[t] = in ? P.chi[oq + jq0 + j] : LYA_CHI_SENTINEL;
+                    ws.qw[t] = in ? P.w[oq + jq0 + j] : 0.0;
+                    ws.qu[t] = in ? P.loglam[oq + jq0 + j] - lbq : 0.0;
+                    if (in) ws.qk[j] = key_hi(P.seed, (unsigned long long)(oq + jq0 + j));
+                }
+                __syncwarp();
+            };
             for (int c0 = c_first; c0 <= c_last; c0 += LC) {
                 const int ncol = min(LC, c_last - c0 + 1);
                 const bool first_chunk = (c0 == c_first);
                 const int n_slots = bp.n_par * ncol;
+                __syncwarp();
                 for (int t = lane; t < n_slots; t += 32) { ws.H[0][t] = 0.0; ws.H[1][t] = 0.0; ws.H[2][t] = 0.0; ws.H[3][t] = 0.0; }
                 __syncwarp();
-                // ---- pass 1a: H tables; lanes own diagonals d = j - i, register run-length ----
-                for (int d0 = -(mp - 1); d0 <= mq - 1; d0 += 32) {
-                    const int d = d0 + lane;
-                    const int i_begin = max(0, -min(mq - 1, d0 + 31));
-                    const int i_end = min(mp, mq - d0);
-                    int cur = -1;
-                    double h0 = 0, h1 = 0, h2 = 0, h3 = 0;
-                    evaluated += (unsigned long long)(i_end - i_begin);
-                    for (int i = i_begin; i < i_end; ++i) {
-                        int j = min(max(i + d, -DQPAD), mq + DQPAD - 1);
-                        int bin = lya_pix_bin<POW2>(bp, g, ws.pc[i], qc[j]);
-                        int slot = -1;
-                        if (bin >= 0) {
-                            int bx = bin / bp.n_perp, by = bin - bx * bp.n_perp;
-                            if (by >= c0 && by < c0 + ncol) slot = bx * ncol + (by - c0);
-                        }
-                        if (slot != cur) {
+                // ---- pass 1a: H tables over every tile pair; lanes own diagonals d = j - i, register run-length ----
+                for (int ip0 = 0; ip0 < np; ip0 += DTILE) {
+                    const int mp = min(DTILE, np - ip0);
+                    stage_p(ip0, mp);
+                    for (int jq0 = 0; jq0 < nq; jq0 += DTILE) {
+                        const int mq = min(DTILE, nq - jq0);
+                        stage_q(jq0, mq);
+                        for (int d0 = -(mp - 1); d0 <= mq - 1; d0 += 32) {
+                            const int d = d0 + lane;
+                            const int i_begin = max(0, -min(mq - 1, d0 + 31));
+                            const int i_end = min(mp, mq - d0);
+                            int cur = -1;
+                            double h0 = 0, h1 = 0, h2 = 0, h3 = 0;
+                            evaluated += (unsigned long long)(i_end - i_begin);
+                            for (int i = i_begin; i < i_end; ++i) {
+                                int j = min(max(i + d, -DQPAD), mq + DQPAD - 1);
+                                int bin = lya_pix_bin<POW2>(bp, g, ws.pc[i], qc[j]);
+                                int slot = -1;
+                                if (bin >= 0) {
+                                    int bx = bin / bp.n_perp, by = bin - bx * bp.n_perp;
+                                    if (by >= c0 && by < c0 + ncol) slot = bx * ncol + (by - c0);
+                                }
+                                if (slot != cur) {
+                                    if (cur >= 0) {
+                                        atomicAdd(&ws.H[0][cur], h0); atomicAdd(&ws.H[1][cur], h1);
+                                        atomicAdd(&ws.H[2][cur], h2); atomicAdd(&ws.H[3][cur], h3);
+                                    }
+                                    cur = slot; h0 = h1 = h2 = h3 = 0.0;
+                                }
+                                if (slot >= 0) {
+                                    double ai = ws.pw[i] * invSp, gi = ws.pw[i] * ws.pu[i] * invVp;
+                                    double aj = qw[j] * invSq, gj = qw[j] * qu[j] * invVq;
+                                    h0 = fma(ai, aj, h0); h1 = fma(ai, gj, h1);
+                                    h2 = fma(gi, aj, h2); h3 = fma(gi, gj, h3);
+                                }
+                            }
                             if (cur >= 0) {
                                 atomicAdd(&ws.H[0][cur], h0); atomicAdd(&ws.H[1][cur], h1);
                                 atomicAdd(&ws.H[2][cur], h2); atomicAdd(&ws.H[3][cur], h3);
                             }
-                            cur = slot; h0 = h1 = h2 = h3 = 0.0;
                         }
-                        if (slot >= 0) {
-                            double ai = ws.pw[i] * invSp, gi = ws.pw[i] * ws.pu[i] * invVp;
-                            double aj = qw[j] * invSq, gj = qw[j] * qu[j] * invVq;
-                            h0 = fma(ai, aj, h0); h1 = fma(ai, gj, h1);
-                            h2 = fma(gi, aj, h2); h3 = fma(gi, gj, h3);
-                        }
-                    }
-                    if (cur >= 0) {
-                        atomicAdd(&ws.H[0][cur], h0); atomicAdd(&ws.H[1][cur], h1);
-                        atomicAdd(&ws.H[2][cur], h2); atomicAdd(&ws.H[3][cur], h3);
                     }
                 }
                 __syncwarp();
-                // ---- pass 1b: mask every in-grid pair, queue the kept ones, drain ----
-                int n_q = 0;
-                for (int i = 0; i < mp; ++i) {
-                    const double pci = ws.pc[i];
-                    const unsigned long long ki = ws.pk[i];
-                    for (int j0 = 0; j0 < mq; j0 += 32) {
-                        const int j = j0 + lane;
-                        int bin = -1;
-                        if (j < mq) bin = lya_pix_bin<POW2>(bp, g, pci, qc[j]);
-                        bool kp = (bin >= 0) && keep_pair(ki, ws.qk[min(j, mq - 1)], P.thr);
-                        if (first_chunk) {
-                            binned += (bin >= 0);
-                            kept_total += kp;
-                        }
-                        unsigned bal = __ballot_sync(0xffffffffu, kp);
-                        if (bal) {
-                            if (n_q + __popc(bal) > KEPT_CAP) {
-                                __syncwarp();
-                                drain_kept<POW2>(ws, n_q, mp, mq, P, g, invSp, invVp, invSq, invVq, c0, ncol, first_chunk, lane);
-                                __syncwarp();
-                                n_q = 0;
+                // ---- pass 1b: mask every in-grid pair of every tile pair, queue the kept ones, drain ----
+                for (int ip0 = 0; ip0 < np; ip0 += DTILE) {
+                    const int mp = min(DTILE, np - ip0);
+                    stage_p(ip0, mp);
+                    for (int jq0 = 0; jq0 < nq; jq0 += DTILE) {
+                        const int mq = min(DTILE, nq - jq0);
+                        stage_q(jq0, mq);
+                        int n_q = 0;
+                        for (int i = 0; i < mp; ++i) {
+                            const double pci = ws.pc[i];
+                            const unsigned long long ki = ws.pk[i];
+                            for (int j0 = 0; j0 < mq; j0 += 32) {
+                                const int j = j0 + lane;
+                                int bin = -1;
+                                if (j < mq) bin = lya_pix_bin<POW2>(bp, g, pci, qc[j]);
+                                bool kp = (bin >= 0) && keep_pair(ki, ws.qk[min(j, mq - 1)], P.thr);
+                                if (first_chunk) {
+                                    binned += (bin >= 0);
+                                    kept_total += kp;
+                                }
+                                unsigned bal = __ballot_sync(0xffffffffu, kp);
+                                if (bal) {
+                                    if (n_q + __popc(bal) > KEPT_CAP) {
+                                        __syncwarp();
+                                        drain_kept<POW2>(ws, n_q, P, g, op, np, lbp, invSp, invVp, oq, nq, lbq, invSq, invVq, c0, ncol, first_chunk, lane);
+                                        __syncwarp();
+                                        n_q = 0;
+                                    }
+                                    if (kp) ws.kept[n_q + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)i << 20) | ((unsigned)j << 12) | (unsigned)bin;
+                                    n_q += __popc(bal);
+                                }
                             }
-                            if (kp) ws.kept[n_q + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)i << 20) | ((unsigned)j << 12) | (unsigned)bin;
-                            n_q += __popc(bal);
                         }
+                        __syncwarp();
+                        drain_kept<POW2>(ws, n_q, P, g, op, np, lbp, invSp, invVp, oq, nq, lbq, invSq, invVq, c0, ncol, first_chunk, lane);
+                        __syncwarp();
                     }
                 }
-                __syncwarp();
-                drain_kept<POW2>(ws, n_q, mp, mq, P, g, invSp, invVp, invSq, invVq, c0, ncol, first_chunk, lane);
-                __syncwarp();
             }
         }
     }
@@ -853,8 +873,6 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     const BinParams bp = lya_make_binparams(b);
     const bool use_fast = pairs->n > 0 && (b->n_par + 1) * LYA_NCOL <= FD_SLOTS && b->n_perp + 2 <= 256 &&
                           ctx->dmat_variant != 9;
-    if (!use_fast && max_len > DTILE)
-        return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: forests longer than %d pixels are not supported with this binning", DTILE);
     double *scal = NULL, *Dn = NULL, *Wd = NULL;          // internal accumulators (transposed bin order)
     bool own_Dn = false, own_Wd = false;
     const int64_t nf = f->n_forest;

@@ -199,6 +199,12 @@ def test_long_and_ragged_forests_tiles(ctx, B, orc):
     ref = orc.pairs_brute(f)
     assert pair_set(pairs.export().cpu().numpy()) == pair_set(ref)
     check_xi(ctx.lya_xi2pcf(d, B.binning(), pairs), orc.xi(f, ref), "long forests")
+    # the distortion matrix of forests longer than a tile (native-resolution shapes take the generic kernel)
+    keep = [k for k, n in enumerate(lens) if n >= 2]
+    f2 = f.subset(keep)
+    ref2 = orc.pairs_brute(f2)
+    g = ctx.lya_dmat(B.DeviceForests(f2), B.binning(), ctx.lya_pairs_import(ref2), 0.97, 9)
+    check_dmat(g, orc.dmat(f2, ref2, 0.97, 9), "long forests D")
 
 
 def test_kernel_routes_fast_and_generic(B, orc, monkeypatch):
