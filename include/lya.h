@@ -140,6 +140,16 @@ lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                       const lya_pairs *pairs,
                       double *S, double *W, uint64_t *N, double *xi, lya_stats *stats);
 
+/* NEXT-1: per-sky-region sub-samples of eq. 2.4, the input of the covariance
+ * estimate ("covariance ... from sub-sampling").  region: device int32
+ * [n_forest] with values in [0, n_region); a pixel pair belongs to the sub-sample of the LOWER-index
+ * forest p of its forest pair.  S, W: double [n_region][n_par*n_perp]; N: uint64 [n_region][...]; any
+ * may be NULL.  Summed over the regions they equal lya_xi2pcf's S, W, N (N exactly).
+ * LYA_ERR_INVALID_ARG for a region outside the range; LYA_ERR_CAPACITY if n_region * bins > 2^28. */
+lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
+                          const lya_pairs *pairs, const int32_t *region, int32_t n_region,
+                          double *S, double *W, uint64_t *N, lya_stats *stats);
+
 /* ---- stages 3+4: distortion matrix, eqs. 2.6-2.7 ----------------- */
 /* eta_ii' = delta^K_ii' - w_i'/sum_k w_k - (L_i-Lbar) w_i' (L_i'-Lbar) / sum_k w_k (L_k-Lbar)^2
  * inside a forest (0 across forests), L = loglam, Lbar the w-weighted mean (R-10).

@@ -192,3 +192,13 @@ def subsample_forest_pairs(pairs, reject_fraction: float, seed: int):
     thr = mask_threshold(reject_fraction)
     sel = np.fromiter((keep(seed, int(p), int(q), thr) for p, q in pq), dtype=bool, count=len(pq))
     return pq[sel]
+
+
+def xi_sub(f, pairs, region, n_region, b=None):
+    """Per-sky-region sub-samples of eq. 2.4 (DESIGN.md NEXT-1): sub-sample r is
+    eq. 2.4 over the forest pairs whose lower-index forest p lies in region r."""
+    cat = f if isinstance(f, Catalogue) else Catalogue(f)
+    pq = _pq(pairs)
+    region = np.asarray(region)
+    lo = np.minimum(pq[:, 0], pq[:, 1])
+    return [xi(cat, pq[region[lo] == r], b) for r in range(n_region)]

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "liblya.so")
 
 EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_neighbours",
            "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
-           "lya_xi2pcf", "lya_dmat", "lya_run_host", "lya_measure_peak"]
+           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host", "lya_measure_peak"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
           4: "LYA_ERR_CAPACITY", 5: "LYA_ERR_OOM", 6: "LYA_ERR_CUDA", 7: "LYA_ERR_UNIMPLEMENTED"}
@@ -76,6 +76,8 @@ def load():
                                             C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
         lib.lya_xi2pcf.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
+        lib.lya_xi2pcf_sub.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
+                                       C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
         lib.lya_dmat.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
                                  C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
         lib.lya_run_host.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_int, C.c_int,
@@ -217,6 +219,22 @@ class Context:
         self._check(load().lya_xi2pcf(self.h, C.byref(cf), C.byref(b), pairs.handle,
                                       _ptr(S), _ptr(W), _ptr(N), _ptr(xi), C.byref(stats)))
         return dict(S=S, W=W, N=N, xi=xi, stats=stats.as_dict())
+
+    def lya_xi2pcf_sub(self, forests: DeviceForests, b: CBinning, pairs: Pairs, region, n_region: int):
+        """region: int32 [n_forest] (numpy or torch).  Returns S, W [n_region][nb], N [n_region][nb]."""
+        torch = self.torch
+        if not torch.is_tensor(region):
+            region = torch.from_numpy(np.ascontiguousarray(region, dtype=np.int32))
+        region = region.to(self.device, dtype=torch.int32).contiguous()
+        nb = b.n_par * b.n_perp
+        S = torch.empty((n_region, nb), dtype=torch.float64, device=self.device)
+        W = torch.empty_like(S)
+        N = torch.empty((n_region, nb), dtype=torch.int64, device=self.device)      # uint64 payload
+        stats = CStats()
+        cf = forests.c()
+        self._check(load().lya_xi2pcf_sub(self.h, C.byref(cf), C.byref(b), pairs.handle, _ptr(region), int(n_region),
+                                          _ptr(S), _ptr(W), _ptr(N), C.byref(stats)))
+        return dict(S=S, W=W, N=N, stats=stats.as_dict())
 
     # ---- lya_dmat ----
     def lya_dmat(self, forests: DeviceForests, b: CBinning, pairs: Pairs, reject_fraction: float, seed: int,

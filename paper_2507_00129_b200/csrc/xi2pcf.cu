@@ -236,6 +236,45 @@ __global__ void __launch_bounds__(XI_THREADS, 2) k_xi(XiParams P)
     }
 }
 
+// Sub-sample mode (NEXT-1), pairs the fast kernel cannot take: one warp per forest pair, lanes over
+// the pixel pairs, global atomics into the accumulators of the pair's sub-sample.  Slow and simple.
+template <bool POW2>
+__global__ void k_xi_direct(XiParams P, const int32_t *region)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int64_t n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    const BinParams bp = P.bp;
+    const int nb = bp.n_par * bp.n_perp;
+    unsigned long long visited = 0;
+    for (int64_t k = warp; k < P.n_pairs; k += n_warps) {
+        const int p = P.pq[2 * k], q = P.pq[2 * k + 1];
+        if ((unsigned)p >= (unsigned)P.n_forest || (unsigned)q >= (unsigned)P.n_forest) {
+            if (lane == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_BAD_PAIR);
+            continue;
+        }
+        const int64_t op = P.pix_off[p], oq = P.pix_off[q];
+        const int64_t np = P.pix_off[p + 1] - op, nq = P.pix_off[q + 1] - oq;
+        if (np == 0 || nq == 0) continue;
+        visited += (unsigned long long)(np * nq);
+        double s, c;
+        lya_pair_sc(P.ux[p], P.uy[p], P.uz[p], P.ux[q], P.uy[q], P.uz[q], s, c);
+        const PairBin g = lya_make_pairbin(bp, s, c);
+        const size_t roff = (size_t)(region ? region[p] : 0) * nb;
+        for (int64_t t = lane; t < np * nq; t += 32) {
+            const int64_t i = t / nq, j = t - i * nq;
+            const int A = lya_pix_bin<POW2>(bp, g, P.chi[op + i], P.chi[oq + j]);
+            if (A >= 0) {
+                const double wi = P.w[op + i], wj = P.w[oq + j];
+                atomicAdd(&P.S[roff + A], (wi * P.delta[op + i]) * (wj * P.delta[oq + j]));
+                atomicAdd(&P.W[roff + A], wi * wj);
+                atomicAdd(&P.N[roff + A], 1ull);
+            }
+        }
+    }
+    if (lane == 0 && visited) { atomicAdd(&P.counters[1], visited); atomicAdd(&P.counters[2], visited); }
+}
+
 __global__ void k_xi_finalize(const double *S, const double *W, const unsigned long long *N, int nb,
                               double *S_out, double *W_out, unsigned long long *N_out, double *xi_out)
 {
@@ -282,6 +321,8 @@ struct XiFastParams {
     double *S, *W;
     unsigned long long *N;
     unsigned long long *counters;            // [4] next chunk, [2] evaluated
+    const int32_t *region;                   // NULL, or the sub-sample (sky region) of every forest (NEXT-1)
+    int n_region;
 };
 
 // Sub-histogram slot = col_rel * 2 (n_par + 1) + side * (n_par + 1) + row.
@@ -440,8 +481,9 @@ __device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsi
 }
 
 // merge a warp's sub-histogram (first column c0) into the global accumulators and clear it
-__device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, int c0, int lane)
+__device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, int c0, int reg, int lane)
 {
+    const size_t roff = (size_t)reg * (size_t)(P.bp.n_par * P.bp.n_perp);   // accumulators of sub-sample reg
     const int np1 = P.bp.n_par + 1;
     __syncwarp();
     for (int t = lane; t < np1 * LYA_NCOL; t += 32) {            // t = col_rel * np1 + row
@@ -452,9 +494,9 @@ __device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, in
             if (bx < P.bp.n_par && cr < LYA_NCOL && col < P.bp.n_perp) {
                 const double2 v0 = ws.SW[s0], v1 = ws.SW[s1];
                 const int A = bx * P.bp.n_perp + col;
-                atomicAdd(&P.N[A], (unsigned long long)n);
-                atomicAdd(&P.S[A], v0.x + v1.x);
-                atomicAdd(&P.W[A], v0.y + v1.y);
+                atomicAdd(&P.N[roff + A], (unsigned long long)n);
+                atomicAdd(&P.S[roff + A], v0.x + v1.x);
+                atomicAdd(&P.W[roff + A], v0.y + v1.y);
             }
             ws.N[s0] = 0u; ws.N[s1] = 0u;
         }
@@ -478,7 +520,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
     const double *qc = ws.qc + FPAD;
     const unsigned sw_base = (unsigned)__cvta_generic_to_shared(ws.SW), n_base = (unsigned)__cvta_generic_to_shared(ws.N);
     unsigned long long evaluated = 0, since_merge = 0;
-    int cur_p = -1, head_p = -1, win_c0 = -1;
+    int cur_p = -1, head_p = -1, win_c0 = -1, win_reg = 0;
     ForestHead hp;
     hp.len = 0;
     const int64_t n_chunks = (P.n_pairs + FCHUNK - 1) / FCHUNK;
@@ -501,9 +543,10 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
             const int key = lya_pair_key<POW2>(bp, g, hp, hq, c0);
             if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
             since_merge += (unsigned long long)mp * mq;
-            if (c0 != win_c0 || since_merge > (1ull << 31)) {
-                if (win_c0 >= 0) xi_merge(ws, P, win_c0, lane);
-                win_c0 = c0; since_merge = (unsigned long long)mp * mq;
+            const int reg = P.region ? P.region[p] : 0;       // a pixel pair belongs to the sub-sample of forest p
+            if (c0 != win_c0 || reg != win_reg || since_merge > (1ull << 31)) {
+                if (win_c0 >= 0) xi_merge(ws, P, win_c0, win_reg, lane);
+                win_c0 = c0; win_reg = reg; since_merge = (unsigned long long)mp * mq;
             }
             __syncwarp();
             if (p != cur_p) {
@@ -560,7 +603,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
             }
         }
     }
-    if (win_c0 >= 0) xi_merge(ws, P, win_c0, lane);
+    if (win_c0 >= 0) xi_merge(ws, P, win_c0, win_reg, lane);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
     if (lane == 0 && evaluated) atomicAdd(&P.counters[2], evaluated);
@@ -568,8 +611,18 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
 
 }  // namespace
 
-extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
-                                 double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
+namespace {
+__global__ void k_check_region(const int32_t *region, int64_t n, int n_region, unsigned long long *flag)
+{
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p < n && (unsigned)region[p] >= (unsigned)n_region) atomicMax(flag, 1ull);
+}
+}  // namespace
+
+// region == NULL: eq. 2.4 over the whole list.  Otherwise (NEXT-1) one set of accumulators per sub-sample.
+static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                         const int32_t *region, int n_region,
+                         double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
 {
     if (!ctx) return LYA_ERR_INVALID_ARG;
     if (!pairs) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf: pairs is NULL");
@@ -584,8 +637,21 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
     if (st) return st;
 
     const int nb = b->n_par * b->n_perp;
+    const int n_reg = region ? n_region : 1;
+    const size_t nbt = (size_t)nb * n_reg;                     // accumulator entries
     cudaStream_t s = ctx->stream;
     const BinParams bp = lya_make_binparams(b);
+    if (region) {
+        if (n_region < 1 || (int64_t)n_region * nb > ((int64_t)1 << 28))
+            return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_xi2pcf_sub: need 1 <= n_region and n_region * bins <= 2^28");
+        cudaMemsetAsync(ctx->d_counters + 12, 0, sizeof(unsigned long long), s);
+        if (f->n_forest > 0)
+            k_check_region<<<(unsigned)((f->n_forest + 255) / 256), 256, 0, s>>>(region, f->n_forest, n_region, ctx->d_counters + 12);
+        unsigned long long bad = 0;
+        LYA_CUDA(cudaMemcpyAsync(&bad, ctx->d_counters + 12, sizeof(bad), cudaMemcpyDeviceToHost, s));
+        LYA_CUDA(cudaStreamSynchronize(s));
+        if (bad) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_sub: region[] must lie in [0, n_region)");
+    }
     // fast path: bucketed list + warp-private sub-histograms (variant 9 forces the generic kernel)
     const bool use_fast = pairs->n > 0 && 2 * (b->n_par + 1) * LYA_NCOL <= FSLOTS && b->n_perp + 2 <= 256 && ctx->xi_variant != 9;
     LyaPrep prep;
@@ -603,9 +669,9 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
         if (st) { cleanup(); return st; }
         if (bk.bad_pair) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
     }
-    cudaError_t e = cudaMalloc(&acc, (size_t)nb * 24);
+    cudaError_t e = cudaMalloc(&acc, nbt * 24);
     if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(xi accumulators)"); }
-    cudaMemsetAsync(acc, 0, (size_t)nb * 24, s);
+    cudaMemsetAsync(acc, 0, nbt * 24, s);
     cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
 
     XiParams P;
@@ -615,7 +681,7 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
     P.n_pairs = use_fast ? bk.n_generic : pairs->n;
     P.n_forest = f->n_forest;
     P.bp = bp;
-    P.S = acc; P.W = acc + nb; P.N = (unsigned long long *)(acc + 2 * nb);
+    P.S = acc; P.W = acc + nbt; P.N = (unsigned long long *)(acc + 2 * nbt);
     P.counters = ctx->d_counters;
 
     cudaEventRecord(ctx->ev[0], s);
@@ -623,6 +689,7 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
         XiFastParams F;
         F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
         F.S = P.S; F.W = P.W; F.N = P.N; F.counters = ctx->d_counters;
+        F.region = region; F.n_region = n_reg;
         const size_t fsmem = sizeof(FastWarp) * FW;
         const int fgrid = ctx->sm_count;
         if (bp.pow2) {
@@ -640,7 +707,14 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
     const int64_t n_chunks = (P.n_pairs + CHUNK - 1) / CHUNK;
     int launches = 0;
     unsigned long long h[4] = {0, 0, 0, 0};
-    while (P.n_pairs > 0) {
+    if (region && P.n_pairs > 0) {                 // sub-sample mode: the block-level histogram of k_xi cannot be used
+        const int dgrid = (int)((P.n_pairs + 7) / 8 < (int64_t)ctx->sm_count * 8 ? (P.n_pairs + 7) / 8 : (int64_t)ctx->sm_count * 8);
+        if (bp.pow2) k_xi_direct<true><<<dgrid, 256, 0, s>>>(P, region);
+        else k_xi_direct<false><<<dgrid, 256, 0, s>>>(P, region);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_direct launch"); }
+    }
+    while (!region && P.n_pairs > 0) {
         switch (ctx->xi_variant) {
         case 1: e = launch_xi<1>(P, grid, smem, s); break;
         case 4: e = launch_xi<4>(P, grid, smem, s); break;
@@ -655,7 +729,7 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
         if (launches > 100000) { cleanup(); return lya_fail(ctx, LYA_ERR_CUDA, "k_xi made no progress"); }
     }
     cudaEventRecord(ctx->ev[1], s);
-    k_xi_finalize<<<(nb + 255) / 256, 256, 0, s>>>(P.S, P.W, P.N, nb, S, W, (unsigned long long *)N, xi);
+    k_xi_finalize<<<(unsigned)((nbt + 255) / 256), 256, 0, s>>>(P.S, P.W, P.N, (int)nbt, S, W, (unsigned long long *)N, xi);
     cudaEventRecord(ctx->ev[2], s);
     e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
@@ -667,13 +741,28 @@ extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_b
         stats->n_visited = use_fast ? bk.visited : h[1];
         stats->n_evaluated = h[2];
         // n_binned = sum N: small D2H
-        unsigned long long *hN = (unsigned long long *)malloc(sizeof(unsigned long long) * nb);
-        if (hN && cudaMemcpy(hN, P.N, sizeof(unsigned long long) * nb, cudaMemcpyDeviceToHost) == cudaSuccess)
-            for (int k = 0; k < nb; ++k) stats->n_binned += hN[k];
+        unsigned long long *hN = (unsigned long long *)malloc(sizeof(unsigned long long) * nbt);
+        if (hN && cudaMemcpy(hN, P.N, sizeof(unsigned long long) * nbt, cudaMemcpyDeviceToHost) == cudaSuccess)
+            for (size_t k = 0; k < nbt; ++k) stats->n_binned += hN[k];
         free(hN);
         cudaEventElapsedTime(&stats->ms_main, ctx->ev[0], ctx->ev[1]);
         cudaEventElapsedTime(&stats->ms_total, ctx->ev[3], ctx->ev[2]);
     }
     cleanup();
     return LYA_OK;
+}
+
+extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                                 double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
+{
+    return xi_run(ctx, f, b, pairs, NULL, 1, S, W, N, xi, stats);
+}
+
+extern "C" lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                                     const int32_t *region, int32_t n_region,
+                                     double *S, double *W, uint64_t *N, lya_stats *stats)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (!region) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_sub: region is NULL");
+    return xi_run(ctx, f, b, pairs, region, n_region, S, W, N, NULL, stats);
 }

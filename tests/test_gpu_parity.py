@@ -257,6 +257,33 @@ def test_forest_pair_subsampling_next2(ctx, B, orc):
     assert ctx.lya_pairs_subsample(pairs, 1.0, 3).n == 0 and ctx.lya_pairs_subsample(pairs, 0.0, 3).n == pairs.n
 
 
+def test_region_subsamples_next1(ctx, B, orc):
+    """lya_xi2pcf_sub against the oracle region by region: fast kernel (bucketed list) and, with a grid
+    whose bins exceed the pixel spacing, the direct kernel; the regions add up to lya_xi2pcf."""
+    f = gen.make_config(1, n_forest=600)
+    d = B.DeviceForests(f)
+    rng = np.random.default_rng(5)
+    n_region = 5
+    region = rng.integers(0, n_region - 1, f.n_forest).astype(np.int32)          # region 4 stays empty
+    for grid in ((200.0, 200.0, 50, 50), (200.0, 200.0, 25, 25)):
+        b, ob = B.binning(*grid), orc.binning(*grid)
+        pairs = ctx.lya_neighbours(d, b)
+        pq = pairs.export().cpu().numpy()
+        g = ctx.lya_xi2pcf_sub(d, b, pairs, region, n_region)
+        full = ctx.lya_xi2pcf(d, b, pairs)
+        want = orc.xi_sub(f, pq, region, n_region, ob)
+        N = g["N"].cpu().numpy().view(np.uint64); S = g["S"].cpu().numpy(); W = g["W"].cpu().numpy()
+        for r in range(n_region):
+            o = want[r]
+            assert np.array_equal(N[r], o["N"]), f"region {r}"
+            assert np.all(np.abs(W[r] - o["W"]) <= 1e-9 * o["W"])
+            assert np.all(np.abs(S[r] - o["S"]) <= 1e-9 * np.maximum(np.abs(o["S"]), 1e-4 * o["Sabs"]))
+        assert np.array_equal(N.sum(0), full["N"].cpu().numpy().view(np.uint64)) and N[4].sum() == 0
+        assert g["stats"]["n_binned"] == full["stats"]["n_binned"]
+    with pytest.raises(B.LyaError):
+        ctx.lya_xi2pcf_sub(d, B.binning(), pairs, region + 3, n_region)
+
+
 # ------------------------------------------------------------------ invariances and edge cases
 def test_P7_pair_order_and_swap(ctx, B, orc, cfg0):
     d = B.DeviceForests(cfg0)

@@ -404,3 +404,21 @@ def test_forest_pair_subsample_statistics_and_linearity(cfg0):
     d12 = orc.dmat(cfg0, np.concatenate([some, other]), 0.0, 0)
     assert np.allclose(d12["Dn"], d1["Dn"] + d2["Dn"], rtol=0, atol=1e-9 * np.abs(d12["Dn"]).max())
     assert np.allclose(d12["Wd"], d1["Wd"] + d2["Wd"], rtol=1e-12)
+
+
+# ---------------------------------------------------------------- NEXT-1: per-region sub-samples
+def test_region_subsamples_partition_the_full_result(cfg0, xi0):
+    """Sub-samples partition the forest pairs by the region of the lower-index forest: their N add up
+    to the full N exactly and S, W to rounding; a region without forests is empty."""
+    pq, full = xi0
+    region = (np.arange(cfg0.n_forest) * 7) % 3                       # regions 0, 1, 2 in use; 3 is empty
+    subs = orc.xi_sub(cfg0, pq, region, 4)
+    assert np.array_equal(sum(s["N"] for s in subs), full["N"])
+    assert np.allclose(sum(s["W"] for s in subs), full["W"], rtol=1e-12)
+    assert np.all(np.abs(sum(s["S"] for s in subs) - full["S"]) <= 1e-12 * full["Sabs"])
+    assert subs[3]["N"].sum() == 0
+    # forest 0 has the lowest index of all its pairs: moving it to its own region moves exactly its pairs
+    region2 = region.copy(); region2[0] = 3
+    subs2 = orc.xi_sub(cfg0, pq, region2, 4)
+    only0 = orc.xi(cfg0, pq[pq[:, 0] == 0])
+    assert np.array_equal(subs2[3]["N"], only0["N"])
