@@ -319,7 +319,10 @@ def main():
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "description": wl["desc"], "n_forest": f.n_forest, "n_pix": f.n_pix,
                        "bins": "50x50x4Mpc/h", "reject_fraction": frac, "dmat": do_d,
-                       "l2": "inputs (%.2f GB) larger than L2; Dn (50 MB) re-zeroed every step" % (f.n_pix * 32 / 1e9),
+                       "l2": ("catalogue %.2f GB + forest-pair list %.2f GB per step vs 126 MB of L2 (%s); Dn (50 MB) "
+                              "re-zeroed every step") % (f.n_pix * 32 / 1e9, sx["n_forest_pairs"] * 8 / 1e9,
+                                                         "larger than L2" if f.n_pix * 32 + sx["n_forest_pairs"] * 8 > 126e6
+                                                         else "NOT larger than L2: use the default workload for a valid number"),
                        "parallelism": f"independent catalogue per GPU x{world}"},
             "roofline": roof, "clocks": clocks, "gpu_launches": launches, "e2e": e2e, **extra,
         }
