@@ -3,7 +3,7 @@
 //  (1) lya_prep_build: a padded, 16-byte aligned SoA copy of the catalogue (so a warp can
 //      stage a forest with 16-byte vector loads) with the per-pixel products the kernels
 //      need -- w*delta for eq. 2.4, and u = L - Lbar, w/sum w, w u/sum w u^2 for eq. 2.7
-//       -- plus one 64-byte head per forest (unit vector, first/last chi,
+//       -- plus one 80-byte head per forest (unit vector, first/last chi,
 //      smallest chi spacing, packed offset, length).
 //  (2) lya_bucket_pairs: a stable counting sort of the forest-pair list by the r_perp
 //      column of the pair's first pixel pair.  Pairs of one bucket touch the same
