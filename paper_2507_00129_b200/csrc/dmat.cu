@@ -340,15 +340,15 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
 //  pass C  the kept pairs are drained: T1..T3 per kept pair, T4 with lanes over the table entries and
 //          an inner loop over the kept pairs (the entry stays in registers); every update is one
 //          red.global.add.f64 into the L2-resident Dn.
-constexpr int FD_WARPS = 13;                 // one CTA per SM (shared memory: 17.2 KB per warp)
+constexpr int FD_WARPS = 14;                 // one CTA per SM (shared memory: 16.2 KB per warp)
 constexpr int FD_THREADS = FD_WARPS * 32;
 constexpr int FD_T = LYA_FAST_TILE;
 constexpr int FD_ROWS = 16;
 constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
 constexpr int FD_PAD = 2;
 constexpr int FD_SLOTS = 306;                // (n_par + 1) * LYA_NCOL <= FD_SLOTS
-constexpr int FD_KCAP = 96;                  // kept pairs queued per forest pair
-constexpr int FD_KBATCH = 32;                // kept pairs drained together (coefficient tables)
+constexpr int FD_KCAP = 48;                  // kept pairs queued per forest pair
+constexpr int FD_KBATCH = 24;                // kept pairs drained together (coefficient tables)
 constexpr int FD_CHUNK = 8;
 
 struct DmFastParams {
@@ -368,7 +368,6 @@ struct __align__(16) DmFastWarp {
     unsigned long long pk[FD_T], qk[FD_T];   // stage-4 keys of the pixels
     unsigned kept[FD_KCAP];                  // (i << 20) | (j << 12) | A
     double2 kc01[FD_KBATCH], kc23[FD_KBATCH]; // per kept pair of a batch: om (1, u_j), om (u_i, u_i u_j)
-    double2 kgeo[FD_KBATCH];                 // per kept pair of a batch: chi_i, chi_j
     unsigned short nz[FD_SLOTS];             // non-zero slots
     unsigned char jlo[FD_T], jx[FD_T], jhi[FD_T];
     unsigned nkept, pad_[3];
@@ -539,7 +538,6 @@ __device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, const unsigned *k
         const double omi = om * ui;
         ws.kc01[e] = make_double2(om, om * uj);
         ws.kc23[e] = make_double2(omi, omi * uj);
-        ws.kgeo[e] = make_double2(ws.pc[i], qc[j]);
         atomicAdd(P.Dn + (size_t)A * nb + A, om);
         atomicAdd(P.Wd + A, om);
         n_red += 2;
@@ -548,8 +546,8 @@ __device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, const unsigned *k
     // T2: -(om ea_j' + om u_j eg_j') over row i's window;  T3: -(om ea_i' + om u_i eg_i') over p
     for (int e = 0; e < n; ++e) {
         const unsigned rec = kept[e];
-        const int i = rec >> 20, A = rec & 0xfff;
-        const double2 c01 = ws.kc01[e], c23 = ws.kc23[e], geo = ws.kgeo[e];
+        const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
+        const double2 c01 = ws.kc01[e], c23 = ws.kc23[e], geo = make_double2(ws.pc[i], qc[j]);
         double *row = P.Dn + (size_t)A * nb;
         for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {
             const int B = lya_pix_bin_t<POW2>(bp, g, geo.x, qc[j2]);
