@@ -340,7 +340,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
 //  pass C  the kept pairs are drained: T1..T3 per kept pair, T4 with lanes over the table entries and
 //          an inner loop over the kept pairs (the entry stays in registers); every update is one
 //          red.global.add.f64 into the L2-resident Dn.
-constexpr int FD_WARPS = 14;                 // one CTA per SM (shared memory: 16.2 KB per warp)
+constexpr int FD_WARPS = 15;                 // one CTA per SM (shared memory: 15.1 KB per warp)
 constexpr int FD_THREADS = FD_WARPS * 32;
 constexpr int FD_T = LYA_FAST_TILE;
 constexpr int FD_ROWS = 16;
@@ -361,14 +361,17 @@ struct DmFastParams {
     unsigned long long *counters;   // [4] next chunk, [2] evaluated, [3] error, [5] kept, [6] binned, [7] scatter-adds
 };
 
+struct DmKeysA { unsigned long long pk[FD_T], qk[FD_T]; };                 // pass A: stage-4 keys of the pixels
+struct DmDrainBC {                                                            // passes B and C
+    double2 kc01[FD_KBATCH], kc23[FD_KBATCH];    // per kept pair of a batch: om (1, u_j), om (u_i, u_i u_j)
+    unsigned short nz[FD_SLOTS];                 // non-zero slots
+};
 struct __align__(16) DmFastWarp {
     double2 H01[FD_SLOTS], H23[FD_SLOTS];    // (H_aa, H_ag), (H_ga, H_gg) per slot = col_rel * (n_par + 1) + row
     double pc[FD_TP], pea[FD_TP], peg[FD_TP];            // (w and u of the kept pairs are read from HBM/L2 in the drain)
     double qc[FD_T + 2 * FD_PAD], qea[FD_T + 2 * FD_PAD], qeg[FD_T + 2 * FD_PAD];
-    unsigned long long pk[FD_T], qk[FD_T];   // stage-4 keys of the pixels
+    union { DmKeysA a; DmDrainBC b; } u;     // the keys are dead once pass A is done (shared memory buys occupancy)
     unsigned kept[FD_KCAP];                  // (i << 20) | (j << 12) | A
-    double2 kc01[FD_KBATCH], kc23[FD_KBATCH]; // per kept pair of a batch: om (1, u_j), om (u_i, u_i u_j)
-    unsigned short nz[FD_SLOTS];             // non-zero slots
     unsigned char jlo[FD_T], jx[FD_T], jhi[FD_T];
     unsigned nkept, pad_[3];
 };
@@ -439,7 +442,7 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h
         // keys, mask and queueing of one row (i, window slot of diagonal k = (k + u) % D)
         auto row_keys = [&](int i, int u, bool live, unsigned *key_o, double *fa_o, double *fg_o) {
             const double pci = ws.pc[i];
-            const unsigned long long pki = ws.pk[min(i, FD_T - 1)];
+            const unsigned long long pki = ws.u.a.pk[min(i, FD_T - 1)];
 #pragma unroll
             for (int k = 0; k < D; ++k) {
                 const int sl = (k + u) % D;
@@ -448,7 +451,7 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h
                 fa_o[k] = wa[sl]; fg_o[k] = wg[sl];
                 valid = valid && live;
                 const int j = i + dl + k;
-                const bool kp = valid && keep_pair(pki, ws.qk[min(max(j, 0), FD_T - 1)], thr);
+                const bool kp = valid && keep_pair(pki, ws.u.a.qk[min(max(j, 0), FD_T - 1)], thr);
                 binned += valid ? 1u : 0u;
                 if (kp) {                                    // ~1 % of the pairs at f = 0.99
                     const unsigned idx = atomicAdd(&ws.nkept, 1u);
@@ -536,8 +539,8 @@ __device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, const unsigned *k
         const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
         const double om = P.prep.w[offp + i] * P.prep.w[offq + j], ui = P.prep.u[offp + i], uj = P.prep.u[offq + j];
         const double omi = om * ui;
-        ws.kc01[e] = make_double2(om, om * uj);
-        ws.kc23[e] = make_double2(omi, omi * uj);
+        ws.u.b.kc01[e] = make_double2(om, om * uj);
+        ws.u.b.kc23[e] = make_double2(omi, omi * uj);
         atomicAdd(P.Dn + (size_t)A * nb + A, om);
         atomicAdd(P.Wd + A, om);
         n_red += 2;
@@ -547,7 +550,7 @@ __device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, const unsigned *k
     for (int e = 0; e < n; ++e) {
         const unsigned rec = kept[e];
         const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
-        const double2 c01 = ws.kc01[e], c23 = ws.kc23[e], geo = make_double2(ws.pc[i], qc[j]);
+        const double2 c01 = ws.u.b.kc01[e], c23 = ws.u.b.kc23[e], geo = make_double2(ws.pc[i], qc[j]);
         double *row = P.Dn + (size_t)A * nb;
         for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {
             const int B = lya_pix_bin_t<POW2>(bp, g, geo.x, qc[j2]);
@@ -560,14 +563,14 @@ __device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, const unsigned *k
     }
     // T4: lanes over the non-zero table entries, inner loop over the kept pairs
     for (int t = lane; t < nnz; t += 32) {
-        const int slot = ws.nz[t];
+        const int slot = ws.u.b.nz[t];
         const int cr = slot / np1, bx = slot - cr * np1;
         double *colB = P.Dn + ((c0 + cr) * bp.n_par + bx);
         const double2 a = ws.H01[slot], b = ws.H23[slot];
 #pragma unroll 2
         for (int e = 0; e < n; ++e) {
             const int A = kept[e] & 0xfff;
-            const double2 c01 = ws.kc01[e], c23 = ws.kc23[e];
+            const double2 c01 = ws.u.b.kc01[e], c23 = ws.u.b.kc23[e];
             const double v = fma(c23.y, b.y, fma(c23.x, b.x, fma(c01.y, a.y, c01.x * a.x)));
             atomicAdd(colB + (size_t)A * nb, v);
         }
@@ -635,7 +638,6 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 for (int t = lane; 2 * t < mp; t += 32) {
                     ((double2 *)ws.pc)[t] = s0[t]; ((double2 *)ws.pea)[t] = s3[t]; ((double2 *)ws.peg)[t] = s4[t];
                 }
-                for (int t = lane; t < mp; t += 32) ws.pk[t] = key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
                 __syncwarp();
                 for (int t = mp + lane; t < FD_TP; t += 32) {            // sentinel rows (!= q's sentinel: r_par never 0)
                     ws.pc[t] = 2.0 * LYA_CHI_SENTINEL; ws.pea[t] = 0.0; ws.peg[t] = 0.0;
@@ -649,7 +651,9 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 for (int t = lane; t < npad2; t += 32) {
                     ((double2 *)qc)[t] = s0[t]; ((double2 *)(ws.qea + FD_PAD))[t] = s3[t]; ((double2 *)(ws.qeg + FD_PAD))[t] = s4[t];
                 }
-                for (int t = lane; t < mq; t += 32) ws.qk[t] = key_hi(P.seed, (unsigned long long)(hq.pix0 + t));
+                for (int t = lane; t < mq; t += 32) ws.u.a.qk[t] = key_hi(P.seed, (unsigned long long)(hq.pix0 + t));
+                // (the keys share their storage with the drain tables, so p's keys are rebuilt for every pair)
+                for (int t = lane; t < mp; t += 32) ws.u.a.pk[t] = key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
                 if (lane < FD_PAD) {
                     const int j = FD_PAD + 2 * npad2 + lane;
                     ws.qc[j] = LYA_CHI_SENTINEL; ws.qea[j] = 0.0; ws.qeg[j] = 0.0;
@@ -706,7 +710,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                     nzf = (bx < bp.n_par) && (cr < LYA_NCOL) && (a.x != 0.0 || a.y != 0.0 || b.x != 0.0 || b.y != 0.0);
                 }
                 const unsigned bal = __ballot_sync(0xffffffffu, nzf);
-                if (nzf) ws.nz[nnz + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)t;
+                if (nzf) ws.u.b.nz[nnz + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)t;
                 nnz += __popc(bal);
             }
             __syncwarp();
@@ -726,7 +730,8 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                         const int j = sj + lane;
                         int A = -1;
                         if (j < jh) A = lya_pix_bin_t<POW2>(bp, g, ws.pc[si], qc[j]);
-                        const bool kp = (A >= 0) && keep_pair(ws.pk[si], ws.qk[min(j, FD_T - 1)], P.thr);
+                        const bool kp = (A >= 0) && keep_pair(key_lo(P.seed, (unsigned long long)(hp.pix0 + si)),
+                                                              key_hi(P.seed, (unsigned long long)(hq.pix0 + j)), P.thr);   // (the staged keys are gone)
                         const unsigned bal = __ballot_sync(0xffffffffu, kp);
                         if (n_q + __popc(bal) > FD_KCAP) break;          // drain first, then redo these 32 pixels
                         if (kp) ws.kept[n_q + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)si << 20) | ((unsigned)j << 12) | (unsigned)A;
