@@ -172,14 +172,18 @@ CONFIGS[3] = CONFIGS[2]            # configs[3] = the same arrays as configs[2]
 
 
 def make_config(cfg: int, n_forest: int | None = None, density_scale: float = 1.0,
-                seed: int | None = None) -> Forests:
+                seed: int | None = None, fine: int = 1) -> Forests:
     """Catalogue for BASELINE.json configs[cfg].
 
     n_forest / density_scale give *shaped* sub-workloads for tests: fewer
     forests over a proportionally smaller RA width (same sky density, same
     pixel recipe) -- so the neighbour structure stays that of the config.
+    fine = k divides the pixel step by k (k times more pixels per forest):
+    native-resolution shapes of DESIGN.md NEXT-3 (fine=2 on configs[2] is the
+    3.3 Mpc/h spacing of SDSS).  Throughput workloads only.
     """
     c = CONFIGS[cfg]
+    fine = int(fine)
     seed_cfg = 2 if cfg == 3 else cfg
     rng = np.random.default_rng(SEED_BASE + seed_cfg if seed is None else seed)
     n = c["n"] if n_forest is None else int(n_forest)
@@ -194,27 +198,29 @@ def make_config(cfg: int, n_forest: int | None = None, density_scale: float = 1.
     ux, uy, uz = unit_vectors(ra, dec)
 
     if c["grid"] == "log24":
-        counts = np.full(n, 24, dtype=np.int64)
+        counts = np.full(n, 24 * fine, dtype=np.int64)
         off, fid, k = _ragged(counts)
-        loglam = np.log10(LAM_REST_MIN * (1.0 + zq[fid])) + 1e-3 * k
+        loglam = np.log10(LAM_REST_MIN * (1.0 + zq[fid])) + (1e-3 / fine) * k
         lam = 10.0 ** loglam
     elif c["grid"] == "logglobal":
         l0 = np.log10(LAM_OBS_MIN)
         # global grid index range per forest: 1040(1+zq) <= lam_k <= 1200(1+zq), lam_k >= 3600
-        klo = np.ceil((np.log10(LAM_REST_MIN * (1 + zq)) - l0) / 1e-3 - 1e-9).astype(np.int64)
-        khi = np.floor((np.log10(LAM_REST_MAX * (1 + zq)) - l0) / 1e-3 + 1e-9).astype(np.int64)
+        dl = 1e-3 / fine
+        klo = np.ceil((np.log10(LAM_REST_MIN * (1 + zq)) - l0) / dl - 1e-9).astype(np.int64)
+        khi = np.floor((np.log10(LAM_REST_MAX * (1 + zq)) - l0) / dl + 1e-9).astype(np.int64)
         klo = np.maximum(klo, 0)
         counts = np.maximum(khi - klo + 1, 0)
         off, fid, k = _ragged(counts)
-        loglam = l0 + 1e-3 * (klo[fid] + k)
+        loglam = l0 + dl * (klo[fid] + k)
         lam = 10.0 ** loglam
     elif c["grid"] == "lin2p4":
         # R-9a: 2.4 A steps in the REST frame, k = 0..66
-        kmin = np.ceil((LAM_OBS_MIN / (1 + zq) - LAM_REST_MIN) / 2.4 - 1e-9).astype(np.int64)
+        st = 2.4 / fine
+        kmin = np.ceil((LAM_OBS_MIN / (1 + zq) - LAM_REST_MIN) / st - 1e-9).astype(np.int64)
         kmin = np.maximum(kmin, 0)
-        counts = np.maximum(67 - kmin, 0)
+        counts = np.maximum(int(np.floor(160.0 / st + 1e-9)) + 1 - kmin, 0)
         off, fid, k = _ragged(counts)
-        lam = (LAM_REST_MIN + 2.4 * (kmin[fid] + k)) * (1 + zq[fid])
+        lam = (LAM_REST_MIN + st * (kmin[fid] + k)) * (1 + zq[fid])
         loglam = np.log10(lam)
     else:
         raise ValueError(c["grid"])
