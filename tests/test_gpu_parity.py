@@ -408,7 +408,7 @@ def test_full_size_properties_and_sampled_parity(ctx, B, orc, cfg):
     sel = torch.from_numpy(rng.choice(pairs.n, 20000, replace=False)).to(pq.device)
     sub = pq[sel].cpu().numpy()
     check_xi(ctx.lya_xi2pcf(d, b, ctx.lya_pairs_import(sub)), orc.xi(f, sub), f"cfg{cfg} sampled pairs")
-    subd = sub[:1500]
+    subd = sub[:5000]
     seed = gen.mask_seed(3 if cfg == 2 else cfg)
     check_dmat(ctx.lya_dmat(d, b, ctx.lya_pairs_import(subd), 0.99, seed), orc.dmat(f, subd, 0.99, seed),
                f"cfg{cfg} sampled pairs D")
