@@ -97,6 +97,7 @@ struct DmWarpSmem {
     unsigned long long qk[DTILE];
     double H[4][H_SLOTS];
     unsigned kept[KEPT_CAP];        // (i << 20) | (j << 12) | bin
+    unsigned short nz[H_SLOTS];     // non-zero slots of the H tables of the current column chunk
 };
 
 __device__ __forceinline__ void red_add(double *addr, double v) { atomicAdd(addr, v); }
@@ -108,44 +109,45 @@ template <bool POW2>
 __device__ void drain_kept(DmWarpSmem &ws, int n_kept, const DmParams &P, const PairBin &g,
                            int64_t op, int np, double lbp, double invSp, double invVp,
                            int64_t oq, int nq, double lbq, double invSq, double invVq,
-                           int c0, int ncol, bool first_chunk, int lane)
+                           int c0, int ncol, int nnz, bool first_chunk, int lane)
 {
     const BinParams &bp = P.bp;
     const int nb = bp.n_par * bp.n_perp;
     const double *qc = ws.qc + DQPAD, *qw = ws.qw + DQPAD, *qu = ws.qu + DQPAD;
-    for (int e = 0; e < n_kept; ++e) {
+    for (int e = 0; first_chunk && e < n_kept; ++e) {
         const unsigned rec = ws.kept[e];
         const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
         const double om = ws.pw[i] * qw[j];
         const double ui = ws.pu[i], uj = qu[j];
         const int At = lya_bin_tr(bp, A);                                  // Dn, Wd are accumulated in transposed bin order
         double *row = P.Dn + (size_t)At * nb;
-        if (first_chunk) {
-            if (lane == 0) { red_add(row + At, om); red_add(P.Wd + At, om); }
-            for (int j2 = lane; j2 < nq; j2 += 32) {                       // T2
-                int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i], P.chi[oq + j2]);
-                if (B >= 0) {
-                    const double w2 = P.w[oq + j2], u2 = P.loglam[oq + j2] - lbq;
-                    red_add(row + B, -om * (w2 * invSq + uj * (w2 * u2 * invVq)));
-                }
-            }
-            for (int i2 = lane; i2 < np; i2 += 32) {                       // T3
-                int B = lya_pix_bin_t<POW2>(bp, g, P.chi[op + i2], qc[j]);
-                if (B >= 0) {
-                    const double w2 = P.w[op + i2], u2 = P.loglam[op + i2] - lbp;
-                    red_add(row + B, -om * (w2 * invSp + ui * (w2 * u2 * invVp)));
-                }
+        if (lane == 0) { red_add(row + At, om); red_add(P.Wd + At, om); }
+        for (int j2 = lane; j2 < nq; j2 += 32) {                           // T2
+            int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i], P.chi[oq + j2]);
+            if (B >= 0) {
+                const double w2 = P.w[oq + j2], u2 = P.loglam[oq + j2] - lbq;
+                red_add(row + B, -om * (w2 * invSq + uj * (w2 * u2 * invVq)));
             }
         }
-        const int n_slots = bp.n_par * ncol;                               // T4
-        for (int t = lane; t < n_slots; t += 32) {
-            double haa = ws.H[0][t];
-            if (haa != 0.0 || ws.H[3][t] != 0.0 || ws.H[1][t] != 0.0 || ws.H[2][t] != 0.0) {
-                int bx = t / ncol, lc = t - bx * ncol;
-                int B = (c0 + lc) * bp.n_par + bx;
-                double v = haa + uj * ws.H[1][t] + ui * ws.H[2][t] + ui * uj * ws.H[3][t];
-                red_add(row + B, om * v);
+        for (int i2 = lane; i2 < np; i2 += 32) {                           // T3
+            int B = lya_pix_bin_t<POW2>(bp, g, P.chi[op + i2], qc[j]);
+            if (B >= 0) {
+                const double w2 = P.w[op + i2], u2 = P.loglam[op + i2] - lbp;
+                red_add(row + B, -om * (w2 * invSp + ui * (w2 * u2 * invVp)));
             }
+        }
+    }
+    // T4: lanes over the non-zero table entries of this column chunk, inner loop over the kept pairs
+    for (int t = lane; t < nnz; t += 32) {
+        const int slot = ws.nz[t];
+        const int bx = slot / ncol, lc = slot - bx * ncol;
+        double *colB = P.Dn + ((c0 + lc) * bp.n_par + bx);
+        const double h0 = ws.H[0][slot], h1 = ws.H[1][slot], h2 = ws.H[2][slot], h3 = ws.H[3][slot];
+        for (int e = 0; e < n_kept; ++e) {
+            const unsigned rec = ws.kept[e];
+            const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
+            const double om = ws.pw[i] * qw[j], ui = ws.pu[i], uj = qu[j];
+            red_add(colB + (size_t)lya_bin_tr(bp, A) * nb, om * ((h0 + uj * h1) + ui * (h2 + uj * h3)));
         }
     }
 }
@@ -275,6 +277,15 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
                     }
                 }
                 __syncwarp();
+                int nnz = 0;                                               // compact the non-zero entries once per chunk
+                for (int t0 = 0; t0 < n_slots; t0 += 32) {
+                    const int t = t0 + lane;
+                    const bool nzf = t < n_slots && (ws.H[0][t] != 0.0 || ws.H[1][t] != 0.0 || ws.H[2][t] != 0.0 || ws.H[3][t] != 0.0);
+                    const unsigned bal = __ballot_sync(0xffffffffu, nzf);
+                    if (nzf) ws.nz[nnz + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)t;
+                    nnz += __popc(bal);
+                }
+                __syncwarp();
                 // ---- pass 1b: mask every in-grid pair of every tile pair, queue the kept ones, drain ----
                 for (int ip0 = 0; ip0 < np; ip0 += DTILE) {
                     const int mp = min(DTILE, np - ip0);
@@ -299,7 +310,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
                                 if (bal) {
                                     if (n_q + __popc(bal) > KEPT_CAP) {
                                         __syncwarp();
-                                        drain_kept<POW2>(ws, n_q, P, g, op, np, lbp, invSp, invVp, oq, nq, lbq, invSq, invVq, c0, ncol, first_chunk, lane);
+                                        drain_kept<POW2>(ws, n_q, P, g, op, np, lbp, invSp, invVp, oq, nq, lbq, invSq, invVq, c0, ncol, nnz, first_chunk, lane);
                                         __syncwarp();
                                         n_q = 0;
                                     }
@@ -309,7 +320,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
                             }
                         }
                         __syncwarp();
-                        drain_kept<POW2>(ws, n_q, P, g, op, np, lbp, invSp, invVp, oq, nq, lbq, invSq, invVq, c0, ncol, first_chunk, lane);
+                        drain_kept<POW2>(ws, n_q, P, g, op, np, lbp, invSp, invVp, oq, nq, lbq, invSq, invVq, c0, ncol, nnz, first_chunk, lane);
                         __syncwarp();
                     }
                 }
