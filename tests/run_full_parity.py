@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Full-size parity, run by hand on a GPU box (too slow for the pytest suite: the oracle needs minutes):
 
-    python tests/run_full_parity.py [cfg] [--dmat]
+    python tests/run_full_parity.py [cfg] [--dmat] [--no-xi]
 
 configs[cfg] (default 2) in full: lya_neighbours -> lya_xi2pcf against the CPU oracle over EVERY listed
 forest pair (N bit-exact, S/W to 1e-9), and with --dmat lya_dmat (f = 0.99, the config's mask seed)
@@ -20,17 +20,8 @@ from oracle import oracle as orc                      # noqa: E402
 from paper_2507_00129_b200 import binding as B, gen   # noqa: E402
 
 
-def main():
-    cfg = int(sys.argv[1]) if len(sys.argv) > 1 and sys.argv[1].isdigit() else 2
-    do_d = "--dmat" in sys.argv
-    f = gen.make_config(cfg)
-    ctx = B.Context("cuda:0")
-    d = B.DeviceForests(f)
-    b = B.binning()
-    pairs = ctx.lya_neighbours(d, b)
-    pq = pairs.export().cpu().numpy()
+def xi_check(ctx, d, b, pairs, cat, pq, cfg):
     g = ctx.lya_xi2pcf(d, b, pairs)
-    cat = orc.Catalogue(f)
     t0 = time.time()
     o = orc.xi(cat, pq)
     N = g["N"].cpu().numpy().view(np.uint64)
@@ -41,6 +32,21 @@ def main():
           f"{int((N != o['N']).sum())}; max rel err S {errS:.2e} W {errW:.2e}; GPU {g['stats']['ms_main']:.0f} ms, "
           f"oracle {time.time() - t0:.0f} s on {orc.num_threads()} threads", flush=True)
     assert np.array_equal(N, o["N"]) and errS <= 1e-9 and errW <= 1e-9
+
+
+def main():
+    cfg = int(sys.argv[1]) if len(sys.argv) > 1 and sys.argv[1].isdigit() else 2
+    do_d = "--dmat" in sys.argv
+    do_xi = "--no-xi" not in sys.argv
+    f = gen.make_config(cfg)
+    ctx = B.Context("cuda:0")
+    d = B.DeviceForests(f)
+    b = B.binning()
+    pairs = ctx.lya_neighbours(d, b)
+    pq = pairs.export().cpu().numpy()
+    cat = orc.Catalogue(f)
+    if do_xi:
+        xi_check(ctx, d, b, pairs, cat, pq, cfg)
     if do_d:
         seed = gen.mask_seed(3 if cfg == 2 else cfg)
         gd = ctx.lya_dmat(d, b, pairs, 0.99, seed, want_Dn=False)
