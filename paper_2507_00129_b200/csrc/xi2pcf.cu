@@ -12,20 +12,21 @@
 //     accumulators (red.global) only when the warp moves to another bucket;
 //   * both forests are staged in shared memory from the padded catalogue with 16-byte
 //     loads (forest p is reused across the consecutive pairs that share it);
-//   * lanes own DIAGONALS d = j - i of the (i, j) pixel-pair matrix.  Along a diagonal
-//     r_par is nearly constant and r_perp grows slowly, so consecutive pairs fall in the
-//     same bin: a lane accumulates a RUN (S, W, count) in registers and touches the
-//     sub-histogram only when the bin changes;
-//   * B200 has no native shared-memory fp64 (or 64-bit) atomic add -- they compile to a
-//     CAS loop -- so the run flush is a plain load-add-store, made safe by construction:
-//     the lanes of one flush hold pixel pairs (i, j_lane) with the same i and distinct j,
-//     and the pair is walked twice, once over chi_i >= chi_j and once over chi_i < chi_j,
-//     so two lanes can share a bin only if q's pixel spacing is below the r_par bin width;
-//     such pairs (and long forests, wide column spans) go to the generic kernel below,
-//     which uses CAS atomics on a block-level histogram;
-//   * only diagonals/rows that can hold an in-grid pair are walked: per-row binary
-//     searches on the increasing chi give the r_par window and the sign change, and a
-//     binary search along the first diagonal of each pass cuts the rows past r_perp_max.
+//   * lanes own DIAGONALS d = j - i of the (i, j) pixel-pair matrix (1, 2 or 4 adjacent ones per
+//     lane, sliding register window over q).  Along a diagonal r_par is nearly constant and
+//     r_perp grows slowly, so consecutive pairs fall in the same bin: a lane works on a RUN and
+//     touches the sub-histogram only when the bin changes;
+//   * B200 has no native shared-memory fp64 (or 64-bit) atomic add -- they compile to a CAS loop.
+//     The fast kernel needs none: the lanes of one row step hold pixel pairs (i, j_lane) with the
+//     same i and distinct j, which fall in distinct bins on each side of chi_i = chi_j when q's
+//     pixel spacing exceeds the r_par bin width (the two sides have their own rows), so every
+//     entry has one lane working on it and that lane simply HOLDS the entry (S, W, N) in registers,
+//     storing it back and loading the next one with predicated st/ld.shared when its bin changes.
+//     Pairs that break the assumption (and long forests, wide column spans) go to the generic
+//     kernel below, which uses CAS atomics on a block-level histogram;
+//   * only rows/diagonals that can hold an in-grid pair are walked: two binary searches per row of p
+//     on the increasing chi of q give the window (r_par band and r_perp cut), and the matrix is
+//     walked 16 rows at a time over exactly the diagonals those rows need.
 // Geometry is exact binary64, operation by operation (lya_internal.cuh), so N is
 // bit-identical to the oracle for any traversal order.
 #include <stdlib.h>
