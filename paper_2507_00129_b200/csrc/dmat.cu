@@ -17,11 +17,15 @@
 // rank-4 update (about 14 kept pairs x 116 bins per forest pair at f = 0.99): not a
 // dense GEMM, so no tensor cores.
 //
-// One warp per forest pair.  Pass 1a: diagonal walk with register run-length
-// accumulation of (H_aa, H_ag, H_ga, H_gg) into a warp-private shared-memory table
-// indexed by (b_par, b_perp - c0).  Pass 1b: every in-grid pair is hashed (stage 4
-// mask, pure integer); kept pairs are queued in shared memory and drained by the whole
-// warp: T1-T4 go to the L2-resident Dn with red.global.add.f64.
+// Two kernels, one warp per forest pair in both, every update one red.global.add.f64 into the
+// L2-resident Dn (kept in TRANSPOSED bin order b_perp * n_par + b_par; k_dmat_normalise permutes):
+//   k_dmat_fast  (below, second half of the file) for the pairs of the bucketed list: H tables by the
+//                xi kernel's diagonal walk with entries held in registers, mask hashed on the fly,
+//                compacted drain -- see its header;
+//   k_dmat       generic: forests of any length in 128-pixel tiles, any column span (chunks of LC
+//                columns), any pixel spacing; H tables with CAS shared atomics (pass 1a), mask and
+//                drain per tile pair (pass 1b), T2/T3 read the whole forests from global memory.
+// lya_pairs_subsample (forest-pair subsampling) lives here too: it shares the mask.
 #include <stdlib.h>
 #include "lya_internal.cuh"
 
