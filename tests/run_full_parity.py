@@ -1,11 +1,13 @@
 #!/usr/bin/env python
 """Full-size parity, run by hand on a GPU box (too slow for the pytest suite: the oracle needs minutes):
 
-    python tests/run_full_parity.py [cfg] [--dmat] [--no-xi]
+    python tests/run_full_parity.py [cfg] [--dmat] [--no-xi] [--dmat-frac F]
 
 configs[cfg] (default 2) in full: lya_neighbours -> lya_xi2pcf against the CPU oracle over EVERY listed
 forest pair (N bit-exact, S/W to 1e-9), and with --dmat lya_dmat (f = 0.99, the config's mask seed)
-against the naive quadruple sum (n_kept exact, D to 1e-7 per entry).  Prints one summary line per check.
+against the naive quadruple sum (n_kept exact, D to 1e-7 per entry); --dmat-frac F restricts the D check
+to the first fraction F of the forest-pair list (the naive oracle of configs[4] needs ~75 min for all of
+it).  Prints one summary line per check.
 """
 import os
 import sys
@@ -49,13 +51,17 @@ def main():
         xi_check(ctx, d, b, pairs, cat, pq, cfg)
     if do_d:
         seed = gen.mask_seed(3 if cfg == 2 else cfg)
+        frac = float(sys.argv[sys.argv.index("--dmat-frac") + 1]) if "--dmat-frac" in sys.argv else 1.0
+        if frac < 1.0:
+            pq = pq[: int(len(pq) * frac)]
+            pairs = ctx.lya_pairs_import(pq)
         gd = ctx.lya_dmat(d, b, pairs, 0.99, seed, want_Dn=False)
         t0 = time.time()
         od = orc.dmat(cat, pq, 0.99, seed)
         D = gd["D"].cpu().numpy()
         err = np.max(np.abs(D - od["D"]) / np.maximum(np.abs(od["D"]), 1e-6))
         errWd = np.max(np.abs(gd["Wd"].cpu().numpy() - od["Wd"]) / np.maximum(od["Wd"], 1e-300))
-        print(f"cfg{cfg} D (f=0.99): n_kept GPU {gd['stats']['n_kept']} oracle {od['n_kept']}; max err D / max(|D|,1e-6) "
+        print(f"cfg{cfg} D (f=0.99, {len(pq)} forest pairs): n_kept GPU {gd['stats']['n_kept']} oracle {od['n_kept']}; max err D / max(|D|,1e-6) "
               f"{err:.2e}; Wd {errWd:.2e}; GPU {gd['stats']['ms_main']:.0f} ms, oracle {time.time() - t0:.0f} s", flush=True)
         assert gd["stats"]["n_kept"] == od["n_kept"] and err <= 1e-7 and errWd <= 1e-9
     print("full parity ok")
