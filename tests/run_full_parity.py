@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Full-size parity, run by hand on a GPU box (too slow for the pytest suite: the oracle needs minutes):
 
-    python tests/run_full_parity.py [cfg] [--dmat] [--no-xi] [--dmat-frac F]
+    python tests/run_full_parity.py [cfg] [--dmat] [--no-xi] [--dmat-frac F] [--dmat-skip F0]
 
 configs[cfg] (default 2) in full: lya_neighbours -> lya_xi2pcf against the CPU oracle over EVERY listed
 forest pair (N bit-exact, S/W to 1e-9), and with --dmat lya_dmat (f = 0.99, the config's mask seed)
@@ -52,8 +52,9 @@ def main():
     if do_d:
         seed = gen.mask_seed(3 if cfg == 2 else cfg)
         frac = float(sys.argv[sys.argv.index("--dmat-frac") + 1]) if "--dmat-frac" in sys.argv else 1.0
-        if frac < 1.0:
-            pq = pq[: int(len(pq) * frac)]
+        skip = float(sys.argv[sys.argv.index("--dmat-skip") + 1]) if "--dmat-skip" in sys.argv else 0.0
+        if frac < 1.0 or skip > 0.0:                   # forest pairs [skip, skip + frac) of the list
+            pq = pq[int(len(pq) * skip): int(len(pq) * min(skip + frac, 1.0))]
             pairs = ctx.lya_pairs_import(pq)
         gd = ctx.lya_dmat(d, b, pairs, 0.99, seed, want_Dn=False)
         t0 = time.time()
