@@ -86,6 +86,20 @@ class ClockSampler:
                     reasons=sorted(reasons), samples=len(sm))
 
 
+def micro_peaks(device=0):
+    """Roofline denominators measured by liblya_peaks.so (include/lya_peaks.h; bench-only library)."""
+    import ctypes as C
+    from paper_2507_00129_b200 import build
+    lib = C.CDLL(build.build_peaks())
+    lib.lya_measure_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+    out = {}
+    for kind, name in enumerate(("fp64_fma", "fp64_add", "smem_cas64", "smem_add32", "l2_red64")):
+        r = C.c_double()
+        rc = lib.lya_measure_peak(device, kind, C.byref(r))
+        out[name] = r.value if rc == 0 else None
+    return out
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -291,7 +305,7 @@ def main():
         peak_alu = ctx.sm_count() * FP64_LANES_PER_SM * peaks.get("sm_max_mhz", 1965.0) * 1e6
         peak_src = (f"derived: {ctx.sm_count()} SMs x {FP64_LANES_PER_SM} fp64 lanes x sm_max_mhz "
                     f"({peak_kind} MEASURED_PEAKS.json); DFMA/DADD microbenchmarks in measured_peaks")
-        mp = {k: ctx.lya_measure_peak(k) for k in ("fp64_fma", "fp64_add", "smem_cas64", "smem_add32", "l2_red64")}
+        mp = micro_peaks(local)
         alg_xi = 8.0 * sx["n_binned"]
         roof_xi = {"bound": "alu", "kernel": "k_xi_fast", "achieved": alg_xi / t_xi / 1e12, "peak": peak_alu / 1e12,
                    "unit": "Tops/s (fp64 lane-operations)", "frac": alg_xi / t_xi / peak_alu, "traffic": None,

@@ -103,6 +103,16 @@ void        lya_destroy(lya_ctx *ctx);
 const char *lya_last_error(const lya_ctx *ctx);   /* host string, owned by ctx */
 const char *lya_version(void);
 
+/* Explicit, per-ctx switches (there are no environment variables or global flags).
+ *   LYA_OPT_FORCE_GENERIC     0 (default) / 1: route EVERY forest pair to the generic kernels (block-level
+ *                             histogram / CAS H tables) instead of the fast ones.  Results are identical
+ *                             (N, n_kept exactly; sums to rounding); tests use it to cover both routes.
+ *   LYA_OPT_GENERIC_DIAGONALS 1, 2 (default) or 4: diagonals of the pixel-pair matrix per lane in the
+ *                             generic xi kernel (a tuning knob; results do not depend on it).
+ * LYA_ERR_INVALID_ARG for an unknown option or value. */
+typedef enum { LYA_OPT_FORCE_GENERIC = 0, LYA_OPT_GENERIC_DIAGONALS = 1 } lya_option;
+lya_status  lya_set_option(lya_ctx *ctx, lya_option opt, int64_t value);
+
 /* ---- stage 1: neighbour search (north_star stage 1) ------------ */
 /* Lists every unordered pair of distinct non-empty forests {p<q} with
  *   (chi_p[0] + chi_q[0]) * s_pq < rperp_max            (reading G4)
@@ -184,22 +194,6 @@ lya_status lya_run_host(lya_ctx *ctx, const lya_forests *f_host, const lya_binni
                         double *S, double *W, uint64_t *N, double *xi,
                         double *D, double *Wd,
                         int64_t *n_pairs, lya_stats *stats_xi, lya_stats *stats_dmat);
-
-/* ---- measured roofline denominators ------------------------ */
-/* Microbenchmarks of the units that bound the pair loops, run on the ctx device.
- * Each returns operations per second through *rate (host out) and synchronises.
- *   LYA_PEAK_FP64_FMA     warp-level DFMA instructions x 32 lanes per second
- *   LYA_PEAK_FP64_ADD     same for DADD
- *   LYA_PEAK_SMEM_CAS64   lane-level shared-memory fp64 atomic adds (CAS loop) per second,
- *                         random bins of a 2500-entry histogram
- *   LYA_PEAK_SMEM_ADD32   lane-level native shared-memory u32 atomic adds per second
- *   LYA_PEAK_L2_RED64     lane-level red.global.add.f64 per second into an L2-resident
- *                         2500 x 2500 double matrix (random row, contiguous segment) */
-typedef enum {
-    LYA_PEAK_FP64_FMA = 0, LYA_PEAK_FP64_ADD = 1, LYA_PEAK_SMEM_CAS64 = 2,
-    LYA_PEAK_SMEM_ADD32 = 3, LYA_PEAK_L2_RED64 = 4
-} lya_peak_kind;
-lya_status lya_measure_peak(lya_ctx *ctx, lya_peak_kind kind, double *rate);
 
 #ifdef __cplusplus
 }

@@ -13,13 +13,13 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblya.so")
 
-EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_neighbours",
+EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_set_option", "lya_neighbours",
            "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
-           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host", "lya_measure_peak"]
+           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
           4: "LYA_ERR_CAPACITY", 5: "LYA_ERR_OOM", 6: "LYA_ERR_CUDA", 7: "LYA_ERR_UNIMPLEMENTED"}
-PEAK_KINDS = {"fp64_fma": 0, "fp64_add": 1, "smem_cas64": 2, "smem_add32": 3, "l2_red64": 4}
+OPTIONS = {"force_generic": 0, "generic_diagonals": 1}
 
 
 class LyaError(RuntimeError):
@@ -83,7 +83,7 @@ def load():
         lib.lya_run_host.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_int, C.c_int,
                                      C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.POINTER(C.c_int64), C.POINTER(CStats), C.POINTER(CStats)]
-        lib.lya_measure_peak.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+        lib.lya_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         _lib = lib
     return _lib
 
@@ -279,7 +279,5 @@ class Context:
         out["stats_dmat"] = sd.as_dict()
         return out
 
-    def lya_measure_peak(self, kind: str) -> float:
-        r = C.c_double()
-        self._check(load().lya_measure_peak(self.h, PEAK_KINDS[kind], C.byref(r)))
-        return r.value
+    def lya_set_option(self, opt: str, value: int):
+        self._check(load().lya_set_option(self.h, OPTIONS[opt], int(value)))

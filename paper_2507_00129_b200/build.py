@@ -1,4 +1,5 @@
-"""In-tree build of liblya.so with nvcc for sm_100a (no JIT cache, no torch extension)."""
+"""In-tree build of liblya.so (the product) and liblya_peaks.so (bench-only microbenchmarks)
+with nvcc for sm_100a (no JIT cache, no torch extension)."""
 from __future__ import annotations
 
 import os
@@ -8,9 +9,11 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblya.so")
-SOURCES = ["lya_api.cu", "neighbours.cu", "prep.cu", "xi2pcf.cu", "dmat.cu", "peaks.cu"]
+LIB_PEAKS = os.path.join(HERE, "liblya_peaks.so")
+SOURCES = ["lya_api.cu", "neighbours.cu", "prep.cu", "xi2pcf.cu", "dmat.cu"]
+HEADERS = ["lya_internal.cuh", "lya_walk.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC"]
 
 
 def _nvcc() -> str:
@@ -20,25 +23,25 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+def _stale(lib, srcs) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + [os.path.join(CSRC, "lya_internal.cuh"),
-                                                        os.path.join(HERE, "..", "include", "lya.h")]
-    return any(os.path.getmtime(d) > t for d in deps)
+    t = os.path.getmtime(lib)
+    deps = [os.path.join(CSRC, s) for s in srcs] + [os.path.join(CSRC, h) for h in HEADERS]
+    deps += [os.path.join(HERE, "..", "include", h) for h in ("lya.h", "lya_peaks.h")]
+    return any(os.path.exists(d) and os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
     """Compile csrc/*.cu into paper_2507_00129_b200/liblya.so (sm_100a, -lineinfo)."""
-    if not force and not _stale():
+    if not force and not _stale(LIB, SOURCES):
         return LIB
     nvcc = _nvcc()
     objs = []
     procs = []
     for src in SOURCES:
         obj = os.path.join(CSRC, src.replace(".cu", ".o"))
-        cmd = [nvcc, *[f for f in NVCC_FLAGS if f != "--use_fast_math=false"], "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, *extra_flags, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT)))
@@ -53,5 +56,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_peaks(force: bool = False) -> str:
+    """liblya_peaks.so: roofline-denominator microbenchmarks, loaded by bench.py only."""
+    if not force and not _stale(LIB_PEAKS, ["peaks.cu"]):
+        return LIB_PEAKS
+    subprocess.check_call([_nvcc(), *NVCC_FLAGS, "-shared", os.path.join(CSRC, "peaks.cu"), "-o", LIB_PEAKS, "-lcudart"])
+    return LIB_PEAKS
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build_peaks(force="--force" in sys.argv))

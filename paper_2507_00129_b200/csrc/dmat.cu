@@ -890,7 +890,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     cudaStream_t s = ctx->stream;
     const BinParams bp = lya_make_binparams(b);
     const bool use_fast = pairs->n > 0 && (b->n_par + 1) * LYA_NCOL <= FD_SLOTS && b->n_perp + 2 <= 256 &&
-                          ctx->dmat_variant != 9;
+                          !ctx->force_generic;
     double *scal = NULL, *Dn = NULL, *Wd = NULL;          // internal accumulators (transposed bin order)
     bool own_Dn = false, own_Wd = false;
     const int64_t nf = f->n_forest;

@@ -42,10 +42,8 @@ extern "C" lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     if (cudaMalloc(&ctx->d_counters, 16 * sizeof(unsigned long long)) != cudaSuccess) { free(ctx); return LYA_ERR_OOM; }
     for (int i = 0; i < 4; ++i)
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { cudaFree(ctx->d_counters); free(ctx); return LYA_ERR_CUDA; }
-    const char *v = getenv("LYA_XI_VARIANT");
-    ctx->xi_variant = v ? atoi(v) : 0;
-    v = getenv("LYA_DMAT_VARIANT");
-    ctx->dmat_variant = v ? atoi(v) : 0;
+    ctx->force_generic = 0;
+    ctx->generic_diagonals = 2;
     ctx->err[0] = 0;
     *out = ctx;
     return LYA_OK;
@@ -61,6 +59,23 @@ extern "C" void lya_destroy(lya_ctx *ctx)
 }
 
 extern "C" const char *lya_last_error(const lya_ctx *ctx) { return ctx ? ctx->err : "null ctx"; }
+
+extern "C" lya_status lya_set_option(lya_ctx *ctx, lya_option opt, int64_t value)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    switch (opt) {
+    case LYA_OPT_FORCE_GENERIC:
+        if (value != 0 && value != 1) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "LYA_OPT_FORCE_GENERIC takes 0 or 1");
+        ctx->force_generic = (int)value;
+        return LYA_OK;
+    case LYA_OPT_GENERIC_DIAGONALS:
+        if (value != 1 && value != 2 && value != 4) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "LYA_OPT_GENERIC_DIAGONALS takes 1, 2 or 4");
+        ctx->generic_diagonals = (int)value;
+        return LYA_OK;
+    default:
+        return lya_fail(ctx, LYA_ERR_INVALID_ARG, "unknown option %d", (int)opt);
+    }
+}
 
 lya_status lya_check_binning(lya_ctx *ctx, const lya_binning *b)
 {

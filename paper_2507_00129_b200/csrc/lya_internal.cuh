@@ -18,8 +18,8 @@ struct lya_ctx {
     int sm_count;
     // small persistent device scratch
     unsigned long long *d_counters;   // [16] work counters / flags
-    int xi_variant;                   // kernel variant selector (env LYA_XI_VARIANT; tuning)
-    int dmat_variant;
+    int force_generic;                // LYA_OPT_FORCE_GENERIC: route every pair to the generic kernels
+    int generic_diagonals;            // LYA_OPT_GENERIC_DIAGONALS: diagonals per lane of the generic xi kernel (1, 2, 4)
     cudaEvent_t ev[4];
 };
 

@@ -1,7 +1,9 @@
-// peaks.cu -- lya_measure_peak: microbenchmarks of the units that bound the pair
-// loops (fp64 pipe issue rate, shared-memory atomics, L2 fp64 reductions).  They give
-// the MEASURED roofline denominators quoted in DESIGN.md / bench.py.
-#include "lya_internal.cuh"
+// peaks.cu -- liblya_peaks.so (include/lya_peaks.h): microbenchmarks of the units that bound the
+// pair loops (fp64 pipe issue rate, shared-memory atomics, L2 fp64 reductions).  They give the
+// MEASURED roofline denominators quoted in DESIGN.md / bench.py.  Built as its own library: the
+// product library liblya.so does not contain them.
+#include <cuda_runtime.h>
+#include "../../include/lya_peaks.h"
 
 namespace {
 
@@ -60,21 +62,27 @@ __global__ void k_peak_red(double *mat, int nb, int iters)
 
 }  // namespace
 
-extern "C" lya_status lya_measure_peak(lya_ctx *ctx, lya_peak_kind kind, double *rate)
+extern "C" int lya_measure_peak(int device, lya_peak_kind kind, double *rate)
 {
-    if (!ctx) return LYA_ERR_INVALID_ARG;
-    if (!rate) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_measure_peak: rate is NULL");
-    LYA_CUDA(cudaSetDevice(ctx->device));
-    cudaStream_t s = ctx->stream;
-    const int grid = ctx->sm_count * 4;
+    if (!rate) return (int)cudaErrorInvalidValue;
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return (int)e;
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) return (int)e;
+    const int grid = prop.multiProcessorCount * 4;
+    cudaEvent_t ev0, ev1;
+    if ((e = cudaEventCreate(&ev0)) != cudaSuccess) return (int)e;
+    if ((e = cudaEventCreate(&ev1)) != cudaSuccess) { cudaEventDestroy(ev0); return (int)e; }
+    cudaStream_t s = 0;
     double ops = 0.0;
     float ms = 0.f;
     double *buf = NULL;
     const int nb = 2500;
-    LYA_CUDA(cudaMalloc(&buf, sizeof(double) * (size_t)nb * nb));
+    auto done = [&](cudaError_t err) { cudaFree(buf); cudaEventDestroy(ev0); cudaEventDestroy(ev1); return (int)err; };
+    if ((e = cudaMalloc(&buf, sizeof(double) * (size_t)nb * nb)) != cudaSuccess) return done(e);
     cudaMemsetAsync(buf, 0, sizeof(double) * (size_t)nb * nb, s);
     for (int rep = 0; rep < 2; ++rep) {          // rep 0 = warm-up
-        cudaEventRecord(ctx->ev[0], s);
+        cudaEventRecord(ev0, s);
         switch (kind) {
         case LYA_PEAK_FP64_FMA: {
             int iters = 1 << 14;
@@ -102,16 +110,14 @@ extern "C" lya_status lya_measure_peak(lya_ctx *ctx, lya_peak_kind kind, double 
             ops = (double)grid * PK_THREADS * iters;
             break; }
         default:
-            cudaFree(buf);
-            return lya_fail(ctx, LYA_ERR_INVALID_ARG, "unknown peak kind");
+            return done(cudaErrorInvalidValue);
         }
-        cudaEventRecord(ctx->ev[1], s);
-        cudaError_t e = cudaGetLastError();
+        cudaEventRecord(ev1, s);
+        e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        if (e != cudaSuccess) { cudaFree(buf); return lya_cuda_fail(ctx, e, "lya_measure_peak"); }
-        cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]);
+        if (e != cudaSuccess) return done(e);
+        cudaEventElapsedTime(&ms, ev0, ev1);
     }
-    cudaFree(buf);
     *rate = ops / ((double)ms * 1e-3);
-    return LYA_OK;
+    return done(cudaSuccess);
 }

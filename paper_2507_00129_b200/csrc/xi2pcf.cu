@@ -653,8 +653,8 @@ static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *
         LYA_CUDA(cudaStreamSynchronize(s));
         if (bad) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_sub: region[] must lie in [0, n_region)");
     }
-    // fast path: bucketed list + warp-private sub-histograms (variant 9 forces the generic kernel)
-    const bool use_fast = pairs->n > 0 && 2 * (b->n_par + 1) * LYA_NCOL <= FSLOTS && b->n_perp + 2 <= 256 && ctx->xi_variant != 9;
+    // fast path: bucketed list + warp-private sub-histograms (LYA_OPT_FORCE_GENERIC routes everything to the generic kernel)
+    const bool use_fast = pairs->n > 0 && 2 * (b->n_par + 1) * LYA_NCOL <= FSLOTS && b->n_perp + 2 <= 256 && !ctx->force_generic;
     LyaPrep prep;
     LyaBuckets bk;
     memset(&prep, 0, sizeof(prep));
@@ -716,7 +716,7 @@ static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_direct launch"); }
     }
     while (!region && P.n_pairs > 0) {
-        switch (ctx->xi_variant) {
+        switch (ctx->generic_diagonals) {
         case 1: e = launch_xi<1>(P, grid, smem, s); break;
         case 4: e = launch_xi<4>(P, grid, smem, s); break;
         default: e = launch_xi<2>(P, grid, smem, s); break;

@@ -91,9 +91,10 @@ def test_cfg0_xi_all_pairs_and_neighbour_list(ctx, B, orc, cfg0):
 
 
 @pytest.mark.parametrize("variant", [1, 2, 4])
-def test_cfg0_xi_kernel_variants(B, orc, cfg0, variant, monkeypatch):
-    monkeypatch.setenv("LYA_XI_VARIANT", str(variant))
+def test_cfg0_xi_kernel_variants(B, orc, cfg0, variant):
     c = B.Context("cuda:0")
+    c.lya_set_option("force_generic", 1)
+    c.lya_set_option("generic_diagonals", variant)
     d = B.DeviceForests(cfg0)
     pq = orc.pairs_brute(cfg0)
     check_xi(c.lya_xi2pcf(d, B.binning(), c.lya_pairs_import(pq)), orc.xi(cfg0, pq), f"variant {variant}")
@@ -207,7 +208,7 @@ def test_long_and_ragged_forests_tiles(ctx, B, orc):
     check_dmat(g, orc.dmat(f2, ref2, 0.97, 9), "long forests D")
 
 
-def test_kernel_routes_fast_and_generic(B, orc, monkeypatch):
+def test_kernel_routes_fast_and_generic(B, orc):
     """The same catalogue through (a) the fast kernels (bucketed list, warp-private tables), (b) the
     generic kernels forced for the whole list, (c) a grid whose 8 Mpc/h r_par bins exceed the pixel
     spacing, so that the bucketing pass itself routes every pair to the generic kernels, and (d) a grid
@@ -219,10 +220,9 @@ def test_kernel_routes_fast_and_generic(B, orc, monkeypatch):
     seed = gen.mask_seed(4)
     ox, od = orc.xi(f, pq), orc.dmat(f, pq_d, 0.9, seed)
     res = {}
-    for variant in ("0", "9"):
-        monkeypatch.setenv("LYA_XI_VARIANT", variant)
-        monkeypatch.setenv("LYA_DMAT_VARIANT", variant)
+    for variant in ("0", "9"):                                # "9": LYA_OPT_FORCE_GENERIC
         c = B.Context("cuda:0")
+        c.lya_set_option("force_generic", 1 if variant == "9" else 0)
         d = B.DeviceForests(f)
         gx = c.lya_xi2pcf(d, B.binning(), c.lya_pairs_import(pq))
         gd = c.lya_dmat(d, B.binning(), c.lya_pairs_import(pq_d), 0.9, seed)
@@ -232,7 +232,8 @@ def test_kernel_routes_fast_and_generic(B, orc, monkeypatch):
         c.close()
     assert np.array_equal(res["0"][0], res["9"][0]) and res["0"][1:3] == res["9"][1:3]
     assert res["0"][3] > 0 and res["9"][3] == 0            # scatter-adds are counted by the fast kernel only
-    monkeypatch.delenv("LYA_XI_VARIANT"); monkeypatch.delenv("LYA_DMAT_VARIANT")
+    with pytest.raises(B.LyaError):
+        c.lya_set_option("generic_diagonals", 3)
     c = B.Context("cuda:0")
     d = B.DeviceForests(f)
     for (rp, rt, n_par, n_perp) in ((200.0, 200.0, 25, 25), (200.0, 200.0, 64, 50)):
