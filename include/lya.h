@@ -183,6 +183,17 @@ lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                     const lya_pairs *pairs, double reject_fraction, uint64_t seed,
                     double *D, double *Dn, double *Wd, lya_stats *stats);
 
+/* ---- final divisions on already-summed numerators (multi-GPU) ----------- */
+/* Every output above is an additive accumulator before its final division, so a catalogue's
+ * forest-pair list can be split over ranks ("distribute the work load"): each rank runs
+ * lya_xi2pcf / lya_dmat on its chunk asking for S, W, N / Dn, Wd, the numerators are summed across
+ * ranks (one all-reduce), and these two calls then take the divisions of eq. 2.4 and eq. 2.6.
+ * lya_xi_normalise:   xi[k] = S[k] / W[k] (0 where W[k] == 0), k < n  (n <= 2^30; D may alias nothing).
+ * lya_dmat_normalise: D[A][B] = Dn[A][B] / Wd[A] (row 0 where Wd[A] == 0); D may alias Dn.
+ * Device pointers; enqueued on the ctx stream, no synchronisation. */
+lya_status lya_xi_normalise(lya_ctx *ctx, int64_t n, const double *S, const double *W, double *xi);
+lya_status lya_dmat_normalise(lya_ctx *ctx, const lya_binning *b, const double *Dn, const double *Wd, double *D);
+
 /* ---- end-to-end convenience with HOST buffers ------------------------------------- */
 /* Uploads a HOST catalogue (every pointer in *f_host is a host pointer; ux/uy/uz
  * required), runs lya_neighbours, then lya_xi2pcf when do_xi and lya_dmat when

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "liblya.so")
 
 EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_set_option", "lya_neighbours",
            "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
-           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host"]
+           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host", "lya_xi_normalise", "lya_dmat_normalise"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
           4: "LYA_ERR_CAPACITY", 5: "LYA_ERR_OOM", 6: "LYA_ERR_CUDA", 7: "LYA_ERR_UNIMPLEMENTED"}
@@ -83,6 +83,8 @@ def load():
         lib.lya_run_host.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_int, C.c_int,
                                      C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.POINTER(C.c_int64), C.POINTER(CStats), C.POINTER(CStats)]
+        lib.lya_xi_normalise.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.lya_dmat_normalise.argtypes = [C.c_void_p, C.POINTER(CBinning), C.c_void_p, C.c_void_p, C.c_void_p]
         lib.lya_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         _lib = lib
     return _lib
@@ -238,10 +240,10 @@ class Context:
 
     # ---- lya_dmat ----
     def lya_dmat(self, forests: DeviceForests, b: CBinning, pairs: Pairs, reject_fraction: float, seed: int,
-                 want_Dn=True):
+                 want_Dn=True, want_D=True):
         torch = self.torch
         nb = b.n_par * b.n_perp
-        D = torch.empty((nb, nb), dtype=torch.float64, device=self.device)
+        D = torch.empty((nb, nb), dtype=torch.float64, device=self.device) if want_D else None
         Dn = torch.empty((nb, nb), dtype=torch.float64, device=self.device) if want_Dn else None
         Wd = torch.empty(nb, dtype=torch.float64, device=self.device)
         stats = CStats()
@@ -278,6 +280,16 @@ class Context:
         out["stats_xi"] = sx.as_dict()
         out["stats_dmat"] = sd.as_dict()
         return out
+
+    def lya_xi_normalise(self, S, W):
+        xi = self.torch.empty_like(S)
+        self._check(load().lya_xi_normalise(self.h, S.numel(), _ptr(S), _ptr(W), _ptr(xi)))
+        return xi
+
+    def lya_dmat_normalise(self, b: CBinning, Dn, Wd):
+        D = self.torch.empty_like(Dn)
+        self._check(load().lya_dmat_normalise(self.h, C.byref(b), _ptr(Dn), _ptr(Wd), _ptr(D)))
+        return D
 
     def lya_set_option(self, opt: str, value: int):
         self._check(load().lya_set_option(self.h, OPTIONS[opt], int(value)))

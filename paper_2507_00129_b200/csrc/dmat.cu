@@ -798,6 +798,15 @@ __global__ void k_dmat_normalise(const double *Dn_t, const double *Wd_t, BinPara
     if (Wd && B == 0) Wd[A] = wd;
 }
 
+// API-order version for already-summed numerators: D[A][B] = Dn[A][B] / Wd[A] (row 0 where Wd[A] == 0)
+__global__ void k_dmat_divide(const double *Dn, const double *Wd, int nb, double *D)
+{
+    const int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (idx >= (int64_t)nb * nb) return;
+    const double wd = Wd[idx / nb];
+    D[idx] = (wd != 0.0) ? Dn[idx] / wd : 0.0;
+}
+
 }  // namespace
 
 namespace {
@@ -995,5 +1004,18 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         cudaEventElapsedTime(&stats->ms_main, ctx->ev[0], ctx->ev[1]);
         cudaEventElapsedTime(&stats->ms_total, ctx->ev[3], ctx->ev[2]);
     }
+    return LYA_OK;
+}
+
+extern "C" lya_status lya_dmat_normalise(lya_ctx *ctx, const lya_binning *b, const double *Dn, const double *Wd, double *D)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    lya_status st = lya_check_binning(ctx, b);
+    if (st) return st;
+    if (!Dn || !Wd || !D) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat_normalise: NULL argument");
+    LYA_CUDA(cudaSetDevice(ctx->device));
+    const int nb = b->n_par * b->n_perp;
+    k_dmat_divide<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, ctx->stream>>>(Dn, Wd, nb, D);
+    LYA_CUDA(cudaGetLastError());
     return LYA_OK;
 }

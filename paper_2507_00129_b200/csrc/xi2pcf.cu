@@ -767,3 +767,17 @@ extern "C" lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const l
     if (!region) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_sub: region is NULL");
     return xi_run(ctx, f, b, pairs, region, n_region, S, W, N, NULL, stats);
 }
+
+// xi_A = S_A / W_A (0 where W_A == 0) from already-summed numerators (section 8(e): after the all-reduce).
+extern "C" lya_status lya_xi_normalise(lya_ctx *ctx, int64_t n, const double *S, const double *W, double *xi)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (n < 0 || (n > 0 && (!S || !W || !xi))) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi_normalise: bad arguments");
+    if (n > ((int64_t)1 << 30)) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_xi_normalise: n above 2^30");
+    LYA_CUDA(cudaSetDevice(ctx->device));
+    if (n > 0) {
+        k_xi_finalize<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(S, W, NULL, (int)n, NULL, NULL, NULL, xi);
+        LYA_CUDA(cudaGetLastError());
+    }
+    return LYA_OK;
+}

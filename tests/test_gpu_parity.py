@@ -258,6 +258,29 @@ def test_forest_pair_subsampling_next2(ctx, B, orc):
     assert ctx.lya_pairs_subsample(pairs, 1.0, 3).n == 0 and ctx.lya_pairs_subsample(pairs, 0.0, 3).n == pairs.n
 
 
+def test_mask_known_answer_vectors_gpu(ctx, B):
+    """The CUDA keep mask against the big-integer vectors of tests/golden/mask_vectors.txt (the
+    specification of DESIGN.md section 2.1, written by a script that imports nothing from the repo),
+    through lya_pairs_subsample (forest indices as ids), one call per (seed, fraction) group."""
+    import os
+    from collections import defaultdict
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "mask_vectors.txt")
+    groups = defaultdict(list)
+    for l in open(path):
+        if l.strip() and not l.startswith("#"):
+            r = l.split()
+            if int(r[1]) < 2 ** 31 and int(r[2]) < 2 ** 31:
+                groups[(int(r[0]), r[3])].append((int(r[1]), int(r[2]), int(r[6])))
+    n_checked = 0
+    for (seed, f), rows in groups.items():
+        pq = np.array([[a, b] for a, b, _ in rows], dtype=np.int32)
+        sub = ctx.lya_pairs_subsample(ctx.lya_pairs_import(pq), float(f), seed)
+        want = np.array([[min(a, b), max(a, b)] for a, b, k in rows if k], dtype=np.int32).reshape(-1, 2)
+        assert sub.n == len(want) and np.array_equal(sub.export().cpu().numpy(), want), (seed, f)
+        n_checked += len(rows)
+    assert n_checked > 600
+
+
 def test_region_subsamples_next1(ctx, B, orc):
     """lya_xi2pcf_sub against the oracle region by region: fast kernel (bucketed list) and, with a grid
     whose bins exceed the pixel spacing, the direct kernel; the regions add up to lya_xi2pcf."""
@@ -283,6 +306,45 @@ def test_region_subsamples_next1(ctx, B, orc):
         assert g["stats"]["n_binned"] == full["stats"]["n_binned"]
     with pytest.raises(B.LyaError):
         ctx.lya_xi2pcf_sub(d, B.binning(), pairs, region + 3, n_region)
+
+
+def test_sharded_halves_sum_to_full(ctx, B, orc):
+    """SURVEY 8(e) on one device: the two chunks of shard.split_pairs, run separately and summed,
+    equal the un-split run (N, n_kept exactly) and, after lya_xi_normalise / lya_dmat_normalise,
+    the oracle on the full list."""
+    import torch
+    from paper_2507_00129_b200 import shard
+    f = gen.make_config(4, n_forest=500, density_scale=2.0)
+    d = B.DeviceForests(f)
+    b = B.binning()
+    seed = gen.mask_seed(4)
+    pairs = ctx.lya_neighbours(d, b)
+    pq = pairs.export()
+    lens = d.pix_off[1:] - d.pix_off[:-1]
+    full_x = ctx.lya_xi2pcf(d, b, pairs)
+    acc = None
+    n_chunk = []
+    for r in range(2):
+        mine = shard.split_pairs(pq, lens, r, 2).contiguous()
+        n_chunk.append(len(mine))
+        pr = ctx.lya_pairs_import(mine)
+        x = ctx.lya_xi2pcf(d, b, pr)
+        dm = ctx.lya_dmat(d, b, pr, 0.9, seed, want_Dn=True, want_D=False)
+        assert dm["D"] is None
+        part = [x["S"], x["W"], x["N"], dm["Dn"], dm["Wd"], dm["stats"]["n_kept"]]
+        acc = part if acc is None else [a + p for a, p in zip(acc, part)]
+    assert sum(n_chunk) == pairs.n and min(n_chunk) > 0
+    assert torch.equal(acc[2], full_x["N"])
+    ref = orc.pairs_window(f)
+    ox, od = orc.xi(f, ref), orc.dmat(f, ref, 0.9, seed)
+    g = dict(S=acc[0], W=acc[1], N=acc[2], xi=ctx.lya_xi_normalise(acc[0], acc[1]), stats=full_x["stats"])
+    check_xi(g, ox, "two chunks summed")
+    gd = dict(D=ctx.lya_dmat_normalise(b, acc[3], acc[4]), Dn=acc[3], Wd=acc[4], stats=dict(n_kept=acc[5]))
+    check_dmat(gd, od, "two chunks summed D")
+    # the sharded step itself (world = 1: no group needed) equals the same oracle
+    st = shard.sharded_step(ctx, d, b, 0.9, seed, 0, 1)
+    check_xi(dict(S=st["S"], W=st["W"], N=st["N"], xi=st["xi"], stats=st["stats_xi"]), ox, "sharded_step")
+    check_dmat(dict(D=st["D"], Dn=st["Dn"], Wd=st["Wd"], stats=st["stats_dmat"]), od, "sharded_step D")
 
 
 # ------------------------------------------------------------------ invariances and edge cases

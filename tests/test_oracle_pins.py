@@ -346,6 +346,23 @@ def test_PD7_mask_statistics_and_symmetry():
     assert abs((k6 == k5[:100, :100]).mean() - 0.5) < 0.03
 
 
+def _mask_vectors():
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "mask_vectors.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    return [(int(r[0]), int(r[1]), int(r[2]), float(r[3]), int(r[4]), int(r[5]), int(r[6])) for r in rows]
+
+
+def test_PD7_mask_known_answer_vectors():
+    """DESIGN.md section 2.1 restated in Python big integers by tests/golden/make_mask_vectors.py
+    (imports nothing from the repo): threshold and keep decision of every vector."""
+    rows = _mask_vectors()
+    assert len(rows) > 600 and 50 < sum(r[6] for r in rows) < len(rows) - 50
+    for seed, a, b, f, thr, _, kp in rows:
+        assert orc.mask_threshold(f) == thr
+        assert int(orc.keep(seed, a, b, thr)) == kp, (seed, a, b, f)
+
+
 def test_PD7_kept_fraction_in_dmat(cfg0):
     pq = orc.pairs_brute(cfg0)
     x = orc.xi(cfg0, pq)
