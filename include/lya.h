@@ -109,8 +109,12 @@ const char *lya_version(void);
  *                             (N, n_kept exactly; sums to rounding); tests use it to cover both routes.
  *   LYA_OPT_GENERIC_DIAGONALS 1, 2 (default) or 4: diagonals of the pixel-pair matrix per lane in the
  *                             generic xi kernel (a tuning knob; results do not depend on it).
+ *   LYA_OPT_CHECK_HOLDERS     0 (default) / 1: run the debug variant of the fast kernels, which checks at every
+ *                             row step that no two lanes of a warp hold the same table entry (the invariant
+ *                             their atomic-free accumulation rests on).  Much slower; a
+ *                             violation makes the call return LYA_ERR_CUDA with the count in lya_last_error.
  * LYA_ERR_INVALID_ARG for an unknown option or value. */
-typedef enum { LYA_OPT_FORCE_GENERIC = 0, LYA_OPT_GENERIC_DIAGONALS = 1 } lya_option;
+typedef enum { LYA_OPT_FORCE_GENERIC = 0, LYA_OPT_GENERIC_DIAGONALS = 1, LYA_OPT_CHECK_HOLDERS = 2 } lya_option;
 lya_status  lya_set_option(lya_ctx *ctx, lya_option opt, int64_t value);
 
 /* ---- stage 1: neighbour search (north_star stage 1) ------------ */

@@ -27,7 +27,7 @@
 //                drain per tile pair (pass 1b), T2/T3 read the whole forests from global memory.
 // lya_pairs_subsample (forest-pair subsampling) lives here too: it shares the mask.
 #include <stdlib.h>
-#include "lya_internal.cuh"
+#include "lya_walk.cuh"
 
 namespace {
 
@@ -38,29 +38,6 @@ constexpr int DQPAD = 4;
 constexpr int H_SLOTS = 512;             // local (b_par, column) slots per H table
 constexpr int KEPT_CAP = 256;
 constexpr int DCHUNK = 8;
-
-// ---- stage 4: the keep mask (integer only) -------------------------
-__device__ __forceinline__ unsigned long long mix64(unsigned long long z)
-{
-    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
-    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
-    return z ^ (z >> 31);
-}
-__device__ __forceinline__ unsigned long long key_lo(unsigned long long seed, unsigned long long id)
-{
-    return mix64(seed + id * 0x9E3779B97F4A7C15ULL);
-}
-__device__ __forceinline__ unsigned long long key_hi(unsigned long long seed, unsigned long long id)
-{
-    return mix64((seed ^ 0xD1B54A32D192ED03ULL) + id * 0x9E3779B97F4A7C15ULL);
-}
-__device__ __forceinline__ bool keep_pair(unsigned long long klo, unsigned long long khi, unsigned long long thr)
-{
-    unsigned long long x = klo + khi;
-    x ^= x >> 32;
-    x *= 0xD6E8FEB86659FD93ULL;
-    return (x >> 32) >= thr;
-}
 
 struct DmParams {
     const int64_t *pix_off;
@@ -213,7 +190,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
                     ws.pc[t] = P.chi[op + ip0 + t];
                     ws.pw[t] = P.w[op + ip0 + t];
                     ws.pu[t] = P.loglam[op + ip0 + t] - lbp;
-                    ws.pk[t] = key_lo(P.seed, (unsigned long long)(op + ip0 + t));
+                    ws.pk[t] = lya_key_lo(P.seed, (unsigned long long)(op + ip0 + t));
                 }
                 cur_p = p; cur_ip0 = ip0;
                 __syncwarp();
@@ -226,7 +203,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
                     ws.qc[t] = in ? P.chi[oq + jq0 + j] : LYA_CHI_SENTINEL;
                     ws.qw[t] = in ? P.w[oq + jq0 + j] : 0.0;
                     ws.qu[t] = in ? P.loglam[oq + jq0 + j] - lbq : 0.0;
-                    if (in) ws.qk[j] = key_hi(P.seed, (unsigned long long)(oq + jq0 + j));
+                    if (in) ws.qk[j] = lya_key_hi(P.seed, (unsigned long long)(oq + jq0 + j));
                 }
                 __syncwarp();
             };
@@ -305,7 +282,7 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
                                 const int j = j0 + lane;
                                 int bin = -1;
                                 if (j < mq) bin = lya_pix_bin<POW2>(bp, g, pci, qc[j]);
-                                bool kp = (bin >= 0) && keep_pair(ki, ws.qk[min(j, mq - 1)], P.thr);
+                                bool kp = (bin >= 0) && lya_keep_pair(ki, ws.qk[min(j, mq - 1)], P.thr);
                                 if (first_chunk) {
                                     binned += (bin >= 0);
                                     kept_total += kp;
@@ -345,443 +322,6 @@ __global__ void __launch_bounds__(DM_THREADS) k_dmat(DmParams P)
     }
 }
 
-// ======================= fast kernel ======================================
-// One warp per forest pair of the bucket-sorted list, forests staged from the padded catalogue.
-//  pass A  diagonal walk (the xi kernel's traversal): the four H tables of the pair, each lane
-//          holding the table entry of its current run in registers (predicated release/acquire, no
-//          atomics: the walk is done once per side of chi_i = chi_j, so entries have one holder);
-//          every in-grid pair is hashed on the fly (stage 4) and the kept ones are queued;
-//  pass B  the non-zero table entries are compacted into a list;
-//  pass C  the kept pairs are drained: T1..T3 per kept pair, T4 with lanes over the table entries and
-//          an inner loop over the kept pairs (the entry stays in registers); every update is one
-//          red.global.add.f64 into the L2-resident Dn.
-constexpr int FD_WARPS = 15;                 // one CTA per SM (shared memory: 15.1 KB per warp)
-constexpr int FD_THREADS = FD_WARPS * 32;
-constexpr int FD_T = LYA_FAST_TILE;
-constexpr int FD_ROWS = 16;
-constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
-constexpr int FD_PAD = 2;
-constexpr int FD_SLOTS = 306;                // (n_par + 1) * LYA_NCOL <= FD_SLOTS
-constexpr int FD_KCAP = 48;                  // kept pairs queued per forest pair
-constexpr int FD_KBATCH = 24;                // kept pairs drained together (coefficient tables)
-constexpr int FD_CHUNK = 8;
-
-struct DmFastParams {
-    LyaPrep prep;
-    const int32_t *pq;
-    int64_t n_pairs;
-    BinParams bp;
-    unsigned long long seed, thr;
-    double *Dn, *Wd;
-    unsigned long long *counters;   // [4] next chunk, [2] evaluated, [3] error, [5] kept, [6] binned, [7] scatter-adds
-};
-
-struct DmKeysA { unsigned long long pk[FD_T], qk[FD_T]; };                 // pass A: stage-4 keys of the pixels
-struct DmDrainBC {                                                            // passes B and C
-    double2 kc01[FD_KBATCH], kc23[FD_KBATCH];    // per kept pair of a batch: om (1, u_j), om (u_i, u_i u_j)
-    unsigned short nz[FD_SLOTS];                 // non-zero slots
-};
-struct __align__(16) DmFastWarp {
-    double2 H01[FD_SLOTS], H23[FD_SLOTS];    // (H_aa, H_ag), (H_ga, H_gg) per slot = col_rel * (n_par + 1) + row
-    double pc[FD_TP], pea[FD_TP], peg[FD_TP];            // (w and u of the kept pairs are read from HBM/L2 in the drain)
-    double qc[FD_T + 2 * FD_PAD], qea[FD_T + 2 * FD_PAD], qeg[FD_T + 2 * FD_PAD];
-    union { DmKeysA a; DmDrainBC b; } u;     // the keys are dead once pass A is done (shared memory buys occupancy)
-    unsigned kept[FD_KCAP];                  // (i << 20) | (j << 12) | A
-    unsigned char jlo[FD_T], jx[FD_T], jhi[FD_T];
-    unsigned nkept, pad_[3];
-};
-
-__device__ __forceinline__ void dsts_v2_if(bool p, unsigned addr, double x, double y)
-{
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q st.shared.v2.f64 [%1], {%2, %3};\n}"
-                 :: "r"((unsigned)p), "r"(addr), "d"(x), "d"(y) : "memory");
-}
-__device__ __forceinline__ void dlds_v2_if(bool p, unsigned addr, double &x, double &y)
-{
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %2, 0;\n @q ld.shared.v2.f64 {%0, %1}, [%3];\n}"
-                 : "+d"(x), "+d"(y) : "r"((unsigned)p), "r"(addr) : "memory");
-}
-
-// byte offset (16 * slot) of a pixel pair in the H tables and whether it is a pair of THIS walk
-// (inside the grid and on the walk's side of chi_i = chi_j: sgn = 0 for chi_i >= chi_j, -1 otherwise);
-// A = its bin.  Pairs outside get the garbage row / column.
-template <bool POW2>
-__device__ __forceinline__ unsigned dm_key(const BinParams &bp, const PairBin &g, double chi_i, double chi_j, unsigned c0,
-                                           unsigned np1, int sgn, bool &valid, unsigned &A)
-{
-    const double d = __dsub_rn(chi_i, chi_j);
-    const double t = __dadd_rn(chi_i, chi_j);
-    unsigned bx, by;
-    if (POW2) {
-        bx = lya_floor_u32(__dmul_rn(fabs(d), g.cx));
-        by = lya_floor_u32(__dmul_rn(t, g.sy));
-    } else {
-        const double rpar = __dmul_rn(fabs(d), g.c), rperp = __dmul_rn(t, g.s);
-        bx = (rpar < bp.rpar_max) ? min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1)) : (unsigned)bp.n_par;
-        by = (rperp < bp.rperp_max) ? min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1)) : 0x7fffffffu;
-    }
-    const bool side = ((__double2hiint(d) ^ sgn) >= 0);
-    valid = side & (bx < (unsigned)bp.n_par) & (by < (unsigned)bp.n_perp);
-    A = by * (unsigned)bp.n_par + bx;                   // transposed bin order (see lya_pix_bin_t)
-    bx = valid ? bx : np1 - 1u;                          // everything else -> the garbage entry (0, n_par)
-    const unsigned col = valid ? by - c0 : 0u;
-    return (col * np1 + bx) * 16u;
-}
-
-// stage-4 keep mask on precomputed pixel keys (same integer function as keep_pair above)
-__device__ __forceinline__ bool dm_keep(unsigned long long klo, unsigned long long khi, unsigned long long thr)
-{
-    return keep_pair(klo, khi, thr);
-}
-
-// pass A over rows [r0, r1] (a multiple of D rows; rows >= len are sentinels) and diagonals [dlo, dhi].
-// Same scheme as k_xi_fast: a lane holds the H entry of its current run in registers (predicated
-// release / acquire around a warp barrier); the keys, mask and queueing of row i+1 are computed
-// between the acquire of row i and the FMAs that need it.
-template <int D, bool POW2>
-__device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, unsigned h23, int r0, int r1, int mq, int dlo, int dhi,
-                                        int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned np1,
-                                        unsigned long long thr, int lane, unsigned &binned, unsigned &kept_n,
-                                        unsigned long long &evaluated)
-{
-    const double *qc = ws.qc + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
-    const unsigned garbage = (np1 - 1u) * 16u;
-    for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
-        const int dl = d0 + lane * D;
-        unsigned cur[D], key[D];
-        double h0[D], h1[D], h2[D], h3[D], fa[D], fg[D];
-        double wc[D], wa[D], wg[D];                         // sliding window over q: chi, ea, eg
-        double pa_c, pg_c;
-#pragma unroll
-        for (int k = 0; k < D; ++k) { cur[k] = garbage; h0[k] = 0.0; h1[k] = 0.0; h2[k] = 0.0; h3[k] = 0.0; }
-        // keys, mask and queueing of one row (i, window slot of diagonal k = (k + u) % D)
-        auto row_keys = [&](int i, int u, bool live, unsigned *key_o, double *fa_o, double *fg_o) {
-            const double pci = ws.pc[i];
-            const unsigned long long pki = ws.u.a.pk[min(i, FD_T - 1)];
-#pragma unroll
-            for (int k = 0; k < D; ++k) {
-                const int sl = (k + u) % D;
-                bool valid; unsigned A;
-                key_o[k] = dm_key<POW2>(bp, g, pci, wc[sl], c0, np1, sgn, valid, A);
-                fa_o[k] = wa[sl]; fg_o[k] = wg[sl];
-                valid = valid && live;
-                const int j = i + dl + k;
-                const bool kp = valid && keep_pair(pki, ws.u.a.qk[min(max(j, 0), FD_T - 1)], thr);
-                binned += valid ? 1u : 0u;
-                if (kp) {                                    // ~1 % of the pairs at f = 0.99
-                    const unsigned idx = atomicAdd(&ws.nkept, 1u);
-                    if (idx < FD_KCAP) ws.kept[idx] = ((unsigned)i << 20) | ((unsigned)j << 12) | A;
-                    kept_n += 1u;
-                }
-            }
-        };
-#pragma unroll
-        for (int k = 0; k < D; ++k) {
-            const int j = min(max(r0 + dl + k, -FD_PAD), mq + FD_PAD - 1);
-            wc[k] = qc[j]; wa[k] = qea[j]; wg[k] = qeg[j];
-        }
-        row_keys(r0, 0, true, key, fa, fg);
-        pa_c = ws.pea[r0]; pg_c = ws.peg[r0];
-        evaluated += (unsigned long long)(r1 - r0 + 1) * D;
-        for (int ib = r0; ib <= r1; ib += D) {
-#pragma unroll
-            for (int u = 0; u < D; ++u) {
-                const int i = ib + u;
-                bool ch[D];
-#pragma unroll
-                for (int k = 0; k < D; ++k) {
-                    ch[k] = key[k] != cur[k];
-                    dsts_v2_if(ch[k], h01 + cur[k], h0[k], h1[k]);                      // release
-                    dsts_v2_if(ch[k], h23 + cur[k], h2[k], h3[k]);
-                }
-                __syncwarp();
-#pragma unroll
-                for (int k = 0; k < D; ++k) {
-                    dlds_v2_if(ch[k], h01 + key[k], h0[k], h1[k]);                      // acquire
-                    dlds_v2_if(ch[k], h23 + key[k], h2[k], h3[k]);
-                    cur[k] = key[k];
-                }
-                // row i + 1: its new q pixel replaces q[i + dl] in window slot u
-                unsigned key_n[D];
-                double fa_n[D], fg_n[D];
-                {
-                    const int j = min(max(i + dl + D, -FD_PAD), mq + FD_PAD - 1);
-                    wc[u] = qc[j]; wa[u] = qea[j]; wg[u] = qeg[j];
-                    row_keys(i + 1, u + 1, i + 1 <= r1, key_n, fa_n, fg_n);
-                }
-#pragma unroll
-                for (int k = 0; k < D; ++k) {
-                    h0[k] = fma(pa_c, fa[k], h0[k]); h1[k] = fma(pa_c, fg[k], h1[k]);
-                    h2[k] = fma(pg_c, fa[k], h2[k]); h3[k] = fma(pg_c, fg[k], h3[k]);
-                    fa[k] = fa_n[k]; fg[k] = fg_n[k]; key[k] = key_n[k];
-                }
-                pa_c = ws.pea[i + 1]; pg_c = ws.peg[i + 1];
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < D; ++k) {
-            dsts_v2_if(true, h01 + cur[k], h0[k], h1[k]);
-            dsts_v2_if(true, h23 + cur[k], h2[k], h3[k]);
-        }
-        __syncwarp();
-    }
-}
-
-template <bool POW2>
-__device__ __forceinline__ void dm_walk_any(DmFastWarp &ws, unsigned h01, unsigned h23, int r0, int r1, int mq, int dlo, int dhi,
-                                            int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned np1,
-                                            unsigned long long thr, int lane, unsigned &binned, unsigned &kept_n,
-                                            unsigned long long &evaluated)
-{
-    if (dhi < dlo) return;
-    const int nd = dhi - dlo + 1;
-    if (nd <= 32) dm_walk<1, POW2>(ws, h01, h23, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, np1, thr, lane, binned, kept_n, evaluated);
-    else dm_walk<2, POW2>(ws, h01, h23, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, np1, thr, lane, binned, kept_n, evaluated);
-}
-
-// pass C: drain n queued kept pairs.
-template <bool POW2>
-__device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, const unsigned *kept, int n, int nnz, int mp, int mq, const DmFastParams &P,
-                                         const PairBin &g, int c0, long long offp, long long offq, int lane,
-                                         unsigned long long &n_red)
-{
-    const BinParams &bp = P.bp;
-    const int nb = bp.n_par * bp.n_perp, np1 = bp.n_par + 1;
-    const double *qc = ws.qc + FD_PAD, *qea = ws.qea + FD_PAD, *qeg = ws.qeg + FD_PAD;
-    // coefficients of every kept pair (lanes over kept pairs) and T1: Dn[A][A] += om, Wd[A] += om
-    for (int e = lane; e < n; e += 32) {
-        const unsigned rec = kept[e];
-        const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
-        const double om = P.prep.w[offp + i] * P.prep.w[offq + j], ui = P.prep.u[offp + i], uj = P.prep.u[offq + j];
-        const double omi = om * ui;
-        ws.u.b.kc01[e] = make_double2(om, om * uj);
-        ws.u.b.kc23[e] = make_double2(omi, omi * uj);
-        atomicAdd(P.Dn + (size_t)A * nb + A, om);
-        atomicAdd(P.Wd + A, om);
-        n_red += 2;
-    }
-    __syncwarp();
-    // T2: -(om ea_j' + om u_j eg_j') over row i's window;  T3: -(om ea_i' + om u_i eg_i') over p
-    for (int e = 0; e < n; ++e) {
-        const unsigned rec = kept[e];
-        const int i = rec >> 20, j = (rec >> 12) & 0xff, A = rec & 0xfff;
-        const double2 c01 = ws.u.b.kc01[e], c23 = ws.u.b.kc23[e], geo = make_double2(ws.pc[i], qc[j]);
-        double *row = P.Dn + (size_t)A * nb;
-        for (int j2 = ws.jlo[i] + lane; j2 < ws.jhi[i]; j2 += 32) {
-            const int B = lya_pix_bin_t<POW2>(bp, g, geo.x, qc[j2]);
-            if (B >= 0) { atomicAdd(row + B, -fma(c01.y, qeg[j2], c01.x * qea[j2])); n_red += 1; }
-        }
-        for (int i2 = lane; i2 < mp; i2 += 32) {
-            const int B = lya_pix_bin_t<POW2>(bp, g, ws.pc[i2], geo.y);
-            if (B >= 0) { atomicAdd(row + B, -fma(c23.x, ws.peg[i2], c01.x * ws.pea[i2])); n_red += 1; }
-        }
-    }
-    // T4: lanes over the non-zero table entries, inner loop over the kept pairs
-    for (int t = lane; t < nnz; t += 32) {
-        const int slot = ws.u.b.nz[t];
-        const int cr = slot / np1, bx = slot - cr * np1;
-        double *colB = P.Dn + ((c0 + cr) * bp.n_par + bx);
-        const double2 a = ws.H01[slot], b = ws.H23[slot];
-#pragma unroll 2
-        for (int e = 0; e < n; ++e) {
-            const int A = kept[e] & 0xfff;
-            const double2 c01 = ws.u.b.kc01[e], c23 = ws.u.b.kc23[e];
-            const double v = fma(c23.y, b.y, fma(c23.x, b.x, fma(c01.y, a.y, c01.x * a.x)));
-            atomicAdd(colB + (size_t)A * nb, v);
-        }
-        n_red += (unsigned long long)n;
-    }
-}
-
-template <bool POW2>
-__device__ __forceinline__ void dm_drain(DmFastWarp &ws, int n, int nnz, int mp, int mq, const DmFastParams &P,
-                                         const PairBin &g, int c0, long long offp, long long offq, int lane,
-                                         unsigned long long &n_red)
-{
-    for (int e0 = 0; e0 < n; e0 += FD_KBATCH) {
-        dm_drain_batch<POW2>(ws, ws.kept + e0, min(FD_KBATCH, n - e0), nnz, mp, mq, P, g, c0, offp, offq, lane, n_red);
-        __syncwarp();
-    }
-}
-
-template <bool POW2>
-__global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    DmFastWarp &ws = ((DmFastWarp *)smem_raw)[wid];
-    const BinParams bp = P.bp;
-    const unsigned np1 = (unsigned)bp.n_par + 1u;
-    const int n_slots = (int)np1 * LYA_NCOL;
-    for (int t = lane; t < FD_SLOTS; t += 32) { ws.H01[t] = make_double2(0.0, 0.0); ws.H23[t] = make_double2(0.0, 0.0); }
-    if (lane < FD_PAD) { ws.qc[lane] = LYA_CHI_SENTINEL; ws.qea[lane] = 0.0; ws.qeg[lane] = 0.0; }
-    if (lane == 0) ws.nkept = 0u;
-    __syncwarp();
-    const double *qc = ws.qc + FD_PAD;
-    const unsigned h01 = (unsigned)__cvta_generic_to_shared(ws.H01), h23 = (unsigned)__cvta_generic_to_shared(ws.H23);
-    unsigned long long evaluated = 0, kept_total = 0, binned_total = 0, n_red = 0;
-    int cur_p = -1, head_p = -1;
-    ForestHead hp;
-    hp.len = 0;
-    const int64_t n_chunks = (P.n_pairs + FD_CHUNK - 1) / FD_CHUNK;
-    for (;;) {
-        unsigned long long chunk = 0;
-        if (lane == 0) chunk = atomicAdd(&P.counters[4], 1ull);
-        chunk = __shfl_sync(0xffffffffu, chunk, 0);
-        if ((int64_t)chunk >= n_chunks) break;
-        const int64_t k0 = (int64_t)chunk * FD_CHUNK, k1 = min(k0 + FD_CHUNK, P.n_pairs);
-        for (int64_t k = k0; k < k1; ++k) {
-            const int2 e = ((const int2 *)P.pq)[k];
-            const int p = e.x, q = e.y;
-            if (p != head_p) { hp = P.prep.head[p]; head_p = p; }
-            const ForestHead hq = P.prep.head[q];
-            const int mp = hp.len, mq = hq.len;
-            if ((hp.flags | hq.flags) & 1) {
-                if (lane == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_DEGENERATE);
-                continue;
-            }
-            double s, c;
-            lya_pair_sc(hp.ux, hp.uy, hp.uz, hq.ux, hq.uy, hq.uz, s, c);
-            const PairBin g = lya_make_pairbin(bp, s, c);
-            int c0;
-            const int key = lya_pair_key<POW2>(bp, g, hp, hq, c0);
-            if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
-            __syncwarp();
-            if (p != cur_p) {
-                const double2 *s0 = (const double2 *)(P.prep.chi + hp.off), *s3 = (const double2 *)(P.prep.ea + hp.off),
-                              *s4 = (const double2 *)(P.prep.eg + hp.off);
-                for (int t = lane; 2 * t < mp; t += 32) {
-                    ((double2 *)ws.pc)[t] = s0[t]; ((double2 *)ws.pea)[t] = s3[t]; ((double2 *)ws.peg)[t] = s4[t];
-                }
-                __syncwarp();
-                for (int t = mp + lane; t < FD_TP; t += 32) {            // sentinel rows (!= q's sentinel: r_par never 0)
-                    ws.pc[t] = 2.0 * LYA_CHI_SENTINEL; ws.pea[t] = 0.0; ws.peg[t] = 0.0;
-                }
-                cur_p = p;
-            }
-            {
-                const double2 *s0 = (const double2 *)(P.prep.chi + hq.off), *s3 = (const double2 *)(P.prep.ea + hq.off),
-                              *s4 = (const double2 *)(P.prep.eg + hq.off);
-                const int npad2 = (mq + 1) >> 1;
-                for (int t = lane; t < npad2; t += 32) {
-                    ((double2 *)qc)[t] = s0[t]; ((double2 *)(ws.qea + FD_PAD))[t] = s3[t]; ((double2 *)(ws.qeg + FD_PAD))[t] = s4[t];
-                }
-                for (int t = lane; t < mq; t += 32) ws.u.a.qk[t] = key_hi(P.seed, (unsigned long long)(hq.pix0 + t));
-                // (the keys share their storage with the drain tables, so p's keys are rebuilt for every pair)
-                for (int t = lane; t < mp; t += 32) ws.u.a.pk[t] = key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
-                if (lane < FD_PAD) {
-                    const int j = FD_PAD + 2 * npad2 + lane;
-                    ws.qc[j] = LYA_CHI_SENTINEL; ws.qea[j] = 0.0; ws.qeg[j] = 0.0;
-                }
-            }
-            __syncwarp();
-            // per row of p: in-grid window [jlo, jhi) of q and the sign change jx (chi_i >= chi_j below it)
-            const double R = (c > 0.0) ? (bp.rpar_max / c) * (1.0 + 1e-12) + 1e-9 : 1e300;
-            const double Tchi = (s > 0.0) ? (bp.rperp_max / s) * (1.0 + 1e-12) + 1e-9 : 1e300;
-            for (int i = lane; i < mp; i += 32) {
-                const double x = ws.pc[i];
-                int lo = 0, hi = mq;
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x - R) hi = mid; else lo = mid + 1; }
-                const int jlo = lo;
-                const double top = fmin(x + R, Tchi - x);
-                hi = mq;
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] >= top) hi = mid; else lo = mid + 1; }
-                const int jhi = lo;
-                lo = jlo; hi = jhi;
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x) hi = mid; else lo = mid + 1; }
-                ws.jlo[i] = (unsigned char)jlo; ws.jhi[i] = (unsigned char)jhi; ws.jx[i] = (unsigned char)lo;
-            }
-            __syncwarp();
-            // ---- pass A ----
-            unsigned binned = 0, kept_n = 0;
-            for (int i0 = 0; i0 < mp; i0 += FD_ROWS) {
-                const int i = i0 + lane;
-                int plo = 1 << 20, phi = -(1 << 20), nlo = 1 << 20, nhi = -(1 << 20), r0 = 1 << 20, r1 = -1;
-                if (lane < FD_ROWS && i < mp) {
-                    const int jl = ws.jlo[i], jh = ws.jhi[i], jx = ws.jx[i];
-                    if (jx > jl) { plo = jl - i; phi = jx - 1 - i; }
-                    if (jh > jx) { nlo = jx - i; nhi = jh - 1 - i; }
-                    if (jh > jl) { r0 = i; r1 = i; }
-                }
-                plo = __reduce_min_sync(0xffffffffu, plo); phi = __reduce_max_sync(0xffffffffu, phi);
-                nlo = __reduce_min_sync(0xffffffffu, nlo); nhi = __reduce_max_sync(0xffffffffu, nhi);
-                r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
-                if (r1 < r0) continue;
-#pragma unroll 1
-                for (int sgn = 0; sgn >= -1; --sgn)         // one call site: chi_i >= chi_j, then chi_i < chi_j
-                    dm_walk_any<POW2>(ws, h01, h23, r0 & ~1, r1 | 1, mq, sgn ? nlo : plo, sgn ? nhi : phi, sgn, bp, g,
-                                      (unsigned)c0, np1, P.thr, lane, binned, kept_n, evaluated);
-            }
-            binned_total += binned; kept_total += kept_n;
-            __syncwarp();
-            // ---- pass B: compact the non-zero entries (H_aa > 0 wherever a pair with weight fell) ----
-            int nnz = 0;
-            for (int t0 = 0; t0 < n_slots; t0 += 32) {
-                const int t = t0 + lane;
-                bool nzf = false;
-                if (t < n_slots) {
-                    const int cr = t / (int)np1, bx = t - cr * (int)np1;
-                    const double2 a = ws.H01[t], b = ws.H23[t];
-                    nzf = (bx < bp.n_par) && (cr < LYA_NCOL) && (a.x != 0.0 || a.y != 0.0 || b.x != 0.0 || b.y != 0.0);
-                }
-                const unsigned bal = __ballot_sync(0xffffffffu, nzf);
-                if (nzf) ws.u.b.nz[nnz + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)t;
-                nnz += __popc(bal);
-            }
-            __syncwarp();
-            // ---- pass C (one drain call site: the kernel's code has to stay small for the instruction cache) ----
-            // Normally the queue holds every kept pair.  With more kept pairs than the queue holds (small
-            // reject fractions) the mask is redone row by row and the queue drained each time it fills.
-            const unsigned nk = ws.nkept;
-            const bool overflow = nk > FD_KCAP;
-            int n_q = overflow ? 0 : (int)nk;
-            int si = 0, sj = (overflow && mp > 0) ? (int)ws.jlo[0] : 0;
-            for (;;) {
-                bool done = true;
-                if (overflow) {
-                    while (si < mp) {
-                        const int jh = ws.jhi[si];
-                        if (sj >= jh) { ++si; sj = (si < mp) ? (int)ws.jlo[si] : 0; continue; }
-                        const int j = sj + lane;
-                        int A = -1;
-                        if (j < jh) A = lya_pix_bin_t<POW2>(bp, g, ws.pc[si], qc[j]);
-                        const bool kp = (A >= 0) && keep_pair(key_lo(P.seed, (unsigned long long)(hp.pix0 + si)),
-                                                              key_hi(P.seed, (unsigned long long)(hq.pix0 + j)), P.thr);   // (the staged keys are gone)
-                        const unsigned bal = __ballot_sync(0xffffffffu, kp);
-                        if (n_q + __popc(bal) > FD_KCAP) break;          // drain first, then redo these 32 pixels
-                        if (kp) ws.kept[n_q + __popc(bal & ((1u << lane) - 1u))] = ((unsigned)si << 20) | ((unsigned)j << 12) | (unsigned)A;
-                        n_q += __popc(bal);
-                        sj += 32;
-                    }
-                    done = si >= mp;
-                }
-                __syncwarp();
-                dm_drain<POW2>(ws, n_q, nnz, mp, mq, P, g, c0, hp.off, hq.off, lane, n_red);
-                __syncwarp();
-                if (done) break;
-                n_q = 0;
-            }
-            __syncwarp();
-            // clear the table and the queue for the next pair
-            for (int t = lane; t < n_slots; t += 32) { ws.H01[t] = make_double2(0.0, 0.0); ws.H23[t] = make_double2(0.0, 0.0); }
-            if (lane == 0) ws.nkept = 0u;
-        }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
-        kept_total += __shfl_xor_sync(0xffffffffu, kept_total, o);
-        binned_total += __shfl_xor_sync(0xffffffffu, binned_total, o);
-        n_red += __shfl_xor_sync(0xffffffffu, n_red, o);
-    }
-    if (lane == 0) {
-        atomicAdd(&P.counters[2], evaluated);
-        atomicAdd(&P.counters[5], kept_total);
-        atomicAdd(&P.counters[6], binned_total);
-        atomicAdd(&P.counters[7], n_red);
-    }
-}
-
 // Dn_t, Wd_t: accumulators in transposed bin order.  Writes the API-order outputs (any may be NULL):
 // D[A][B] = Dn[A][B] / Wd[A] (row 0 where Wd[A] == 0), Dn, Wd.
 __global__ void k_dmat_normalise(const double *Dn_t, const double *Wd_t, BinParams bp, double *D, double *Dn, double *Wd)
@@ -809,6 +349,8 @@ __global__ void k_dmat_divide(const double *Dn, const double *Wd, int nb, double
 
 }  // namespace
 
+#include "dmat_fast.cuh"
+
 namespace {
 __global__ void k_fp_flag(const int32_t *pq, int64_t n, unsigned long long seed, unsigned long long thr, unsigned *flag)
 {
@@ -816,7 +358,7 @@ __global__ void k_fp_flag(const int32_t *pq, int64_t n, unsigned long long seed,
     if (k >= n) return;
     const int2 e = ((const int2 *)pq)[k];
     const unsigned long long lo = (unsigned long long)min(e.x, e.y), hi = (unsigned long long)max(e.x, e.y);
-    flag[k] = keep_pair(key_lo(seed, lo), key_hi(seed, hi), thr) ? 1u : 0u;
+    flag[k] = lya_keep_pair(lya_key_lo(seed, lo), lya_key_hi(seed, hi), thr) ? 1u : 0u;
 }
 __global__ void k_fp_compact(const int32_t *pq, int64_t n, const unsigned *flag, const unsigned long long *pos, int32_t *out)
 {
@@ -924,7 +466,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_dmat)"); }
     cudaMemsetAsync(Dn, 0, sizeof(double) * (size_t)nb * nb, s);
     cudaMemsetAsync(Wd, 0, sizeof(double) * (size_t)nb, s);
-    cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
+    cudaMemsetAsync(ctx->d_counters, 0, 16 * sizeof(unsigned long long), s);
     unsigned long long thr;
     {
         double t = floor(reject_fraction * 4294967296.0 + 0.5);
@@ -954,13 +496,13 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         F.Dn = Dn; F.Wd = Wd; F.counters = ctx->d_counters;
         const size_t fsmem = sizeof(DmFastWarp) * FD_WARPS;
         const int fgrid = ctx->sm_count;
-        if (bp.pow2) {
-            e = cudaFuncSetAttribute(k_dmat_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (e == cudaSuccess) k_dmat_fast<true><<<fgrid, FD_THREADS, fsmem, s>>>(F);
-        } else {
-            e = cudaFuncSetAttribute(k_dmat_fast<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (e == cudaSuccess) k_dmat_fast<false><<<fgrid, FD_THREADS, fsmem, s>>>(F);
-        }
+        auto launch = [&](auto kern) {
+            cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
+            if (le == cudaSuccess) kern<<<fgrid, FD_THREADS, fsmem, s>>>(F);
+            return le;
+        };
+        if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_fast<true, true>) : launch(k_dmat_fast<false, true>);
+        else e = bp.pow2 ? launch(k_dmat_fast<true, false>) : launch(k_dmat_fast<false, false>);
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_dmat_fast launch"); }
     }
@@ -981,7 +523,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     cudaEventRecord(ctx->ev[1], s);
     k_dmat_normalise<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, s>>>(Dn, Wd, bp, D, Dn_out, Wd_out);
     cudaEventRecord(ctx->ev[2], s);
-    unsigned long long h[8];
+    unsigned long long h[16];
     e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "lya_dmat"); }
@@ -993,6 +535,8 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     case LYA_DEV_TOO_LONG: return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: a listed forest has more than %d pixels", DTILE);
     default: return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)");
     }
+    if (h[10] != 0)
+        return lya_fail(ctx, LYA_ERR_CUDA, "k_dmat_fast: %llu table entries had two holders (LYA_OPT_CHECK_HOLDERS)", h[10]);
     if (stats) {
         memset(stats, 0, sizeof(*stats));
         stats->n_forest_pairs = (uint64_t)pairs->n;

@@ -44,6 +44,7 @@ extern "C" lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
         if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) { cudaFree(ctx->d_counters); free(ctx); return LYA_ERR_CUDA; }
     ctx->force_generic = 0;
     ctx->generic_diagonals = 2;
+    ctx->check_holders = 0;
     ctx->err[0] = 0;
     *out = ctx;
     return LYA_OK;
@@ -71,6 +72,10 @@ extern "C" lya_status lya_set_option(lya_ctx *ctx, lya_option opt, int64_t value
     case LYA_OPT_GENERIC_DIAGONALS:
         if (value != 1 && value != 2 && value != 4) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "LYA_OPT_GENERIC_DIAGONALS takes 1, 2 or 4");
         ctx->generic_diagonals = (int)value;
+        return LYA_OK;
+    case LYA_OPT_CHECK_HOLDERS:
+        if (value != 0 && value != 1) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "LYA_OPT_CHECK_HOLDERS takes 0 or 1");
+        ctx->check_holders = (int)value;
         return LYA_OK;
     default:
         return lya_fail(ctx, LYA_ERR_INVALID_ARG, "unknown option %d", (int)opt);

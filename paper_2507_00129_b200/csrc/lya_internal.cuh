@@ -19,6 +19,7 @@ struct lya_ctx {
     // small persistent device scratch
     unsigned long long *d_counters;   // [16] work counters / flags
     int force_generic;                // LYA_OPT_FORCE_GENERIC: route every pair to the generic kernels
+    int check_holders;                // LYA_OPT_CHECK_HOLDERS: debug variant of the fast kernels that asserts the one-holder invariant
     int generic_diagonals;            // LYA_OPT_GENERIC_DIAGONALS: diagonals per lane of the generic xi kernel (1, 2, 4)
     cudaEvent_t ev[4];
 };
@@ -59,9 +60,10 @@ struct __align__(16) ForestHead {   // 80 bytes, one per forest
 struct LyaPrep {
     int64_t n_forest, n_pack;
     ForestHead *head;               // [n_forest]
-    double *chi, *w;                // [n_pack]
-    double *a;                      // xi: w * delta
-    double *u, *ea, *eg;            // dmat: u = L - Lbar, ea = w / sum w, eg = w u / sum w u^2 (eq. 2.7)
+    double *w;                      // [n_pack]
+    double *chi, *a;                // xi: chi, w * delta
+    double2 *ce;                    // dmat: (chi, ea) interleaved, ea = w / sum w            (eq. 2.7)
+    double *eg, *u;                 // dmat: eg = w u / sum w u^2, u = L - Lbar
     void *base;                     // single allocation behind all of the above
     int max_len;
 };

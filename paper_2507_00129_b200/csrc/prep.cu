@@ -73,13 +73,12 @@ __global__ void k_pack(lya_forests f, const unsigned long long *off2, LyaPrep P)
         const bool in = t < n;
         const double c = in ? f.chi[a + t] : LYA_CHI_SENTINEL;
         const double w = in ? f.w[a + t] : 0.0;
-        P.chi[o + t] = c;
         P.w[o + t] = w;
-        if (XI) P.a[o + t] = in ? w * f.delta[a + t] : 0.0;
+        if (XI) { P.chi[o + t] = c; P.a[o + t] = in ? w * f.delta[a + t] : 0.0; }
         if (DMAT) {
             const double u = in ? f.loglam[a + t] - lbar : 0.0;
             P.u[o + t] = u;
-            P.ea[o + t] = w * invS;
+            P.ce[o + t] = make_double2(c, w * invS);
             P.eg[o + t] = w * u * invV;
         }
     }
@@ -204,17 +203,16 @@ lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { drop(); return lya_cuda_fail(ctx, e, "prep scan"); }
     out->n_pack = (int64_t)total;
-    const int n_arr = 2 + (want_xi ? 1 : 0) + (want_dmat ? 3 : 0);
+    const int n_arr = 1 + (want_xi ? 2 : 0) + (want_dmat ? 4 : 0);
     const size_t head_bytes = sizeof(ForestHead) * (size_t)n;
     const size_t arr_bytes = ((size_t)total * 8 + 255) & ~(size_t)255;
     e = cudaMalloc(&out->base, head_bytes + arr_bytes * n_arr + 256);
     if (e != cudaSuccess) { drop(); out->base = NULL; return lya_cuda_fail(ctx, e, "cudaMalloc(prepared catalogue)"); }
     char *b = (char *)out->base;
     out->head = (ForestHead *)b; b += (head_bytes + 255) & ~(size_t)255;
-    out->chi = (double *)b; b += arr_bytes;
     out->w = (double *)b; b += arr_bytes;
-    if (want_xi) { out->a = (double *)b; b += arr_bytes; }
-    if (want_dmat) { out->u = (double *)b; b += arr_bytes; out->ea = (double *)b; b += arr_bytes; out->eg = (double *)b; b += arr_bytes; }
+    if (want_xi) { out->chi = (double *)b; b += arr_bytes; out->a = (double *)b; b += arr_bytes; }
+    if (want_dmat) { out->ce = (double2 *)b; b += 2 * arr_bytes; out->eg = (double *)b; b += arr_bytes; out->u = (double *)b; b += arr_bytes; }
     const unsigned blocks = (unsigned)((n * 32 + 255) / 256);
     if (want_xi && want_dmat) k_pack<true, true><<<blocks, 256, 0, s>>>(*f, off2, *out);
     else if (want_xi) k_pack<true, false><<<blocks, 256, 0, s>>>(*f, off2, *out);
