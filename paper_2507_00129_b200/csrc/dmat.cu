@@ -440,7 +440,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     const int nb = b->n_par * b->n_perp;
     cudaStream_t s = ctx->stream;
     const BinParams bp = lya_make_binparams(b);
-    const bool use_fast = pairs->n > 0 && (b->n_par + 1) * LYA_NCOL <= FD_SLOTS && b->n_perp + 2 <= 256 &&
+    const bool use_fast = pairs->n > 0 && b->n_par * LYA_NCOL + 1 <= FD_SLOTS && b->n_perp + 2 <= 256 &&
                           !ctx->force_generic;
     double *scal = NULL, *Dn = NULL, *Wd = NULL;          // internal accumulators (transposed bin order)
     bool own_Dn = false, own_Wd = false;
@@ -494,7 +494,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         DmFastParams F;
         F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp; F.seed = seed; F.thr = thr;
         F.Dn = Dn; F.Wd = Wd; F.counters = ctx->d_counters;
-        const size_t fsmem = sizeof(DmFastWarp) * FD_WARPS;
+        const size_t fsmem = FD_SMEM_BYTES;
         const int fgrid = ctx->sm_count;
         auto launch = [&](auto kern) {
             cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);

@@ -20,17 +20,24 @@
 
 namespace {
 
-constexpr int FD_WARPS = 15;                 // one CTA per SM (shared memory: 15.0 KB per warp)
+#ifndef LYA_FD_WARPS
+#define LYA_FD_WARPS 15
+#endif
+constexpr int FD_WARPS = LYA_FD_WARPS;       // one CTA per SM; 5.6 KB of private shared memory per warp + the table pool
 constexpr int FD_THREADS = FD_WARPS * 32;
+constexpr int FD_SMEM_MAX = 232448;          // 227 KB: the most a CTA can have on sm_100
 constexpr int FD_T = LYA_FAST_TILE;
 constexpr int FD_ROWS = 16;
 constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
 constexpr int FD_PAD = 2;
 constexpr int FD_TQ = FD_T + 2 * FD_PAD;
-constexpr int FD_SLOTS = 306;                // (n_par + 1) * LYA_NCOL <= FD_SLOTS
+constexpr int FD_SLOTS = 302;                // n_par * LYA_NCOL + 1 <= FD_SLOTS (the last slot used is garbage)
 constexpr int FD_KCAP = 48;                  // kept pairs queued per forest pair
 constexpr int FD_KBATCH = 24;                // kept pairs drained together (coefficient tables)
 constexpr int FD_CHUNK = 8;
+// Profiling aids (compile-time, off by default; results are WRONG with any of them): -DLYA_ABL_NO_T23,
+// -DLYA_ABL_NO_T4, -DLYA_ABL_NO_MASK, -DLYA_ABL_NO_WALK drop one phase so that its share of the kernel time can
+// be measured as a difference (profiles/r2*_dmat_ablation.md).
 
 struct DmFastParams {
     LyaPrep prep;
@@ -42,27 +49,46 @@ struct DmFastParams {
     unsigned long long *counters;   // [4] next chunk, [2] evaluated, [3] error, [5] kept, [6] binned, [7] scatter-adds, [10] holder conflicts (CHECK)
 };
 
-struct DmKeysA { unsigned long long pk[FD_T], qk[FD_T]; };                 // mask scan: stage-4 keys of the pixels
+struct DmKeysA {                                                             // mask scan
+    unsigned long long qk[FD_T], pk[FD_T];       // stage-4 keys of the pixels of q and p
+    unsigned short pre[FD_T + 2];                // pre[i] = in-window pairs of the rows before i
+};
 struct DmDrainBC {                                                            // passes B and C
     double2 kc01[FD_KBATCH], kc23[FD_KBATCH];    // per kept pair of a batch: om (1, u_j), om (u_i, u_i u_j)
     unsigned short nz[FD_SLOTS];                 // non-zero slots
 };
+// H tables live in a POOL shared by the warps of the CTA: a warp needs one only from pass A to the end of T4
+// (about a third of its time on a forest pair), so fewer tables than warps are enough and the shared memory
+// saved buys resident warps (the kernel is latency-bound: IPC follows the warp count).  A free table is all zero.
+struct __align__(16) DmTable {
+    double2 H01[FD_SLOTS], H23[FD_SLOTS];    // (H_aa, H_ag), (H_ga, H_gg) per slot = col_rel * n_par + b_par; slot LYA_NCOL * n_par = garbage
+};
 struct __align__(16) DmFastWarp {
-    double2 H01[FD_SLOTS], H23[FD_SLOTS];    // (H_aa, H_ag), (H_ga, H_gg) per slot = col_rel * (n_par + 1) + row
     double2 pce[FD_TP];                      // (chi, ea) of p; rows >= len are sentinels
     double2 qce[FD_TQ];                      // (chi, ea) of q, FD_PAD sentinels either side
     double peg[FD_TP], qeg[FD_TQ];           // eg
     union { DmKeysA a; DmDrainBC b; } u;     // the keys are dead once the mask scan is done (shared memory buys occupancy)
     unsigned kept[FD_KCAP];                  // (A << 16) | (i << 8) | j   (A is filled in by the drain)
-    unsigned char jlo[FD_T], jx[FD_T], jhi[FD_T];
+    unsigned char jlo[FD_T + 4], jx[FD_T + 4], jhi[FD_T + 4];   // (row len = a stop row for the mask scan)
+    unsigned nkept, pad_[1];
 };
+constexpr int FD_POOL_HDR = 128;             // owner flags of the tables (one int each)
+#ifdef LYA_FD_NTABLES
+constexpr int FD_NTABLES = LYA_FD_NTABLES;
+#else
+constexpr int FD_NTABLES = (FD_SMEM_MAX - FD_POOL_HDR - (int)sizeof(DmFastWarp) * FD_WARPS) / (int)sizeof(DmTable) < FD_WARPS
+                               ? (FD_SMEM_MAX - FD_POOL_HDR - (int)sizeof(DmFastWarp) * FD_WARPS) / (int)sizeof(DmTable) : FD_WARPS;
+#endif
+static_assert(FD_NTABLES >= 2 && FD_NTABLES * 4 <= FD_POOL_HDR, "table pool");
+constexpr size_t FD_SMEM_BYTES = FD_POOL_HDR + sizeof(DmTable) * FD_NTABLES + sizeof(DmFastWarp) * FD_WARPS;
 
 // shared-memory ADDRESS of the H01 entry of a pixel pair in THIS walk (inside the grid and on the walk's
 // side of chi_i = chi_j: sgn = 0 for chi_i >= chi_j, -1 otherwise); everything else -> the garbage entry.
-// lim = min(LYA_NCOL, n_perp - c0).
+// lim = min(LYA_NCOL, n_perp - c0).  The slot col * n_par + b_par is also the pair's offset from the first
+// bin of column c0 in the transposed bin order of Dn.
 template <bool POW2>
 __device__ __forceinline__ unsigned dm_key(const BinParams &bp, const PairBin &g, double chi_i, double chi_j, unsigned c0,
-                                           unsigned lim, unsigned np1, int sgn, unsigned h01, unsigned garbage)
+                                           unsigned lim, unsigned npar, int sgn, unsigned h01, unsigned garbage)
 {
     const double d = __dsub_rn(chi_i, chi_j);
     const double t = __dadd_rn(chi_i, chi_j);
@@ -76,21 +102,25 @@ __device__ __forceinline__ unsigned dm_key(const BinParams &bp, const PairBin &g
         by = (rperp < bp.rperp_max) ? min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1)) : 0x7fffffffu;
     }
     const unsigned col = by - c0;
-    const bool valid = ((__double2hiint(d) ^ sgn) >= 0) & (bx < np1 - 1u) & (col < lim);
-    return valid ? h01 + ((col * np1 + bx) << 4) : garbage;
+    const unsigned addr = h01 + ((col * npar + bx) << 4);
+    unsigned key;
+    asm("{\n .reg .pred v;\n setp.ge.s32 v, %1, 0;\n setp.lt.and.u32 v, %2, %3, v;\n setp.lt.and.u32 v, %4, %5, v;\n"
+        " selp.u32 %0, %6, %7, v;\n}"
+        : "=r"(key) : "r"(__double2hiint(d) ^ sgn), "r"(bx), "r"(npar), "r"(col), "r"(lim), "r"(addr), "r"(garbage));
+    return key;
 }
 
 // pass A over rows [r0, r1] (a multiple of D rows; rows >= len are sentinels) and diagonals [dlo, dhi].
 // `key`/`cur` are shared-memory addresses of H01 entries; H23 sits at a fixed offset.
 template <int D, bool POW2, bool CHECK>
 __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi,
-                                        int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned np1,
+                                        int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned npar,
                                         int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
-    constexpr unsigned H23OFF = (unsigned)(sizeof(double2) * FD_SLOTS);
+    constexpr unsigned H23OFF = (unsigned)(sizeof(double2) * FD_SLOTS);     // DmTable: H23 follows H01
     const double2 *qce = ws.qce + FD_PAD;
     const double *qeg = ws.qeg + FD_PAD;
-    const unsigned garbage = h01 + ((np1 - 1u) << 4);
+    const unsigned garbage = h01 + ((npar * LYA_NCOL) << 4);
     for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
         const int dl = d0 + lane * D;
         unsigned cur[D], key[D];
@@ -109,7 +139,7 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, int r0, in
             const double2 pv = ws.pce[r0];
 #pragma unroll
             for (int k = 0; k < D; ++k) {
-                key[k] = dm_key<POW2>(bp, g, pv.x, wc[k], c0, lim, np1, sgn, h01, garbage);
+                key[k] = dm_key<POW2>(bp, g, pv.x, wc[k], c0, lim, npar, sgn, h01, garbage);
                 fa[k] = wa[k]; fg[k] = wg[k];
             }
             pa_c = pv.y; pg_c = ws.peg[r0];
@@ -156,7 +186,7 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, int r0, in
 #pragma unroll
                 for (int k = 0; k < D; ++k) {
                     const int sl = (k + u + 1) % D;
-                    key_n[k] = dm_key<POW2>(bp, g, pv.x, wc[sl], c0, lim, np1, sgn, h01, garbage);
+                    key_n[k] = dm_key<POW2>(bp, g, pv.x, wc[sl], c0, lim, npar, sgn, h01, garbage);
                     fa_n[k] = wa[sl]; fg_n[k] = wg[sl];
                 }
 #pragma unroll
@@ -179,81 +209,159 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, int r0, in
 
 template <bool POW2, bool CHECK>
 __device__ __forceinline__ void dm_walk_any(DmFastWarp &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi,
-                                            int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned np1,
+                                            int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned npar,
                                             int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
     if (dhi < dlo) return;
     const int nd = dhi - dlo + 1;
-    if (nd <= 32) dm_walk<1, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, lim, np1, lane, evaluated, conflicts);
-    else dm_walk<2, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, lim, np1, lane, evaluated, conflicts);
+    if (nd <= 32) dm_walk<1, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
+    else dm_walk<2, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
 }
 
-// pass C: drain n queued kept pairs (kept[e] = (i << 8) | j on entry; the bin A is OR-ed into bits 16.. here).
-// clear: T4 zeroes the table entries it read (last batch of a forest pair).
+// transposed bin index b_perp * n_par + b_par of a pixel pair KNOWN to be inside the grid (exact windows)
 template <bool POW2>
-__device__ __forceinline__ void dm_drain_batch(DmFastWarp &ws, unsigned *kept, int n, int nnz, int mp, const DmFastParams &P,
-                                               const PairBin &g, int c0, long long offp, long long offq, int lane,
-                                               bool clear, unsigned long long &n_red)
+__device__ __forceinline__ int dm_bin_in(const BinParams &bp, const PairBin &g, double chi_i, double chi_j)
+{
+    const double d = __dsub_rn(chi_i, chi_j);
+    const double t = __dadd_rn(chi_i, chi_j);
+    unsigned bx, by;
+    if (POW2) {
+        bx = lya_floor_u32(__dmul_rn(fabs(d), g.cx));
+        by = lya_floor_u32(__dmul_rn(t, g.sy));
+    } else {
+        bx = min(lya_floor_u32(__dmul_rn(__dmul_rn(fabs(d), g.c), bp.inv_par)), (unsigned)(bp.n_par - 1));
+        by = min(lya_floor_u32(__dmul_rn(__dmul_rn(t, g.s), bp.inv_perp)), (unsigned)(bp.n_perp - 1));
+    }
+    return (int)(by * (unsigned)bp.n_par + bx);
+}
+
+__device__ __forceinline__ void dm_red(double *addr, double v)
+{
+    asm volatile("red.global.add.f64 [%0], %1;" :: "l"(addr), "d"(v) : "memory");
+}
+
+
+// ---- pass C, first half (no H table needed) ------------------------------------------------------
+// n queued kept pairs, kept[e] = (i << 8) | j on entry.  Coefficients of every kept pair into kc01 / kc23, the
+// bin A OR-ed into bits 16.. of kept[e]; with scatter: T1 (Dn[A][A] += om, Wd[A] += om), T2 (row i's window)
+// and T3 (the rows whose window holds j).  The windows are exact, so no pair is re-tested against the grid.
+// Dn has n_bins^2 <= 2^24 entries, so element indices are 32-bit and an address is one IMAD.WIDE away.
+// (Tried and dropped: keeping each lane's rows / columns in registers for the whole drain -- fewer shared-memory
+// wavefronts, but the extra live registers spilled and it was 3-9 % slower.)
+template <bool POW2>
+__device__ __forceinline__ void dm_drain_t123(DmFastWarp &ws, unsigned *kept, int n, int mp, const DmFastParams &P,
+                                              const PairBin &g, long long offp, long long offq, int lane,
+                                              bool scatter, unsigned &n_red)
 {
     const BinParams &bp = P.bp;
-    const int nb = bp.n_par * bp.n_perp, np1 = bp.n_par + 1;
+    const unsigned nb = (unsigned)(bp.n_par * bp.n_perp);
     const double2 *qce = ws.qce + FD_PAD;
     const double *qeg = ws.qeg + FD_PAD;
-    // coefficients of every kept pair (lanes over kept pairs) and T1: Dn[A][A] += om, Wd[A] += om
+    double *const Dn = P.Dn;
     for (int e = lane; e < n; e += 32) {
         const unsigned rec = kept[e];
         const int i = (rec >> 8) & 0xff, j = rec & 0xff;
-        const int A = lya_pix_bin_t<POW2>(bp, g, ws.pce[i].x, qce[j].x);           // inside the grid by construction
+        const unsigned A = (unsigned)dm_bin_in<POW2>(bp, g, ws.pce[i].x, qce[j].x);
         const double om = P.prep.w[offp + i] * P.prep.w[offq + j], ui = P.prep.u[offp + i], uj = P.prep.u[offq + j];
         const double omi = om * ui;
         ws.u.b.kc01[e] = make_double2(om, om * uj);
         ws.u.b.kc23[e] = make_double2(omi, omi * uj);
-        kept[e] = ((unsigned)A << 16) | (rec & 0xffffu);
-        atomicAdd(P.Dn + (size_t)A * nb + A, om);
-        atomicAdd(P.Wd + A, om);
-        n_red += 2;
+        kept[e] = (A << 16) | (rec & 0xffffu);
+        if (scatter) {
+            dm_red(Dn + (A * nb + A), om);
+            dm_red(P.Wd + A, om);
+            n_red += 2u;
+        }
     }
     __syncwarp();
-    // T2: -(om ea_j' + om u_j eg_j') over row i's window;  T3: -(om ea_i' + om u_i eg_i') over the rows whose
-    // window holds j.  The windows are exact, so no pair is re-tested against the grid.
+    if (!scatter) return;
+#pragma unroll 1
     for (int e = 0; e < n; ++e) {
         const unsigned rec = kept[e];
         const int i = (rec >> 8) & 0xff, j = rec & 0xff;
-        const double2 c01 = ws.u.b.kc01[e], c23 = ws.u.b.kc23[e];
+        const double2 c01 = ws.u.b.kc01[e];
+        const double m0 = -c01.x, m1 = -c01.y, m2 = -ws.u.b.kc23[e].x;
         const double ci = ws.pce[i].x, cj = qce[j].x;
-        double *row = P.Dn + (size_t)(rec >> 16) * nb;
-        const int jl = ws.jlo[i], jh = ws.jhi[i];
-        for (int j2 = jl + lane; j2 < jh; j2 += 32) {
+        const unsigned row = (rec >> 16) * nb;
+        const int jh = ws.jhi[i];
+#pragma unroll 1
+        for (int j2 = ws.jlo[i] + lane; j2 < jh; j2 += 32) {                      // T2
             const double2 q2 = qce[j2];
-            const int B = lya_pix_bin_t<POW2>(bp, g, ci, q2.x);
-            atomicAdd(row + B, -fma(c01.y, qeg[j2], c01.x * q2.y));
+            dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, ci, q2.x)), fma(m1, qeg[j2], m0 * q2.y));
+            n_red += 1u;
         }
-        n_red += (unsigned long long)(lane == 0 ? jh - jl : 0);
-        for (int i2 = lane; i2 < mp; i2 += 32) {
-            if (j >= (int)ws.jlo[i2] && j < (int)ws.jhi[i2]) {
+#pragma unroll 1
+        for (int i2 = lane; i2 < mp; i2 += 32) {                                  // T3
+            const unsigned lo2 = ws.jlo[i2];
+            if ((unsigned)j - lo2 < (unsigned)ws.jhi[i2] - lo2) {
                 const double2 p2 = ws.pce[i2];
-                const int B = lya_pix_bin_t<POW2>(bp, g, p2.x, cj);
-                atomicAdd(row + B, -fma(c23.x, ws.peg[i2], c01.x * p2.y));
-                n_red += 1;
+                dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, p2.x, cj)), fma(m2, ws.peg[i2], m0 * p2.y));
+                n_red += 1u;
             }
         }
     }
-    // T4: lanes over the non-zero table entries, inner loop over the kept pairs
-    for (int t = lane; t < nnz; t += 32) {
-        const int slot = ws.u.b.nz[t];
-        const int cr = slot / np1, bx = slot - cr * np1;
-        double *colB = P.Dn + ((c0 + cr) * bp.n_par + bx);
-        const double2 a = ws.H01[slot], b = ws.H23[slot];
-        if (clear) { ws.H01[slot] = make_double2(0.0, 0.0); ws.H23[slot] = make_double2(0.0, 0.0); }
-#pragma unroll 2
-        for (int e = 0; e < n; ++e) {
-            const unsigned A = kept[e] >> 16;
-            const double2 c01 = ws.u.b.kc01[e], c23 = ws.u.b.kc23[e];
-            const double v = fma(c23.y, b.y, fma(c23.x, b.x, fma(c01.y, a.y, c01.x * a.x)));
-            atomicAdd(colB + (size_t)A * nb, v);
+}
+
+// ---- pass C, second half: T4 of n kept pairs whose coefficients are in kc01 / kc23: lanes over the non-zero
+// table entries (consecutive slots are consecutive bins of Dn's row), kept pairs EIGHT at a time with their
+// coefficients in registers.  wipe: zero the table entries read (last use of the table for this forest pair).
+#ifndef LYA_FD_T4B
+#define LYA_FD_T4B 4
+#endif
+constexpr int FD_T4B = LYA_FD_T4B;
+__device__ __forceinline__ void dm_drain_t4(DmFastWarp &ws, DmTable &tb, const unsigned *kept, int n, int nnz,
+                                            const DmFastParams &P, int c0, int lane, bool wipe_after, unsigned &n_red)
+{
+    const unsigned nb = (unsigned)(P.bp.n_par * P.bp.n_perp);
+    double *const Dn = P.Dn;
+    const unsigned col0 = (unsigned)(c0 * P.bp.n_par);
+#ifdef LYA_ABL_NO_T4
+    if (n > 0) n = 0;
+#endif
+    for (int e0 = 0; e0 < n || (wipe_after && e0 == 0); e0 += FD_T4B) {
+        double2 k01[FD_T4B], k23[FD_T4B];
+        unsigned ro[FD_T4B];
+#pragma unroll
+        for (int k = 0; k < FD_T4B; ++k) {
+            const int e = min(e0 + k, max(n - 1, 0));
+            k01[k] = ws.u.b.kc01[e];
+            k23[k] = ws.u.b.kc23[e];
+            ro[k] = (kept[e] >> 16) * nb + col0;
         }
-        n_red += (unsigned long long)n;
+        const int m = min(FD_T4B, n - e0);
+        const bool wipe = wipe_after && e0 + FD_T4B >= n;
+#pragma unroll 1
+        for (int t = lane; t < nnz; t += 32) {
+            const unsigned slot = ws.u.b.nz[t];
+            const double2 a = tb.H01[slot], b = tb.H23[slot];
+            if (wipe) { tb.H01[slot] = make_double2(0.0, 0.0); tb.H23[slot] = make_double2(0.0, 0.0); }
+#pragma unroll
+            for (int k = 0; k < FD_T4B; ++k)
+                if (k < m) dm_red(Dn + (ro[k] + slot), fma(k23[k].y, b.y, fma(k23[k].x, b.x, fma(k01[k].y, a.y, k01[k].x * a.x))));
+        }
+        if (lane == 0) n_red += (unsigned)(max(m, 0) * nnz);
     }
+}
+
+// table pool: lane 0 claims a free table (owner flag 0 -> 1), probing round-robin from the warp's own slot
+__device__ __forceinline__ int dm_table_acquire(int *owner, int wid, int lane)
+{
+    int t = 0;
+    if (lane == 0) {
+        const int t0 = wid % FD_NTABLES;
+        t = t0;
+        while (atomicCAS(&owner[t], 0, 1) != 0) {
+            t = (t + 1 == FD_NTABLES) ? 0 : t + 1;
+            __nanosleep(64);
+        }
+        __threadfence_block();
+    }
+    return __shfl_sync(0xffffffffu, t, 0);
+}
+__device__ __forceinline__ void dm_table_release(int *owner, int t, int lane)
+{
+    __syncwarp();
+    if (lane == 0) { __threadfence_block(); atomicExch(&owner[t], 0); }
 }
 
 template <bool POW2, bool CHECK>
@@ -261,15 +369,27 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    DmFastWarp &ws = ((DmFastWarp *)smem_raw)[wid];
+    int *owner = (int *)smem_raw;
+    DmTable *tables = (DmTable *)(smem_raw + FD_POOL_HDR);
+    DmFastWarp &ws = ((DmFastWarp *)(smem_raw + FD_POOL_HDR + sizeof(DmTable) * FD_NTABLES))[wid];
     const BinParams bp = P.bp;
-    const unsigned np1 = (unsigned)bp.n_par + 1u;
-    const int n_slots = (int)np1 * LYA_NCOL;
-    for (int t = lane; t < FD_SLOTS; t += 32) { ws.H01[t] = make_double2(0.0, 0.0); ws.H23[t] = make_double2(0.0, 0.0); }
+    const unsigned npar = (unsigned)bp.n_par;
+    const int n_slots = bp.n_par * LYA_NCOL;                  // real slots; slot n_slots is the garbage entry
+    for (int t = threadIdx.x; t < FD_NTABLES * FD_SLOTS; t += FD_THREADS) {
+        tables[t / FD_SLOTS].H01[t % FD_SLOTS] = make_double2(0.0, 0.0);
+        tables[t / FD_SLOTS].H23[t % FD_SLOTS] = make_double2(0.0, 0.0);
+    }
+    if (threadIdx.x < FD_NTABLES) owner[threadIdx.x] = 0;
     if (lane < FD_PAD) { ws.qce[lane] = make_double2(LYA_CHI_SENTINEL, 0.0); ws.qeg[lane] = 0.0; }
-    __syncwarp();
+    if (lane == 0) ws.nkept = 0u;
+    __syncthreads();
     const double2 *qce = ws.qce + FD_PAD;
-    const unsigned h01 = (unsigned)__cvta_generic_to_shared(ws.H01);
+#ifdef LYA_ABL_NO_MASK
+    const bool keep_none = true;
+#else
+    const bool keep_none = P.thr > 0xffffffffull;              // reject_fraction = 1
+#endif
+    const unsigned thr32 = (unsigned)P.thr;
     unsigned long long evaluated = 0, kept_total = 0, binned_total = 0, n_red = 0;
     unsigned conflicts = 0;
     int cur_p = -1, head_p = -1;
@@ -300,7 +420,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
             const unsigned lim = (unsigned)min(LYA_NCOL, bp.n_perp - c0);
             __syncwarp();
-            // ---- stage p (when it changes) and q: (chi, ea) pairs with 16-byte loads, eg, stage-4 keys ----
+            // ---- stage p (when it changes) and q: (chi, ea) pairs with 16-byte loads, eg, q's stage-4 keys ----
             if (p != cur_p) {
                 const double2 *sce = P.prep.ce + hp.off;
                 const double2 *sg = (const double2 *)(P.prep.eg + hp.off);
@@ -318,43 +438,95 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 const int npad = (mq + 1) & ~1;
                 for (int t = lane; t < npad; t += 32) ws.qce[FD_PAD + t] = sce[t];       // (the pad pixel of an odd forest is a sentinel)
                 for (int t = lane; 2 * t < npad; t += 32) ((double2 *)(ws.qeg + FD_PAD))[t] = sg[t];
-                for (int t = lane; t < mq; t += 32) ws.u.a.qk[t] = lya_key_hi(P.seed, (unsigned long long)(hq.pix0 + t));
-                // (the keys share their storage with the drain tables, so p's keys are rebuilt for every pair)
-                for (int t = lane; t < mp; t += 32) ws.u.a.pk[t] = lya_key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
+                if (!keep_none)
+                    for (int t = lane; t < mq; t += 32) ws.u.a.qk[t] = lya_key_hi(P.seed, (unsigned long long)(hq.pix0 + t));
                 if (lane < FD_PAD) {
                     const int j = FD_PAD + npad + lane;
                     ws.qce[j] = make_double2(LYA_CHI_SENTINEL, 0.0); ws.qeg[j] = 0.0;
                 }
             }
             __syncwarp();
-            // ---- windows: per row of p the exact in-grid window [jlo, jhi) of q and the sign change jx ----
+            // ---- windows (lanes over rows): the exact in-grid window [jlo, jhi) of q and the sign change jx;
+            //      mask (same lanes): stage 4 over the window, pure integer; kept pairs (1 % at f = 0.99) are
+            //      queued as (i, j) through a shared counter ----
             const double R = (c > 0.0) ? (bp.rpar_max / c) * (1.0 + 1e-12) + 1e-9 : 1e300;
             const double Tchi = (s > 0.0) ? (bp.rperp_max / s) * (1.0 + 1e-12) + 1e-9 : 1e300;
-            for (int i = lane; i < mp; i += 32) {
-                int jlo, jx, jhi;
-                lya_row_window<POW2>(bp, g, qce, mq, ws.pce[i].x, R, Tchi, jlo, jx, jhi);
-                ws.jlo[i] = (unsigned char)jlo; ws.jx[i] = (unsigned char)jx; ws.jhi[i] = (unsigned char)jhi;
-            }
-            __syncwarp();
-            // ---- mask: stage 4 over the windows (integer only); queue the kept pairs ----
-            unsigned nk = 0, binned = 0;
-            for (int i = 0; i < mp; ++i) {
-                const int jl = ws.jlo[i], jh = ws.jhi[i];
-                const unsigned long long pki = ws.u.a.pk[i];
-                binned += (unsigned)(jh - jl);
-                for (int j0 = jl; j0 < jh; j0 += 32) {
-                    const int j = j0 + lane;
-                    const bool kp = (j < jh) && lya_keep_pair(pki, ws.u.a.qk[min(j, FD_T - 1)], P.thr);
-                    const unsigned bal = __ballot_sync(0xffffffffu, kp);
-                    if (bal) {
-                        const unsigned idx = nk + __popc(bal & ((1u << lane) - 1u));
-                        if (kp && idx < FD_KCAP) ws.kept[idx] = ((unsigned)i << 8) | (unsigned)j;
-                        nk += __popc(bal);
-                    }
+            unsigned binned = 0;
+            for (int ib = 0; ib < mp; ib += 32) {            // (warp-uniform trip counts: the warp must not stay split)
+                const int i = ib + lane;
+                if (i < mp) {
+                    int jlo, jx, jhi;
+                    lya_row_window<POW2>(bp, g, qce, mq, ws.pce[i].x, R, Tchi, jlo, jx, jhi);
+                    ws.jlo[i] = (unsigned char)jlo; ws.jx[i] = (unsigned char)jx; ws.jhi[i] = (unsigned char)jhi;
+                    binned += (unsigned)(jhi - jlo);
                 }
             }
-            binned_total += binned; kept_total += nk;
-            // ---- pass A: H tables ----
+            __syncwarp();
+            if (!keep_none) {
+                // Balanced scan: the in-window pairs of all rows form one list of M entries (row-major); lane l
+                // takes entries [l K, (l + 1) K), K = ceil(M / 32).  pre[] (rows before i) is a warp scan with three
+                // consecutive rows per lane; a lane finds its first row by binary search and then walks along,
+                // stepping to the next non-empty row when its window ends.
+                const int r3 = 3 * lane;
+                unsigned w0 = 0, w1 = 0, w2 = 0;
+                if (r3 < mp) w0 = (unsigned)ws.jhi[r3] - ws.jlo[r3];
+                if (r3 + 1 < mp) w1 = (unsigned)ws.jhi[r3 + 1] - ws.jlo[r3 + 1];
+                if (r3 + 2 < mp) w2 = (unsigned)ws.jhi[r3 + 2] - ws.jlo[r3 + 2];
+                unsigned incl = w0 + w1 + w2;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const unsigned v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+                const unsigned M = __shfl_sync(0xffffffffu, incl, 31);
+                const unsigned excl = incl - (w0 + w1 + w2);
+                if (r3 <= mp) ws.u.a.pre[r3] = (unsigned short)excl;
+                if (r3 + 1 <= mp) ws.u.a.pre[r3 + 1] = (unsigned short)(excl + w0);
+                if (r3 + 2 <= mp) ws.u.a.pre[r3 + 2] = (unsigned short)(excl + w0 + w1);
+                for (int t = lane; t < mp; t += 32) ws.u.a.pk[t] = lya_key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
+                if (lane == 0) { ws.jlo[mp] = 0; ws.jhi[mp] = 0xff; }          // stop row: never left, never counted
+                __syncwarp();
+                const unsigned K = (M + 31u) >> 5;
+                const unsigned first = min((unsigned)lane * K, M), last = min(first + K, M);
+                int row = 0;
+                {   // last row with pre[row] <= first  (pre is non-decreasing, pre[0] = 0)
+                    int lo = 0, hi = mp;
+                    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (ws.u.a.pre[mid] <= first) lo = mid; else hi = mid - 1; }
+                    row = lo;
+                }
+                int j = (int)ws.jlo[row] + (int)(first - ws.u.a.pre[row]);
+                int jend = ws.jhi[row];
+                unsigned long long pki = ws.u.a.pk[min(row, FD_T - 1)];
+                const unsigned n_it = __reduce_max_sync(0xffffffffu, last - first);
+                for (unsigned t = 0; t < n_it; ++t) {
+                    if (j >= jend) {                             // next non-empty row (the stop row ends the search)
+                        do { ++row; } while (ws.jlo[row] == ws.jhi[row]);
+                        j = ws.jlo[row]; jend = ws.jhi[row];
+                        pki = ws.u.a.pk[min(row, FD_T - 1)];
+                    }
+                    const unsigned h = lya_pair_hash32(pki, ws.u.a.qk[min(j, FD_T - 1)]);
+                    if ((first + t < last) & (h >= thr32)) {
+                        const unsigned idx = atomicAdd(&ws.nkept, 1u);
+                        if (idx < FD_KCAP) ws.kept[idx] = ((unsigned)row << 8) | (unsigned)j;
+                    }
+                    ++j;
+                }
+            }
+            binned_total += binned;
+            __syncwarp();
+            const unsigned nk = ws.nkept;
+            kept_total += (lane == 0) ? nk : 0u;
+            // ---- pass C, first half: T1..T3 of the queued kept pairs (no H table needed yet).  Normally the
+            //      queue holds every kept pair; with more than it holds (small reject fractions) the mask is
+            //      redone row by row further down and the queue drained each time it fills ----
+            const bool overflow = nk > FD_KCAP;
+            const int n_q0 = overflow ? 0 : (int)nk;
+            unsigned n_red32 = 0;
+            for (int e0 = 0; e0 < n_q0; e0 += FD_KBATCH) {
+                dm_drain_t123<POW2>(ws, ws.kept + e0, min(FD_KBATCH, n_q0 - e0), mp, P, g, hp.off, hq.off, lane, true, n_red32);
+                __syncwarp();
+            }
+            // ---- pass A: H tables, in a table of the pool ----
+            const int tix = dm_table_acquire(owner, wid, lane);
+            DmTable &tb = tables[tix];
+            const unsigned h01 = (unsigned)__cvta_generic_to_shared(tb.H01);
             for (int i0 = 0; i0 < mp; i0 += FD_ROWS) {
                 const int i = i0 + lane;
                 int plo = 1 << 20, phi = -(1 << 20), nlo = 1 << 20, nhi = -(1 << 20);
@@ -372,8 +544,11 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 for (int sgn = 0; sgn >= -1; --sgn) {       // one call site: chi_i >= chi_j, then chi_i < chi_j
                     const int r0 = sgn ? nr0 : pr0, r1 = sgn ? nr1 : pr1;
                     if (r1 < r0) continue;
+#ifdef LYA_ABL_NO_WALK
+                    continue;
+#endif
                     dm_walk_any<POW2, CHECK>(ws, h01, r0 & ~1, r1 | 1, mq, sgn ? nlo : plo, sgn ? nhi : phi, sgn, bp, g,
-                                             (unsigned)c0, lim, np1, lane, evaluated, conflicts);
+                                             (unsigned)c0, lim, npar, lane, evaluated, conflicts);
                 }
             }
             __syncwarp();
@@ -383,24 +558,30 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 const int t = t0 + lane;
                 bool nzf = false;
                 if (t < n_slots) {
-                    const int cr = t / (int)np1, bx = t - cr * (int)np1;
-                    const double2 a = ws.H01[t], b = ws.H23[t];
-                    nzf = (bx < bp.n_par) && (a.x != 0.0 || a.y != 0.0 || b.x != 0.0 || b.y != 0.0);
+                    const double2 a = tb.H01[t], b = tb.H23[t];
+                    nzf = (a.x != 0.0) | (a.y != 0.0) | (b.x != 0.0) | (b.y != 0.0);
                 }
                 const unsigned bal = __ballot_sync(0xffffffffu, nzf);
                 if (nzf) ws.u.b.nz[nnz + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)t;
                 nnz += __popc(bal);
             }
             __syncwarp();
-            // ---- pass C (one drain call site: the kernel's code has to stay small for the instruction cache) ----
-            // Normally the queue holds every kept pair.  With more kept pairs than the queue holds (small
-            // reject fractions) the mask is redone row by row and the queue drained each time it fills.
-            const bool overflow = nk > FD_KCAP;
-            int n_q = overflow ? 0 : (int)nk;
-            int si = 0, sj = (overflow && mp > 0) ? (int)ws.jlo[0] : 0;
-            for (;;) {
-                bool done = true;
-                if (overflow) {
+            // ---- pass C, second half: T4 (and, in the overflow case, the whole drain batch by batch) ----
+            if (!overflow) {
+                if (n_q0 <= FD_KBATCH) {                     // the coefficients of the only batch are still in place
+                    dm_drain_t4(ws, tb, ws.kept, n_q0, nnz, P, c0, lane, true, n_red32);
+                } else {
+                    for (int e0 = 0; e0 < n_q0; e0 += FD_KBATCH) {
+                        const int nb_e = min(FD_KBATCH, n_q0 - e0);
+                        dm_drain_t123<POW2>(ws, ws.kept + e0, nb_e, mp, P, g, hp.off, hq.off, lane, false, n_red32);
+                        dm_drain_t4(ws, tb, ws.kept + e0, nb_e, nnz, P, c0, lane, e0 + FD_KBATCH >= n_q0, n_red32);
+                        __syncwarp();
+                    }
+                }
+            } else {
+                int si = 0, sj = (mp > 0) ? (int)ws.jlo[0] : 0;
+                for (;;) {
+                    int n_q = 0;
                     while (si < mp) {
                         const int jh = ws.jhi[si];
                         if (sj >= jh) { ++si; sj = (si < mp) ? (int)ws.jlo[si] : 0; continue; }
@@ -413,26 +594,28 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                         n_q += __popc(bal);
                         sj += 32;
                     }
-                    done = si >= mp;
-                }
-                __syncwarp();
-                for (int e0 = 0; e0 < n_q || e0 == 0; e0 += FD_KBATCH) {
-                    const int nb_e = min(FD_KBATCH, n_q - e0);
-                    dm_drain_batch<POW2>(ws, ws.kept + e0, nb_e, nnz, mp, P, g, c0, hp.off, hq.off, lane,
-                                         done && e0 + FD_KBATCH >= n_q, n_red);
+                    const bool done = si >= mp;
                     __syncwarp();
+                    for (int e0 = 0; e0 < n_q || e0 == 0; e0 += FD_KBATCH) {
+                        const int nb_e = max(min(FD_KBATCH, n_q - e0), 0);
+                        dm_drain_t123<POW2>(ws, ws.kept + e0, nb_e, mp, P, g, hp.off, hq.off, lane, true, n_red32);
+                        dm_drain_t4(ws, tb, ws.kept + e0, nb_e, nnz, P, c0, lane, done && e0 + FD_KBATCH >= n_q, n_red32);
+                        __syncwarp();
+                    }
+                    if (done) break;
                 }
-                if (done) break;
-                n_q = 0;
             }
-            // the garbage entry collects every out-of-grid product: clear it too
-            if (lane == 0) { ws.H01[np1 - 1u] = make_double2(0.0, 0.0); ws.H23[np1 - 1u] = make_double2(0.0, 0.0); }
-            __syncwarp();
+            n_red += n_red32;
+            // the garbage entry collects every out-of-grid product: clear it too, then hand the table back
+            if (lane == 0) { tb.H01[n_slots] = make_double2(0.0, 0.0); tb.H23[n_slots] = make_double2(0.0, 0.0); ws.nkept = 0u; }
+            dm_table_release(owner, tix, lane);
         }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
+        kept_total += __shfl_xor_sync(0xffffffffu, kept_total, o);
+        binned_total += __shfl_xor_sync(0xffffffffu, binned_total, o);
         n_red += __shfl_xor_sync(0xffffffffu, n_red, o);
         conflicts += __shfl_xor_sync(0xffffffffu, conflicts, o);
     }
