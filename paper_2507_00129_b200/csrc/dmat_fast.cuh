@@ -27,8 +27,11 @@ constexpr int FD_WARPS = LYA_FD_WARPS;       // one CTA per SM; 5.6 KB of privat
 constexpr int FD_THREADS = FD_WARPS * 32;
 constexpr int FD_SMEM_MAX = 232448;          // 227 KB: the most a CTA can have on sm_100
 constexpr int FD_T = LYA_FAST_TILE;
-constexpr int FD_ROWS = 16;
-constexpr int FD_TP = ((FD_T + FD_ROWS - 1) / FD_ROWS) * FD_ROWS + 2;
+#ifndef LYA_FD_ROWS
+#define LYA_FD_ROWS 16
+#endif
+constexpr int FD_ROWS = LYA_FD_ROWS;         // rows of p per pass-A group
+constexpr int FD_TP = ((FD_T + 15) / 16) * 16 + 2;
 constexpr int FD_PAD = 2;
 constexpr int FD_TQ = FD_T + 2 * FD_PAD;
 constexpr int FD_SLOTS = 302;                // n_par * LYA_NCOL + 1 <= FD_SLOTS (the last slot used is garbage)
@@ -275,6 +278,9 @@ __device__ __forceinline__ void dm_drain_t123(DmFastWarp &ws, unsigned *kept, in
     }
     __syncwarp();
     if (!scatter) return;
+#ifdef LYA_ABL_NO_T23
+    return;
+#endif
 #pragma unroll 1
     for (int e = 0; e < n; ++e) {
         const unsigned rec = kept[e];

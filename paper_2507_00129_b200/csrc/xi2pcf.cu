@@ -308,8 +308,11 @@ cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
 constexpr int FW = 14;                       // warps per block, one block per SM (16.2 KB of shared memory per warp)
 constexpr int FTHREADS = FW * 32;
 constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
-constexpr int FROWS = 16;                    // rows of p walked per pass (keeps lanes busy: DESIGN.md)
-constexpr int FTP = ((FT + FROWS - 1) / FROWS) * FROWS + 2;   // p rows incl. sentinel rows
+#ifndef LYA_FROWS
+#define LYA_FROWS 16
+#endif
+constexpr int FROWS = LYA_FROWS;             // rows of p walked per pass (keeps lanes busy: DESIGN.md)
+constexpr int FTP = ((FT + 15) / 16) * 16 + 2;   // p rows incl. sentinel rows
 constexpr int FPAD = 2;                      // sentinel pixels either side of q (reads are clamped)
 constexpr int FSLOTS = 612;                  // 2 * (n_par + 1) * LYA_NCOL <= FSLOTS
 constexpr int FCHUNK = 16;                   // forest pairs claimed per atomic

@@ -244,6 +244,23 @@ def test_kernel_routes_fast_and_generic(B, orc):
     c.close()
 
 
+def test_one_holder_invariant_debug_variant(B, orc):
+    """LYA_OPT_CHECK_HOLDERS: the debug variant of the fast D kernel checks at every row step of pass A that no
+    two lanes of a warp hold the same H-table entry (the invariant the atomic-free accumulation rests on).
+    It must report no violation on a configs[4]-shaped sub-patch and give the same result."""
+    f = gen.make_config(4, n_forest=300, density_scale=2.0)
+    seed = gen.mask_seed(4)
+    c = B.Context("cuda:0")
+    c.lya_set_option("check_holders", 1)
+    d = B.DeviceForests(f)
+    pairs = c.lya_neighbours(d, B.binning())
+    g = c.lya_dmat(d, B.binning(), pairs, 0.9, seed)          # raises LYA_ERR_CUDA on a violation
+    ref = orc.pairs_window(f)
+    check_dmat(g, orc.dmat(f, ref, 0.9, seed), "check_holders")
+    assert g["stats"]["n_scatter"] > 0                        # the fast kernel ran
+    c.close()
+
+
 def test_forest_pair_subsampling_next2(ctx, B, orc):
     """D from a subset of FOREST pairs = lya_pairs_subsample + lya_dmat(f = 0)."""
     f = gen.make_config(1, n_forest=150, density_scale=4.0)
