@@ -107,70 +107,105 @@ def measured_peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0), "fallback"
 
 
+def cpu_model():
+    try:
+        for l in open("/proc/cpuinfo"):
+            if l.startswith("model name"):
+                return l.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+class OracleSample:
+    """ONE definition of the bounded oracle workload, used by both the `cpu_baseline` leg and `--impl reference`:
+    a shaped sub-catalogue of the workload's config (same sky density), xi over all of its listed forest pairs
+    and the naive quadruple-sum D over the first 1/dmat_div of them."""
+
+    def __init__(self, wl, n_forests, dmat_div):
+        from oracle import oracle as orc
+        from paper_2507_00129_b200 import gen
+        self.orc = orc
+        self.n_s = min(n_forests, gen.CONFIGS[wl["cfg"]]["n"])
+        f = gen.make_config(wl["cfg"], n_forest=self.n_s)
+        self.cat = orc.Catalogue(f)
+        self.pq = orc.pairs_window(self.cat)
+        self.pq_d = self.pq[: max(1, len(self.pq) // dmat_div)]
+        self.seed = gen.mask_seed(wl["mask_cfg"])
+        self.frac = 0.0 if wl["cfg"] == 0 else 0.99
+        self.n_xi = None
+        self.n_d = None
+
+    def describe(self):
+        return (f"{self.n_s} forests at the workload's sky density: xi over {len(self.pq)} forest pairs, "
+                f"naive D (f={self.frac}) over {len(self.pq_d)} forest pairs, per step")
+
+    def step(self):
+        """-> (pairs counted as in the GPU metric, seconds xi, seconds D)."""
+        orc = self.orc
+        t0 = time.perf_counter()
+        x = orc.xi(self.cat, self.pq)
+        t1 = time.perf_counter()
+        orc.dmat(self.cat, self.pq_d, self.frac, self.seed, want_D=False)
+        t2 = time.perf_counter()
+        if self.n_xi is None:
+            self.n_xi = int(x["N"].sum())
+            self.n_d = int(orc.xi(self.cat, self.pq_d)["N"].sum()) if len(self.pq_d) != len(self.pq) else self.n_xi
+        return self.n_xi + self.n_d, t1 - t0, t2 - t1
+
+    def single_thread_xi(self, frac=16):
+        """xi pairs/s of ONE thread on 1/frac of the forest pairs (libgomp's thread count set for this call)."""
+        import ctypes as C
+        try:
+            gomp = C.CDLL("libgomp.so.1")
+            n0 = self.orc.num_threads()
+            gomp.omp_set_num_threads(1)
+            pq = self.pq[: max(1, len(self.pq) // frac)]
+            t0 = time.perf_counter()
+            x = self.orc.xi(self.cat, pq)
+            dt = time.perf_counter() - t0
+            gomp.omp_set_num_threads(n0)
+            return int(x["N"].sum()) / dt
+        except Exception:
+            return None
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on a bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle import oracle as orc
-    from paper_2507_00129_b200 import gen
     wl = WORKLOADS[args.workload]
-    n_s = min(args.ref_forests, gen.CONFIGS[wl["cfg"]]["n"])
-    f = gen.make_config(wl["cfg"], n_forest=n_s)
-    cat = orc.Catalogue(f)
-    pq = orc.pairs_window(cat)
-    pq_d = pq[: max(1, len(pq) // args.ref_dmat_div)]
-    seed = gen.mask_seed(wl["mask_cfg"])
-    frac = 0.0 if wl["cfg"] == 0 else 0.99
-
-    def step():
-        x = orc.xi(cat, pq)
-        d = orc.dmat(cat, pq_d, frac, seed, want_D=False)
-        nd = int(orc.xi(cat, pq_d)["N"].sum()) if len(pq_d) != len(pq) else int(x["N"].sum())
-        return int(x["N"].sum()) + nd
-
+    smp = OracleSample(wl, args.cpu_forests, args.cpu_dmat_div)
     for _ in range(args.warmup):
-        step()
+        smp.step()
     t0 = time.perf_counter()
     pairs = 0
     for _ in range(args.steps):
-        pairs += step()
+        pairs += smp.step()[0]
     dt = time.perf_counter() - t0
     val = pairs / dt
-    sample = (f"{n_s} forests of {args.workload} at the config's sky density: xi on {len(pq)} forest pairs, "
-              f"naive D on {len(pq_d)} forest pairs, per step")
+    sample = smp.describe()
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "description": wl["desc"], "sample": sample},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smp.orc.num_threads(), "cpu": cpu_model(), "kind": "oracle",
+                         "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
 
-def cpu_baseline(wl, budget_forests):
-    """The oracle timed on this box's host cores on a bounded sample (about 10-30 s)."""
-    from oracle import oracle as orc
-    from paper_2507_00129_b200 import gen
-    n_s = min(budget_forests, gen.CONFIGS[wl["cfg"]]["n"])
-    f = gen.make_config(wl["cfg"], n_forest=n_s)
-    cat = orc.Catalogue(f)
-    pq = orc.pairs_window(cat)
-    t0 = time.perf_counter()
-    x = orc.xi(cat, pq)
-    t_xi = time.perf_counter() - t0
-    pq_d = pq[: max(1, len(pq) // 8)]
-    frac = 0.0 if wl["cfg"] == 0 else 0.99
-    t0 = time.perf_counter()
-    orc.dmat(cat, pq_d, frac, gen.mask_seed(wl["mask_cfg"]), want_D=False)
-    t_d = time.perf_counter() - t0
-    nd = int(orc.xi(cat, pq_d)["N"].sum())
-    nx = int(x["N"].sum())
-    return {"value": (nx + nd) / (t_xi + t_d), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-            "xi_pairs_per_s": nx / t_xi, "dmat_pairs_per_s": nd / max(t_d, 1e-9),
-            "sample": f"{n_s} forests at the workload's sky density: xi over {len(pq)} forest pairs ({t_xi:.1f} s), "
-                      f"naive D (f={frac}) over {len(pq_d)} forest pairs ({t_d:.1f} s)"}
+def cpu_baseline(wl, n_forests, dmat_div):
+    """The oracle timed on this box's host cores on the bounded sample (about 10-30 s)."""
+    smp = OracleSample(wl, n_forests, dmat_div)
+    pairs, t_xi, t_d = smp.step()
+    one = smp.single_thread_xi()
+    return {"value": pairs / (t_xi + t_d), "unit": UNIT, "cores": smp.orc.num_threads(), "cpu": cpu_model(), "kind": "oracle",
+            "xi_pairs_per_s": smp.n_xi / t_xi, "dmat_pairs_per_s": smp.n_d / max(t_d, 1e-9),
+            "xi_pairs_per_s_single_thread": one,
+            "sample": smp.describe() + f" (xi {t_xi:.1f} s, D {t_d:.1f} s; single-thread xi on 1/16 of the forest pairs)"}
 
 
 def main():
@@ -180,14 +215,18 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=os.environ.get("LYA_BENCH_WORKLOAD", "cfg4"), choices=list(WORKLOADS))
+    ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
+                    help="N > 1: strong = ONE catalogue, its forest-pair list split over the ranks, one all-reduce of the "
+                         "numerators (DESIGN.md section 8); weak = an independent catalogue per rank, no data-path collective")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-dmat", action="store_true")
-    ap.add_argument("--ref-forests", type=int, default=8000)
-    ap.add_argument("--ref-dmat-div", type=int, default=50)
-    ap.add_argument("--cpu-forests", type=int, default=12000)
+    ap.add_argument("--cpu-forests", type=int, default=10000, help="forests of the bounded oracle sample (both oracle legs)")
+    ap.add_argument("--cpu-dmat-div", type=int, default=20, help="naive D runs on 1/N of the sample's forest pairs")
     ap.add_argument("--forests", type=int, default=0,
                     help="profiling only: a shaped sub-catalogue of this many forests (same sky density)")
+    ap.add_argument("--fine", type=int, default=1,
+                    help="NEXT-3 shapes: divide the pixel step by this factor (gen.make_config(fine=...)); throughput only")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -211,19 +250,27 @@ def main():
     wl = WORKLOADS[args.workload]
     frac = 0.0 if wl["cfg"] == 0 else 0.99
     mseed = gen.mask_seed(wl["mask_cfg"])
-    # weak scaling: every rank owns an independent catalogue of the same shape (seed + rank)
-    f = gen.make_config(wl["cfg"], n_forest=args.forests or None,
-                        seed=shard.rank_seed(gen.SEED_BASE + wl["cfg"], rank))
+    strong = world > 1 and args.scaling == "strong"
+    # strong: every rank holds the SAME catalogue; weak: an independent catalogue of the same shape per rank
+    f = gen.make_config(wl["cfg"], n_forest=args.forests or None, fine=args.fine,
+                        seed=None if strong else shard.rank_seed(gen.SEED_BASE + wl["cfg"], rank))
     ctx = B.Context(f"cuda:{local}")
     d = B.DeviceForests(f, device=f"cuda:{local}")
     b = B.binning()
     do_d = not args.no_dmat
+    lens = d.pix_off[1:] - d.pix_off[:-1]
 
     def step():
+        """One pass of the hot path: neighbours -> (chunk of the list) -> plan -> xi -> D (-> all-reduce + division)."""
+        if strong:
+            r = shard.sharded_step(ctx, d, b, frac, mseed, rank, world, do_dmat=do_d, lens=lens)
+            return dict(stats=r["stats_xi"]), (dict(stats=r["stats_dmat"]) if do_d else None)
         pairs = ctx.lya_neighbours(d, b)
-        x = ctx.lya_xi2pcf(d, b, pairs)
-        dm = ctx.lya_dmat(d, b, pairs, frac, mseed, want_Dn=False) if do_d else None
+        plan = ctx.lya_plan_create(d, b, pairs, want_xi=True, want_dmat=do_d)
         pairs.free()
+        x = ctx.lya_xi2pcf_plan(plan)
+        dm = ctx.lya_dmat_plan(plan, frac, mseed, want_Dn=False) if do_d else None
+        plan.free()
         return x, dm
 
     def barrier():
@@ -239,20 +286,20 @@ def main():
     if rank == 0:
         sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = B.launch_count()
     ev0.record()
-    ms_xi, ms_dm, launches = [], [], 0
+    ms_xi, ms_dm = [], []
     pairs_total = 0
     for _ in range(args.steps):
         x, dm = step()
         ms_xi.append(x["stats"]["ms_main"])
         pairs_total += x["stats"]["n_binned"]
-        launches += 15 + 13          # lya_neighbours: 15 kernels; lya_xi2pcf: validate, prep (5), bucketing (5), k_xi_fast, finalize
         if dm is not None:
             ms_dm.append(dm["stats"]["ms_main"])
             pairs_total += dm["stats"]["n_binned"]
-            launches += 13           # lya_dmat: validate, prep (5), bucketing (5), k_dmat_fast, normalise
     ev1.record()
     barrier()
+    launches = B.launch_count() - launches0          # kernels this rank's library launched inside the timed region
     clocks = sampler.stop() if rank == 0 else None
     ms = ev0.elapsed_time(ev1)
     ms, pairs_all = shard.aggregate(ms, float(pairs_total), device=f"cuda:{local}")
@@ -280,7 +327,7 @@ def main():
         d2h = sum(v.nbytes for v in out.values())
         ctx.lya_run_host(hf, b, True, do_d, frac, mseed, out=dict(out))
         barrier()
-        n_e2e = max(1, min(args.steps, 2))
+        n_e2e = max(1, min(args.steps, 5))
         t0 = time.perf_counter()
         pe = 0
         for _ in range(n_e2e):
@@ -288,9 +335,14 @@ def main():
             pe += r["stats_xi"]["n_binned"] + (r["stats_dmat"]["n_binned"] if do_d else 0)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        dt, pe = shard.aggregate(dt, float(pe), device=f"cuda:{local}")
+        if strong:                                    # every rank ran the whole catalogue: the job's e2e is one rank's
+            dtm, _ = shard.aggregate(dt, 0.0, device=f"cuda:{local}")
+            dt = dtm
+        else:
+            dt, pe = shard.aggregate(dt, float(pe), device=f"cuda:{local}")
         e2e = {"value": pe / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-               "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3}
+               "steps": n_e2e, "ms_per_step": dt / n_e2e * 1e3,
+               "note": "lya_run_host on one rank's whole catalogue (host buffers are not sharded)" if strong else None}
 
     if rank == 0:
         peaks, peak_kind = measured_peaks()
@@ -322,26 +374,34 @@ def main():
                       "unit": "Tops/s (fp64 lane-operations)", "frac": alg_d / t_dm / peak_alu, "traffic": None,
                       "peak_source": peak_src,
                       "scatter_adds_per_s": sd["n_scatter"] / t_dm,
-                      "frac_of_measured_l2_red_peak": sd["n_scatter"] / t_dm / mp["l2_red64"]}
+                      "frac_of_measured_l2_red_peak": sd["n_scatter"] / t_dm / mp["l2_red64"] if mp.get("l2_red64") else None,
+                      "evaluated_per_scanned": sd["n_evaluated"] / max(sd["n_binned"], 1)}
             extra["dmat"] = {"scanned_pairs_per_s": sd["n_binned"] / t_dm, "kept_pairs_per_s": sd["n_kept"] / t_dm,
                              "ms": t_dm * 1e3, "n_kept": sd["n_kept"], "n_scatter": sd["n_scatter"], "roofline": roof_d}
             if t_dm > t_xi:
                 roof = roof_d
+        if world == 1:
+            par = "one GPU"
+        elif strong:
+            par = f"one catalogue, forest-pair list split over {world} ranks by sum n_p n_q, one all-reduce of S,W,N / Dn,Wd"
+        else:
+            par = f"independent catalogue per GPU x{world}, no data-path collective"
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "description": wl["desc"], "n_forest": f.n_forest, "n_pix": f.n_pix,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if strong else "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload + (f" fine={args.fine}" if args.fine != 1 else ""), "description": wl["desc"],
+                       "n_forest": f.n_forest, "n_pix": f.n_pix,
                        "bins": "50x50x4Mpc/h", "reject_fraction": frac, "dmat": do_d,
                        "l2": ("catalogue %.2f GB + forest-pair list %.2f GB per step vs 126 MB of L2 (%s); Dn (50 MB) "
                               "re-zeroed every step") % (f.n_pix * 32 / 1e9, sx["n_forest_pairs"] * 8 / 1e9,
                                                          "larger than L2" if f.n_pix * 32 + sx["n_forest_pairs"] * 8 > 126e6
                                                          else "NOT larger than L2: use the default workload for a valid number"),
-                       "parallelism": f"independent catalogue per GPU x{world}"},
-            "roofline": roof, "clocks": clocks, "gpu_launches": launches, "e2e": e2e, **extra,
+                       "parallelism": par},
+            "roofline": roof, "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, **extra,
         }
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = cpu_baseline(wl, args.cpu_forests)
+            line["cpu_baseline"] = cpu_baseline(wl, args.cpu_forests, args.cpu_dmat_div)
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

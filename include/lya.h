@@ -43,6 +43,7 @@ extern "C" {
 
 typedef struct lya_ctx lya_ctx;      /* opaque: device, stream, scratch, last error */
 typedef struct lya_pairs lya_pairs;  /* opaque, library-owned device forest-pair list */
+typedef struct lya_plan lya_plan;    /* opaque: prepared catalogue + bucket-sorted pair list (see lya_plan_create) */
 
 typedef enum {
     LYA_OK = 0,
@@ -102,6 +103,10 @@ lya_status  lya_create(lya_ctx **ctx, int device, void *cuda_stream);
 void        lya_destroy(lya_ctx *ctx);
 const char *lya_last_error(const lya_ctx *ctx);   /* host string, owned by ctx */
 const char *lya_version(void);
+/* Number of CUDA kernels this library has launched in the process so far (all contexts; every launch site
+ * counts itself; one ctx per host thread, so no synchronisation).  bench.py reports the difference over
+ * its timed region as gpu_launches. */
+uint64_t    lya_launch_count(void);
 
 /* Explicit, per-ctx switches (there are no environment variables or global flags).
  *   LYA_OPT_FORCE_GENERIC     0 (default) / 1: route EVERY forest pair to the generic kernels (block-level
@@ -186,6 +191,26 @@ lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const lya_binning 
 lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                     const lya_pairs *pairs, double reject_fraction, uint64_t seed,
                     double *D, double *Dn, double *Wd, lya_stats *stats);
+
+/* ---- plans: prepare once, run stages 2 and 3+4 on the same catalogue and list -------------------- */
+/* lya_xi2pcf and lya_dmat each validate the catalogue, build a padded 16-byte-aligned copy of it (with the
+ * per-pixel products of eq. 2.4 / eq. 2.7) and bucket-sort the forest-pair list by r_perp column before
+ * their pair kernel runs.  A plan does that ONCE for a (catalogue, binning, pair list) triple:
+ *   lya_plan_create(..., want_xi, want_dmat, &plan);  lya_xi2pcf_plan(plan, ...);  lya_dmat_plan(plan, ...);
+ * give exactly the results of lya_xi2pcf / lya_dmat on the same arguments (those two calls are wrappers
+ * that build a throw-away plan).  want_xi needs delta, want_dmat needs loglam.  The plan keeps the caller's
+ * device pointers: the catalogue arrays must stay alive and unchanged until lya_plan_free; the pair list is
+ * copied and may be freed.  lya_set_option(LYA_OPT_FORCE_GENERIC) is read at creation time.
+ * Device memory: about 8 bytes per listed forest pair plus 24 (xi) / 48 (D) bytes per pixel.
+ * lya_plan_create synchronises the ctx stream; errors as for lya_xi2pcf / lya_dmat (a degenerate listed
+ * forest is reported by lya_dmat_plan, not at creation, so that a plan for both stages still serves xi). */
+lya_status lya_plan_create(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                           int want_xi, int want_dmat, lya_plan **out);
+void       lya_plan_free(lya_ctx *ctx, lya_plan *plan);
+lya_status lya_xi2pcf_plan(lya_ctx *ctx, const lya_plan *plan,
+                           double *S, double *W, uint64_t *N, double *xi, lya_stats *stats);
+lya_status lya_dmat_plan(lya_ctx *ctx, const lya_plan *plan, double reject_fraction, uint64_t seed,
+                         double *D, double *Dn, double *Wd, lya_stats *stats);
 
 /* ---- final divisions on already-summed numerators (multi-GPU) ----------- */
 /* Every output above is an additive accumulator before its final division, so a catalogue's

@@ -13,9 +13,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblya.so")
 
-EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_set_option", "lya_neighbours",
+EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_launch_count", "lya_set_option", "lya_neighbours",
            "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
-           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host", "lya_xi_normalise", "lya_dmat_normalise"]
+           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host", "lya_xi_normalise", "lya_dmat_normalise",
+           "lya_plan_create", "lya_plan_free", "lya_xi2pcf_plan", "lya_dmat_plan"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
           4: "LYA_ERR_CAPACITY", 5: "LYA_ERR_OOM", 6: "LYA_ERR_CUDA", 7: "LYA_ERR_UNIMPLEMENTED"}
@@ -63,6 +64,7 @@ def load():
         lib.lya_last_error.restype = C.c_char_p
         lib.lya_last_error.argtypes = [C.c_void_p]
         lib.lya_version.restype = C.c_char_p
+        lib.lya_launch_count.restype = C.c_uint64
         lib.lya_pairs_count.restype = C.c_int64
         lib.lya_pairs_count.argtypes = [C.c_void_p]
         lib.lya_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
@@ -83,11 +85,23 @@ def load():
         lib.lya_run_host.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_int, C.c_int,
                                      C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.POINTER(C.c_int64), C.POINTER(CStats), C.POINTER(CStats)]
+        lib.lya_plan_create.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p, C.c_int, C.c_int,
+                                        C.POINTER(C.c_void_p)]
+        lib.lya_plan_free.argtypes = [C.c_void_p, C.c_void_p]
+        lib.lya_plan_free.restype = None
+        lib.lya_xi2pcf_plan.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
+        lib.lya_dmat_plan.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                      C.POINTER(CStats)]
         lib.lya_xi_normalise.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.lya_dmat_normalise.argtypes = [C.c_void_p, C.POINTER(CBinning), C.c_void_p, C.c_void_p, C.c_void_p]
         lib.lya_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         _lib = lib
     return _lib
+
+
+def launch_count() -> int:
+    """Kernels launched by liblya.so in this process so far."""
+    return int(load().lya_launch_count())
 
 
 def binning(rpar_max=200.0, rperp_max=200.0, n_par=50, n_perp=50) -> CBinning:
@@ -137,6 +151,24 @@ class Pairs:
     def free(self):
         if self.handle is not None:
             load().lya_pairs_free(self.ctx.h, self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Plan:
+    """lya_plan handle (prepared catalogue + bucketed pair list); keeps the DeviceForests alive."""
+
+    def __init__(self, ctx, handle, forests, b):
+        self.ctx, self.handle, self.forests, self.b = ctx, handle, forests, b
+
+    def free(self):
+        if self.handle is not None:
+            load().lya_plan_free(self.ctx.h, self.handle)
             self.handle = None
 
     def __del__(self):
@@ -208,6 +240,35 @@ class Context:
         self._check(load().lya_pairs_subsample(self.h, pairs.handle, float(reject_fraction), C.c_uint64(seed),
                                                C.byref(h), C.byref(n)))
         return Pairs(self, h, n.value)
+
+    # ---- plans ----
+    def lya_plan_create(self, forests: DeviceForests, b: CBinning, pairs: Pairs, want_xi=True, want_dmat=True) -> Plan:
+        h = C.c_void_p()
+        cf = forests.c()
+        self._check(load().lya_plan_create(self.h, C.byref(cf), C.byref(b), pairs.handle, int(want_xi), int(want_dmat),
+                                           C.byref(h)))
+        return Plan(self, h, forests, b)
+
+    def lya_xi2pcf_plan(self, plan: Plan):
+        torch = self.torch
+        nb = plan.b.n_par * plan.b.n_perp
+        S = torch.empty(nb, dtype=torch.float64, device=self.device)
+        W = torch.empty_like(S); xi = torch.empty_like(S)
+        N = torch.empty(nb, dtype=torch.int64, device=self.device)      # uint64 payload
+        stats = CStats()
+        self._check(load().lya_xi2pcf_plan(self.h, plan.handle, _ptr(S), _ptr(W), _ptr(N), _ptr(xi), C.byref(stats)))
+        return dict(S=S, W=W, N=N, xi=xi, stats=stats.as_dict())
+
+    def lya_dmat_plan(self, plan: Plan, reject_fraction: float, seed: int, want_Dn=True, want_D=True):
+        torch = self.torch
+        nb = plan.b.n_par * plan.b.n_perp
+        D = torch.empty((nb, nb), dtype=torch.float64, device=self.device) if want_D else None
+        Dn = torch.empty((nb, nb), dtype=torch.float64, device=self.device) if want_Dn else None
+        Wd = torch.empty(nb, dtype=torch.float64, device=self.device)
+        stats = CStats()
+        self._check(load().lya_dmat_plan(self.h, plan.handle, float(reject_fraction), C.c_uint64(seed),
+                                         _ptr(D), _ptr(Dn), _ptr(Wd), C.byref(stats)))
+        return dict(D=D, Dn=Dn, Wd=Wd, stats=stats.as_dict())
 
     # ---- lya_xi2pcf ----
     def lya_xi2pcf(self, forests: DeviceForests, b: CBinning, pairs: Pairs):

@@ -65,7 +65,8 @@ __global__ void k_forest_scalars(const int64_t *pix_off, const double *w, const 
     double lb = (sw > 0.0) ? swl / sw : 0.0;
     double v = 0.0;
     for (int64_t k = a; k < b; ++k) { double u = loglam[k] - lb; v += w[k] * u * u; }
-    bool ok = (sw > 0.0) && (v > 0.0);
+    const double tiny = 1e-12 * fabs(lb);                  // reading R-7: all weighted L equal up to rounding of L - Lbar
+    bool ok = (sw > 0.0) && (v > sw * tiny * tiny);
     invS[p] = ok ? 1.0 / sw : nan("");
     lbar[p] = lb;
     invV[p] = ok ? 1.0 / v : nan("");
@@ -394,7 +395,7 @@ extern "C" lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, 
     auto drop = [&]() { cudaFree(flag); cudaFree(pos); cudaFree(tmp); };
     if (e != cudaSuccess) { drop(); free(pl); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_pairs_subsample)"); }
     const unsigned blocks = (unsigned)((n + 255) / 256);
-    k_fp_flag<<<blocks, 256, 0, s>>>(pairs->pq, n, seed, thr, flag);
+    { k_fp_flag<<<blocks, 256, 0, s>>>(pairs->pq, n, seed, thr, flag); lya_note_launch(); }
     e = lya_exclusive_scan(flag, pos, n, tmp, s);
     unsigned long long total = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&total, pos + n, sizeof(total), cudaMemcpyDeviceToHost, s);
@@ -404,7 +405,7 @@ extern "C" lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, 
     if (total > 0) {
         e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)total);
         if (e == cudaSuccess) {
-            k_fp_compact<<<blocks, 256, 0, s>>>(pairs->pq, n, flag, pos, pl->pq);
+            { k_fp_compact<<<blocks, 256, 0, s>>>(pairs->pq, n, flag, pos, pl->pq); lya_note_launch(); }
             e = cudaGetLastError();
             if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         }
@@ -415,54 +416,34 @@ extern "C" lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, 
     return LYA_OK;
 }
 
-extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
-                               double reject_fraction, uint64_t seed, double *D, double *Dn_out, double *Wd_out,
-                               lya_stats *stats)
+static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fraction, uint64_t seed,
+                           double *D, double *Dn_out, double *Wd_out, lya_stats *stats)
 {
     if (!ctx) return LYA_ERR_INVALID_ARG;
-    if (!pairs) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat: pairs is NULL");
+    if (!pl) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat: plan is NULL");
+    if (!pl->has_dmat) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat: the plan was created without want_dmat");
     if (!D && !Dn_out) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat: need D or Dn");
     if (!(reject_fraction >= 0.0 && reject_fraction <= 1.0))
         return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat: reject_fraction must be in [0,1]");
-    lya_status st = lya_check_binning(ctx, b);
-    if (st) return st;
+    const lya_forests *f = &pl->f;
+    const lya_binning *b = &pl->b;
     if (b->n_par > H_SLOTS) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: n_par above %d", H_SLOTS);
-    if ((int64_t)b->n_par * b->n_perp > 4096) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: more than 4096 bins");
-    st = lya_check_forests_host(ctx, f, true, false, true);
-    if (st) return st;
-    if (f->n_forest > 0 && !(f->ux && f->uy && f->uz))
-        return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat needs ux,uy,uz (device)");
+    if (pl->listed_degenerate)
+        return lya_fail(ctx, LYA_ERR_DEGENERATE_FOREST, "a listed forest has sum w == 0 or sum w (L-Lbar)^2 == 0");
     LYA_CUDA(cudaSetDevice(ctx->device));
-    int max_len = 0;
-    st = lya_validate_forests(ctx, f, false, true, &max_len);
-    if (st) return st;
 
     const int nb = b->n_par * b->n_perp;
     cudaStream_t s = ctx->stream;
-    const BinParams bp = lya_make_binparams(b);
-    const bool use_fast = pairs->n > 0 && b->n_par * LYA_NCOL + 1 <= FD_SLOTS && b->n_perp + 2 <= 256 &&
-                          !ctx->force_generic;
+    const BinParams bp = pl->bp;
+    const bool use_fast = pl->use_fast;
+    const LyaBuckets &bk = pl->bk;
     double *scal = NULL, *Dn = NULL, *Wd = NULL;          // internal accumulators (transposed bin order)
-    bool own_Dn = false, own_Wd = false;
     const int64_t nf = f->n_forest;
-    LyaPrep prep;
-    LyaBuckets bk;
-    memset(&prep, 0, sizeof(prep));
-    memset(&bk, 0, sizeof(bk));
-    auto cleanup = [&]() { cudaFree(scal); if (own_Dn) cudaFree(Dn); if (own_Wd) cudaFree(Wd); lya_prep_free(&prep); lya_buckets_free(&bk); };
+    auto cleanup = [&]() { cudaFree(scal); cudaFree(Dn); cudaFree(Wd); };
     cudaEventRecord(ctx->ev[3], s);
-    if (use_fast) {
-        st = lya_prep_build(ctx, f, false, true, &prep);
-        if (st) return st;
-        cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
-        st = lya_bucket_pairs(ctx, &prep, &bp, pairs, 0, &bk);
-        if (st) { cleanup(); return st; }
-        if (bk.bad_pair == LYA_DEV_DEGENERATE) { cleanup(); return lya_fail(ctx, LYA_ERR_DEGENERATE_FOREST, "a listed forest has sum w == 0 or sum w (L-Lbar)^2 == 0"); }
-        if (bk.bad_pair) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
-    }
     cudaError_t e = cudaMalloc(&scal, sizeof(double) * 3 * (size_t)(nf ? nf : 1));
-    if (e == cudaSuccess && !Dn) { e = cudaMalloc(&Dn, sizeof(double) * (size_t)nb * nb); own_Dn = (e == cudaSuccess); if (!own_Dn) Dn = NULL; }
-    if (e == cudaSuccess && !Wd) { e = cudaMalloc(&Wd, sizeof(double) * (size_t)nb); own_Wd = (e == cudaSuccess); if (!own_Wd) Wd = NULL; }
+    if (e == cudaSuccess) e = cudaMalloc(&Dn, sizeof(double) * (size_t)nb * nb);
+    if (e == cudaSuccess) e = cudaMalloc(&Wd, sizeof(double) * (size_t)nb);
     if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_dmat)"); }
     cudaMemsetAsync(Dn, 0, sizeof(double) * (size_t)nb * nb, s);
     cudaMemsetAsync(Wd, 0, sizeof(double) * (size_t)nb, s);
@@ -479,8 +460,8 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.loglam = f->loglam;
     P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
     P.f_invS = scal; P.f_lbar = scal + nf; P.f_invV = scal + 2 * nf;
-    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pairs->pq;
-    P.n_pairs = use_fast ? bk.n_generic : pairs->n;
+    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pl->pq;
+    P.n_pairs = use_fast ? bk.n_generic : pl->n_pairs;
     P.n_forest = nf;
     P.bp = bp;
     P.seed = seed; P.thr = thr;
@@ -492,13 +473,13 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     cudaEventRecord(ctx->ev[0], s);
     if (use_fast && bk.n_fast > 0) {
         DmFastParams F;
-        F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp; F.seed = seed; F.thr = thr;
+        F.prep = pl->prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp; F.seed = seed; F.thr = thr;
         F.Dn = Dn; F.Wd = Wd; F.counters = ctx->d_counters;
         const size_t fsmem = FD_SMEM_BYTES;
         const int fgrid = ctx->sm_count;
         auto launch = [&](auto kern) {
             cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (le == cudaSuccess) kern<<<fgrid, FD_THREADS, fsmem, s>>>(F);
+            if (le == cudaSuccess) { kern<<<fgrid, FD_THREADS, fsmem, s>>>(F); lya_note_launch(); }
             return le;
         };
         if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_fast<true, true>) : launch(k_dmat_fast<false, true>);
@@ -507,27 +488,27 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_dmat_fast launch"); }
     }
     if (P.n_pairs > 0) {
-        k_forest_scalars<<<(unsigned)((nf + 127) / 128), 128, 0, s>>>(f->pix_off, f->w, f->loglam, nf, scal, scal + nf, scal + 2 * nf);
+        { k_forest_scalars<<<(unsigned)((nf + 127) / 128), 128, 0, s>>>(f->pix_off, f->w, f->loglam, nf, scal, scal + nf, scal + 2 * nf); lya_note_launch(); }
         const size_t smem = sizeof(DmWarpSmem) * DM_WARPS;
         int grid = ctx->sm_count * 2;
         if (P.bp.pow2) {
             e = cudaFuncSetAttribute(k_dmat<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e == cudaSuccess) k_dmat<true><<<grid, DM_THREADS, smem, s>>>(P);
+            if (e == cudaSuccess) { k_dmat<true><<<grid, DM_THREADS, smem, s>>>(P); lya_note_launch(); }
         } else {
             e = cudaFuncSetAttribute(k_dmat<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e == cudaSuccess) k_dmat<false><<<grid, DM_THREADS, smem, s>>>(P);
+            if (e == cudaSuccess) { k_dmat<false><<<grid, DM_THREADS, smem, s>>>(P); lya_note_launch(); }
         }
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_dmat launch"); }
     }
     cudaEventRecord(ctx->ev[1], s);
-    k_dmat_normalise<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, s>>>(Dn, Wd, bp, D, Dn_out, Wd_out);
+    { k_dmat_normalise<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, s>>>(Dn, Wd, bp, D, Dn_out, Wd_out); lya_note_launch(); }
     cudaEventRecord(ctx->ev[2], s);
     unsigned long long h[16];
     e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "lya_dmat"); }
-    const unsigned long long visited = use_fast ? bk.visited : h[1];
+    const unsigned long long visited = use_fast ? pl->visited : h[1];
     cleanup();
     switch ((unsigned)h[3]) {
     case LYA_DEV_OK: break;
@@ -539,7 +520,7 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
         return lya_fail(ctx, LYA_ERR_CUDA, "k_dmat_fast: %llu table entries had two holders (LYA_OPT_CHECK_HOLDERS)", h[10]);
     if (stats) {
         memset(stats, 0, sizeof(*stats));
-        stats->n_forest_pairs = (uint64_t)pairs->n;
+        stats->n_forest_pairs = (uint64_t)pl->n_pairs;
         stats->n_visited = visited;
         stats->n_evaluated = h[2];
         stats->n_kept = h[5];
@@ -551,6 +532,29 @@ extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_bin
     return LYA_OK;
 }
 
+extern "C" lya_status lya_dmat_plan(lya_ctx *ctx, const lya_plan *plan, double reject_fraction, uint64_t seed,
+                                    double *D, double *Dn, double *Wd, lya_stats *stats)
+{
+    return dmat_run(ctx, plan, reject_fraction, seed, D, Dn, Wd, stats);
+}
+
+extern "C" lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                               double reject_fraction, uint64_t seed, double *D, double *Dn_out, double *Wd_out,
+                               lya_stats *stats)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (!D && !Dn_out) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat: need D or Dn");
+    if (!(reject_fraction >= 0.0 && reject_fraction <= 1.0))
+        return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat: reject_fraction must be in [0,1]");
+    if (b && (int64_t)b->n_par * b->n_perp > 4096) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: more than 4096 bins");
+    lya_plan *pl = NULL;
+    lya_status st = lya_plan_create(ctx, f, b, pairs, 0, 1, &pl);
+    if (st) return st;
+    st = dmat_run(ctx, pl, reject_fraction, seed, D, Dn_out, Wd_out, stats);
+    lya_plan_free(ctx, pl);
+    return st;
+}
+
 extern "C" lya_status lya_dmat_normalise(lya_ctx *ctx, const lya_binning *b, const double *Dn, const double *Wd, double *D)
 {
     if (!ctx) return LYA_ERR_INVALID_ARG;
@@ -559,7 +563,7 @@ extern "C" lya_status lya_dmat_normalise(lya_ctx *ctx, const lya_binning *b, con
     if (!Dn || !Wd || !D) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat_normalise: NULL argument");
     LYA_CUDA(cudaSetDevice(ctx->device));
     const int nb = b->n_par * b->n_perp;
-    k_dmat_divide<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, ctx->stream>>>(Dn, Wd, nb, D);
+    { k_dmat_divide<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, ctx->stream>>>(Dn, Wd, nb, D); lya_note_launch(); }
     LYA_CUDA(cudaGetLastError());
     return LYA_OK;
 }

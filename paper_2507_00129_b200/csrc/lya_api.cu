@@ -5,6 +5,9 @@
 #include <stdlib.h>
 #include "lya_internal.cuh"
 
+unsigned long long g_lya_launches = 0;
+extern "C" uint64_t lya_launch_count(void) { return g_lya_launches; }
+
 extern "C" const char *lya_version(void) { return "lya-b200 0.1 (sm_100a)"; }
 
 lya_status lya_fail(lya_ctx *ctx, lya_status st, const char *fmt, ...)
@@ -158,7 +161,7 @@ lya_status lya_validate_forests(lya_ctx *ctx, const lya_forests *f, bool need_de
     LYA_CUDA(cudaMemsetAsync(ctx->d_counters + 8, 0, 2 * sizeof(unsigned long long), ctx->stream));
     int threads = 128;
     int64_t blocks = (f->n_forest + threads - 1) / threads;
-    k_validate<<<(unsigned)blocks, threads, 0, ctx->stream>>>(*f, need_delta, need_loglam, d_err, d_maxlen);
+    { k_validate<<<(unsigned)blocks, threads, 0, ctx->stream>>>(*f, need_delta, need_loglam, d_err, d_maxlen); lya_note_launch(); }
     LYA_CUDA(cudaGetLastError());
     unsigned long long h[2];
     LYA_CUDA(cudaMemcpyAsync(h, ctx->d_counters + 8, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
@@ -201,7 +204,7 @@ extern "C" lya_status lya_pairs_import(lya_ctx *ctx, const int32_t *pq, int64_t 
         unsigned *d_err = (unsigned *)(ctx->d_counters + 8);
         cudaMemsetAsync(d_err, 0, sizeof(unsigned long long), ctx->stream);
         int threads = 256;
-        k_import_pairs<<<(unsigned)((n_pairs + threads - 1) / threads), threads, 0, ctx->stream>>>(pq, pl->pq, n_pairs, d_err);
+        { k_import_pairs<<<(unsigned)((n_pairs + threads - 1) / threads), threads, 0, ctx->stream>>>(pq, pl->pq, n_pairs, d_err); lya_note_launch(); }
         unsigned long long h = 0;
         e = cudaMemcpyAsync(&h, d_err, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
@@ -281,14 +284,19 @@ extern "C" lya_status lya_run_host(lya_ctx *ctx, const lya_forests *fh, const ly
     st = lya_neighbours(ctx, &fd, b, &pairs, &n_pairs);
     if (st) return st;
     if (n_pairs_out) *n_pairs_out = n_pairs;
+    lya_plan *plan = NULL;
+    st = lya_plan_create(ctx, &fd, b, pairs, do_xi != 0, do_dmat != 0, &plan);
+    lya_pairs_free(ctx, pairs);                       // (the plan holds its own bucket-sorted copy)
+    pairs = NULL;
+    if (st) return st;
     if (do_xi) {
         cudaError_t e = dS.alloc(8 * nb);
         if (e == cudaSuccess) e = dW.alloc(8 * nb);
         if (e == cudaSuccess) e = dN.alloc(8 * nb);
         if (e == cudaSuccess) e = dxi.alloc(8 * nb);
-        if (e != cudaSuccess) { lya_pairs_free(ctx, pairs); return lya_cuda_fail(ctx, e, "cudaMalloc(xi outputs)"); }
-        st = lya_xi2pcf(ctx, &fd, b, pairs, (double *)dS.p, (double *)dW.p, (uint64_t *)dN.p, (double *)dxi.p, stats_xi);
-        if (st) { lya_pairs_free(ctx, pairs); return st; }
+        if (e != cudaSuccess) { lya_plan_free(ctx, plan); return lya_cuda_fail(ctx, e, "cudaMalloc(xi outputs)"); }
+        st = lya_xi2pcf_plan(ctx, plan, (double *)dS.p, (double *)dW.p, (uint64_t *)dN.p, (double *)dxi.p, stats_xi);
+        if (st) { lya_plan_free(ctx, plan); return st; }
         if (S) cudaMemcpyAsync(S, dS.p, 8 * nb, cudaMemcpyDeviceToHost, s);
         if (W) cudaMemcpyAsync(W, dW.p, 8 * nb, cudaMemcpyDeviceToHost, s);
         if (N) cudaMemcpyAsync(N, dN.p, 8 * nb, cudaMemcpyDeviceToHost, s);
@@ -297,14 +305,15 @@ extern "C" lya_status lya_run_host(lya_ctx *ctx, const lya_forests *fh, const ly
     if (do_dmat) {
         cudaError_t e = dD.alloc(8 * nb * nb);
         if (e == cudaSuccess) e = dWd.alloc(8 * nb);
-        if (e != cudaSuccess) { lya_pairs_free(ctx, pairs); return lya_cuda_fail(ctx, e, "cudaMalloc(D outputs)"); }
-        st = lya_dmat(ctx, &fd, b, pairs, reject_fraction, seed, (double *)dD.p, NULL, (double *)dWd.p, stats_dmat);
-        if (st) { lya_pairs_free(ctx, pairs); return st; }
+        if (e != cudaSuccess) { lya_plan_free(ctx, plan); return lya_cuda_fail(ctx, e, "cudaMalloc(D outputs)"); }
+        st = lya_dmat_plan(ctx, plan, reject_fraction, seed, (double *)dD.p, NULL, (double *)dWd.p, stats_dmat);
+        if (st) { lya_plan_free(ctx, plan); return st; }
         if (D) cudaMemcpyAsync(D, dD.p, 8 * nb * nb, cudaMemcpyDeviceToHost, s);
         if (Wd) cudaMemcpyAsync(Wd, dWd.p, 8 * nb, cudaMemcpyDeviceToHost, s);
     }
     cudaError_t e = cudaStreamSynchronize(s);
-    lya_pairs_free(ctx, pairs);
+    lya_plan_free(ctx, plan);
+
     if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "lya_run_host");
     return LYA_OK;
 }

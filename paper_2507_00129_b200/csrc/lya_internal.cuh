@@ -34,6 +34,10 @@ struct lya_pairs {
 enum { LYA_DEV_OK = 0, LYA_DEV_BAD_OFFSETS = 1, LYA_DEV_NONFINITE = 2, LYA_DEV_UNSORTED = 3,
        LYA_DEV_BAD_PAIR = 4, LYA_DEV_DEGENERATE = 5, LYA_DEV_TOO_LONG = 6 };
 
+// process-wide count of kernel launches made by the library (lya_launch_count): every launch site notes itself
+extern unsigned long long g_lya_launches;
+static inline void lya_note_launch() { ++g_lya_launches; }
+
 lya_status lya_fail(lya_ctx *ctx, lya_status st, const char *fmt, ...);
 lya_status lya_cuda_fail(lya_ctx *ctx, cudaError_t e, const char *what);
 lya_status lya_check_binning(lya_ctx *ctx, const lya_binning *b);
@@ -123,6 +127,25 @@ static inline BinParams lya_make_binparams(const lya_binning *b)
               bp.inv_par * b->rpar_max == (double)b->n_par && bp.inv_perp * b->rperp_max == (double)b->n_perp;
     return bp;
 }
+
+// ---- plan (prep.cu): everything the pair kernels need that depends only on (catalogue, binning, pair list):
+// the validated catalogue, its padded copy and the bucket-sorted forest-pair list.  Built once, used by
+// lya_xi2pcf_plan / lya_dmat_plan any number of times (lya_xi2pcf / lya_dmat build a throw-away one).
+#define LYA_FAST_NPAR_MAX 50         // r_par rows a warp-private table holds (both fast kernels)
+struct lya_plan {
+    lya_forests f;                  // the caller's arrays (must stay alive and unchanged while the plan is used)
+    lya_binning b;
+    BinParams bp;
+    bool has_xi, has_dmat;          // which catalogue arrays were prepared
+    bool use_fast;                  // bucketed list + fast kernels (else: every pair through the generic kernels)
+    LyaPrep prep;
+    LyaBuckets bk;                  // use_fast: sorted list [fast | generic | nothing in grid]
+    int32_t *pq;                    // !use_fast: a copy of the pair list
+    int64_t n_pairs;
+    unsigned long long visited;     // sum n_p n_q over the list (use_fast)
+    int listed_degenerate;          // has_dmat: a listed forest is degenerate for eq. 2.7
+    int max_len;
+};
 
 #ifdef __CUDACC__
 // ---- geometry, one separately rounded binary64 operation each (readings G2-G6) ----

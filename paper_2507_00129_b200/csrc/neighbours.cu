@@ -99,9 +99,9 @@ cudaError_t exclusive_scan(const unsigned *in, unsigned long long *out, int64_t 
     if (nblocks == 0) {
         return cudaMemsetAsync(out, 0, sizeof(unsigned long long), s);
     }
-    k_scan_block<<<(unsigned)nblocks, SCAN_THREADS, 0, s>>>(in, out, tmp, n);
-    k_scan_sums<<<1, 1024, 0, s>>>(tmp, nblocks, tmp + nblocks);
-    k_scan_add<<<(unsigned)nblocks, SCAN_THREADS, 0, s>>>(out, tmp, n, tmp + nblocks);
+    { k_scan_block<<<(unsigned)nblocks, SCAN_THREADS, 0, s>>>(in, out, tmp, n); lya_note_launch(); }
+    { k_scan_sums<<<1, 1024, 0, s>>>(tmp, nblocks, tmp + nblocks); lya_note_launch(); }
+    { k_scan_add<<<(unsigned)nblocks, SCAN_THREADS, 0, s>>>(out, tmp, n, tmp + nblocks); lya_note_launch(); }
     return cudaGetLastError();
 }
 
@@ -296,7 +296,7 @@ extern "C" lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const l
     unsigned long long init = 0x7ff0000000000000ULL;   // +inf
     cudaError_t e = cudaMemcpyAsync(d_min, &init, sizeof(init), cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "init"); }
-    k_prep<<<nblk, T, 0, s>>>(*f, ux, uy, uz, chimin, d_min);
+    { k_prep<<<nblk, T, 0, s>>>(*f, ux, uy, uz, chimin, d_min); lya_note_launch(); }
     unsigned long long min_bits = 0;
     e = cudaMemcpyAsync(&min_bits, d_min, sizeof(min_bits), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
@@ -322,21 +322,21 @@ extern "C" lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const l
     cudaMemsetAsync(hist, 0, sizeof(unsigned) * n_cells, s);
     cudaMemsetAsync(cursor, 0, sizeof(unsigned) * n_cells, s);
 
-    k_cell_hist<<<nblk, T, 0, s>>>(ux, uy, uz, chimin, n, G, cell_of, hist);
+    { k_cell_hist<<<nblk, T, 0, s>>>(ux, uy, uz, chimin, n, G, cell_of, hist); lya_note_launch(); }
     e = exclusive_scan(hist, cell_start, n_cells, scan_tmp, s);
     if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "cell scan"); }
-    k_cell_scatter<<<nblk, T, 0, s>>>(cell_of, n, cell_start, cursor, sorted_id);
-    k_cell_sort<<<(unsigned)((n_cells + T - 1) / T), T, 0, s>>>(cell_start, n_cells, sorted_id);
+    { k_cell_scatter<<<nblk, T, 0, s>>>(cell_of, n, cell_start, cursor, sorted_id); lya_note_launch(); }
+    { k_cell_sort<<<(unsigned)((n_cells + T - 1) / T), T, 0, s>>>(cell_start, n_cells, sorted_id); lya_note_launch(); }
     unsigned long long m_ull = 0;
     e = cudaMemcpyAsync(&m_ull, cell_start + n_cells, sizeof(m_ull), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "cell sort"); }
     const int64_t m = (int64_t)m_ull;                            // non-empty forests
     if (m < 2) { *out = pl; return LYA_OK; }
-    k_gather_sorted<<<(unsigned)((m + T - 1) / T), T, 0, s>>>(sorted_id, m, ux, uy, uz, chimin, sf);
+    { k_gather_sorted<<<(unsigned)((m + T - 1) / T), T, 0, s>>>(sorted_id, m, ux, uy, uz, chimin, sf); lya_note_launch(); }
 
     const unsigned wblk = (unsigned)((m * 32 + T - 1) / T);
-    k_pairs<false><<<wblk, T, 0, s>>>(sf, m, cell_start, G, b->rperp_max, counts, NULL, NULL);
+    { k_pairs<false><<<wblk, T, 0, s>>>(sf, m, cell_start, G, b->rperp_max, counts, NULL, NULL); lya_note_launch(); }
     e = exclusive_scan(counts, offsets, m, scan_tmp, s);
     if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "pair scan"); }
     unsigned long long total = 0;
@@ -348,7 +348,7 @@ extern "C" lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const l
     if (total > 0) {
         e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)total);
         if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "cudaMalloc(pair list)"); }
-        k_pairs<true><<<wblk, T, 0, s>>>(sf, m, cell_start, G, b->rperp_max, NULL, offsets, pl->pq);
+        { k_pairs<true><<<wblk, T, 0, s>>>(sf, m, cell_start, G, b->rperp_max, NULL, offsets, pl->pq); lya_note_launch(); }
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) { cudaFree(pl->pq); free(pl); return lya_cuda_fail(ctx, e, "k_pairs<fill>"); }

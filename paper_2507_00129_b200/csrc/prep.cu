@@ -196,7 +196,7 @@ lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool
     if (e == cudaSuccess) e = cudaMalloc(&tmp, sizeof(unsigned long long) * (size_t)(n / 2048 + 4));
     if (e != cudaSuccess) { cudaFree(padlen); cudaFree(off2); return lya_cuda_fail(ctx, e, "cudaMalloc(prep scratch)"); }
     auto drop = [&]() { cudaFree(padlen); cudaFree(off2); cudaFree(tmp); };
-    k_pad_len<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(f->pix_off, n, padlen);
+    { k_pad_len<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(f->pix_off, n, padlen); lya_note_launch(); }
     e = lya_exclusive_scan(padlen, off2, n, tmp, s);
     unsigned long long total = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&total, off2 + n, sizeof(total), cudaMemcpyDeviceToHost, s);
@@ -214,10 +214,10 @@ lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool
     if (want_xi) { out->chi = (double *)b; b += arr_bytes; out->a = (double *)b; b += arr_bytes; }
     if (want_dmat) { out->ce = (double2 *)b; b += 2 * arr_bytes; out->eg = (double *)b; b += arr_bytes; out->u = (double *)b; b += arr_bytes; }
     const unsigned blocks = (unsigned)((n * 32 + 255) / 256);
-    if (want_xi && want_dmat) k_pack<true, true><<<blocks, 256, 0, s>>>(*f, off2, *out);
-    else if (want_xi) k_pack<true, false><<<blocks, 256, 0, s>>>(*f, off2, *out);
-    else if (want_dmat) k_pack<false, true><<<blocks, 256, 0, s>>>(*f, off2, *out);
-    else k_pack<false, false><<<blocks, 256, 0, s>>>(*f, off2, *out);
+    if (want_xi && want_dmat) { k_pack<true, true><<<blocks, 256, 0, s>>>(*f, off2, *out); lya_note_launch(); }
+    else if (want_xi) { k_pack<true, false><<<blocks, 256, 0, s>>>(*f, off2, *out); lya_note_launch(); }
+    else if (want_dmat) { k_pack<false, true><<<blocks, 256, 0, s>>>(*f, off2, *out); lya_note_launch(); }
+    else { k_pack<false, false><<<blocks, 256, 0, s>>>(*f, off2, *out); lya_note_launch(); }
     e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);      // scratch is freed below
     drop();
@@ -255,12 +255,12 @@ lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *
     if (e != cudaSuccess) { drop(); cudaFree(out->pq); out->pq = NULL; return lya_cuda_fail(ctx, e, "cudaMalloc(bucketing)"); }
     const unsigned blocks = (unsigned)((n_tiles + 3) / 4);
     if (bp->pow2)
-        k_bucket_count<true><<<blocks, 128, 0, s>>>(prep->head, prep->n_forest, *bp, pairs->pq, n, n_tiles, force_generic, keys, counts, ctx->d_counters);
+        { k_bucket_count<true><<<blocks, 128, 0, s>>>(prep->head, prep->n_forest, *bp, pairs->pq, n, n_tiles, force_generic, keys, counts, ctx->d_counters); lya_note_launch(); }
     else
-        k_bucket_count<false><<<blocks, 128, 0, s>>>(prep->head, prep->n_forest, *bp, pairs->pq, n, n_tiles, force_generic, keys, counts, ctx->d_counters);
+        { k_bucket_count<false><<<blocks, 128, 0, s>>>(prep->head, prep->n_forest, *bp, pairs->pq, n, n_tiles, force_generic, keys, counts, ctx->d_counters); lya_note_launch(); }
     e = lya_exclusive_scan(counts, offsets, n_cnt, tmp, s);
     if (e == cudaSuccess) {
-        k_bucket_scatter<<<blocks, 128, 0, s>>>(pairs->pq, keys, n, n_tiles, nk, offsets, out->pq);
+        { k_bucket_scatter<<<blocks, 128, 0, s>>>(pairs->pq, keys, n, n_tiles, nk, offsets, out->pq); lya_note_launch(); }
         e = cudaGetLastError();
     }
     unsigned long long h_start[3] = {0, 0, 0};     // start of key n_perp, n_perp+1, end
@@ -276,5 +276,62 @@ lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *
     out->n_skip = n - (int64_t)h_start[1];
     out->visited = h_cnt[1];
     out->bad_pair = (int)h_cnt[3];
+    return LYA_OK;
+}
+
+// ---- plans ---------------------------------------------------------------------------------------
+extern "C" void lya_plan_free(lya_ctx *ctx, lya_plan *pl)
+{
+    if (!pl) return;
+    if (ctx) cudaSetDevice(ctx->device);
+    lya_prep_free(&pl->prep);
+    lya_buckets_free(&pl->bk);
+    if (pl->pq) cudaFree(pl->pq);
+    free(pl);
+}
+
+extern "C" lya_status lya_plan_create(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                                      int want_xi, int want_dmat, lya_plan **out)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (!out) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_plan_create: out is NULL");
+    *out = NULL;
+    if (!pairs) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_plan_create: pairs is NULL");
+    if (!want_xi && !want_dmat) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_plan_create: want_xi or want_dmat");
+    lya_status st = lya_check_binning(ctx, b);
+    if (st) return st;
+    st = lya_check_forests_host(ctx, f, true, want_xi != 0, want_dmat != 0);
+    if (st) return st;
+    if (f->n_forest > 0 && !(f->ux && f->uy && f->uz))
+        return lya_fail(ctx, LYA_ERR_INVALID_ARG, "the pair kernels need ux,uy,uz (device); derive them once with the catalogue");
+    LYA_CUDA(cudaSetDevice(ctx->device));
+    int max_len = 0;
+    st = lya_validate_forests(ctx, f, want_xi != 0, want_dmat != 0, &max_len);
+    if (st) return st;
+    lya_plan *pl = (lya_plan *)calloc(1, sizeof(lya_plan));
+    if (!pl) return lya_fail(ctx, LYA_ERR_OOM, "host allocation failed");
+    pl->f = *f; pl->b = *b; pl->bp = lya_make_binparams(b);
+    pl->has_xi = want_xi != 0; pl->has_dmat = want_dmat != 0;
+    pl->n_pairs = pairs->n; pl->max_len = max_len;
+    pl->use_fast = pairs->n > 0 && b->n_par <= LYA_FAST_NPAR_MAX && b->n_perp + 2 <= 256 && !ctx->force_generic;
+    cudaStream_t s = ctx->stream;
+    if (pl->use_fast) {
+        st = lya_prep_build(ctx, f, pl->has_xi, pl->has_dmat, &pl->prep);
+        if (st) { lya_plan_free(ctx, pl); return st; }
+        cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
+        st = lya_bucket_pairs(ctx, &pl->prep, &pl->bp, pairs, 0, &pl->bk);
+        if (st) { lya_plan_free(ctx, pl); return st; }
+        if (pl->bk.bad_pair == LYA_DEV_BAD_PAIR) {
+            lya_plan_free(ctx, pl);
+            return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)");
+        }
+        pl->listed_degenerate = pl->bk.bad_pair == LYA_DEV_DEGENERATE;
+        pl->visited = pl->bk.visited;
+    } else if (pairs->n > 0) {
+        cudaError_t e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)pairs->n);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(pl->pq, pairs->pq, sizeof(int32_t) * 2 * (size_t)pairs->n, cudaMemcpyDeviceToDevice, s);
+        if (e != cudaSuccess) { lya_plan_free(ctx, pl); return lya_cuda_fail(ctx, e, "lya_plan_create (pair list copy)"); }
+    }
+    *out = pl;
     return LYA_OK;
 }

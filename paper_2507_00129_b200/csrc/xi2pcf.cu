@@ -295,11 +295,11 @@ cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
     if (P.bp.pow2) {
         e = cudaFuncSetAttribute(k_xi<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        k_xi<D, true><<<grid, XI_THREADS, smem, s>>>(P);
+        { k_xi<D, true><<<grid, XI_THREADS, smem, s>>>(P); lya_note_launch(); }
     } else {
         e = cudaFuncSetAttribute(k_xi<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        k_xi<D, false><<<grid, XI_THREADS, smem, s>>>(P);
+        { k_xi<D, false><<<grid, XI_THREADS, smem, s>>>(P); lya_note_launch(); }
     }
     return cudaGetLastError();
 }
@@ -624,65 +624,46 @@ __global__ void k_check_region(const int32_t *region, int64_t n, int n_region, u
 }  // namespace
 
 // region == NULL: eq. 2.4 over the whole list.  Otherwise (NEXT-1) one set of accumulators per sub-sample.
-static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
-                         const int32_t *region, int n_region,
+static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region, int n_region,
                          double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
 {
     if (!ctx) return LYA_ERR_INVALID_ARG;
-    if (!pairs) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf: pairs is NULL");
-    lya_status st = lya_check_binning(ctx, b);
-    if (st) return st;
-    st = lya_check_forests_host(ctx, f, true, true, false);
-    if (st) return st;
-    if (f->n_forest > 0 && !(f->ux && f->uy && f->uz))
-        return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf needs ux,uy,uz (device); derive them once with the catalogue");
+    if (!pl) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf: plan is NULL");
+    if (!pl->has_xi) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf: the plan was created without want_xi");
     LYA_CUDA(cudaSetDevice(ctx->device));
-    st = lya_validate_forests(ctx, f, true, false, NULL);
-    if (st) return st;
-
+    const lya_forests *f = &pl->f;
+    const lya_binning *b = &pl->b;
     const int nb = b->n_par * b->n_perp;
     const int n_reg = region ? n_region : 1;
     const size_t nbt = (size_t)nb * n_reg;                     // accumulator entries
     cudaStream_t s = ctx->stream;
-    const BinParams bp = lya_make_binparams(b);
+    const BinParams bp = pl->bp;
     if (region) {
         if (n_region < 1 || (int64_t)n_region * nb > ((int64_t)1 << 28))
             return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_xi2pcf_sub: need 1 <= n_region and n_region * bins <= 2^28");
         cudaMemsetAsync(ctx->d_counters + 12, 0, sizeof(unsigned long long), s);
         if (f->n_forest > 0)
-            k_check_region<<<(unsigned)((f->n_forest + 255) / 256), 256, 0, s>>>(region, f->n_forest, n_region, ctx->d_counters + 12);
+            { k_check_region<<<(unsigned)((f->n_forest + 255) / 256), 256, 0, s>>>(region, f->n_forest, n_region, ctx->d_counters + 12); lya_note_launch(); }
         unsigned long long bad = 0;
         LYA_CUDA(cudaMemcpyAsync(&bad, ctx->d_counters + 12, sizeof(bad), cudaMemcpyDeviceToHost, s));
         LYA_CUDA(cudaStreamSynchronize(s));
         if (bad) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_sub: region[] must lie in [0, n_region)");
     }
-    // fast path: bucketed list + warp-private sub-histograms (LYA_OPT_FORCE_GENERIC routes everything to the generic kernel)
-    const bool use_fast = pairs->n > 0 && 2 * (b->n_par + 1) * LYA_NCOL <= FSLOTS && b->n_perp + 2 <= 256 && !ctx->force_generic;
-    LyaPrep prep;
-    LyaBuckets bk;
-    memset(&prep, 0, sizeof(prep));
-    memset(&bk, 0, sizeof(bk));
+    const bool use_fast = pl->use_fast;
+    const LyaBuckets &bk = pl->bk;
     double *acc = NULL;                         // [S | W | N] accumulators
-    auto cleanup = [&]() { cudaFree(acc); lya_prep_free(&prep); lya_buckets_free(&bk); };
+    auto cleanup = [&]() { cudaFree(acc); };
     cudaEventRecord(ctx->ev[3], s);
-    if (use_fast) {
-        st = lya_prep_build(ctx, f, true, false, &prep);
-        if (st) return st;
-        cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
-        st = lya_bucket_pairs(ctx, &prep, &bp, pairs, 0, &bk);
-        if (st) { cleanup(); return st; }
-        if (bk.bad_pair) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
-    }
     cudaError_t e = cudaMalloc(&acc, nbt * 24);
-    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(xi accumulators)"); }
+    if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "cudaMalloc(xi accumulators)");
     cudaMemsetAsync(acc, 0, nbt * 24, s);
     cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
 
     XiParams P;
     P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.delta = f->delta;
     P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
-    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pairs->pq;
-    P.n_pairs = use_fast ? bk.n_generic : pairs->n;
+    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pl->pq;
+    P.n_pairs = use_fast ? bk.n_generic : pl->n_pairs;
     P.n_forest = f->n_forest;
     P.bp = bp;
     P.S = acc; P.W = acc + nbt; P.N = (unsigned long long *)(acc + 2 * nbt);
@@ -691,17 +672,17 @@ static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *
     cudaEventRecord(ctx->ev[0], s);
     if (use_fast && bk.n_fast > 0) {
         XiFastParams F;
-        F.prep = prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
+        F.prep = pl->prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
         F.S = P.S; F.W = P.W; F.N = P.N; F.counters = ctx->d_counters;
         F.region = region; F.n_region = n_reg;
         const size_t fsmem = sizeof(FastWarp) * FW;
         const int fgrid = ctx->sm_count;
         if (bp.pow2) {
             e = cudaFuncSetAttribute(k_xi_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (e == cudaSuccess) k_xi_fast<true><<<fgrid, FTHREADS, fsmem, s>>>(F);
+            if (e == cudaSuccess) { k_xi_fast<true><<<fgrid, FTHREADS, fsmem, s>>>(F); lya_note_launch(); }
         } else {
             e = cudaFuncSetAttribute(k_xi_fast<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (e == cudaSuccess) k_xi_fast<false><<<fgrid, FTHREADS, fsmem, s>>>(F);
+            if (e == cudaSuccess) { k_xi_fast<false><<<fgrid, FTHREADS, fsmem, s>>>(F); lya_note_launch(); }
         }
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_fast launch"); }
@@ -713,8 +694,8 @@ static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *
     unsigned long long h[4] = {0, 0, 0, 0};
     if (region && P.n_pairs > 0) {                 // sub-sample mode: the block-level histogram of k_xi cannot be used
         const int dgrid = (int)((P.n_pairs + 7) / 8 < (int64_t)ctx->sm_count * 8 ? (P.n_pairs + 7) / 8 : (int64_t)ctx->sm_count * 8);
-        if (bp.pow2) k_xi_direct<true><<<dgrid, 256, 0, s>>>(P, region);
-        else k_xi_direct<false><<<dgrid, 256, 0, s>>>(P, region);
+        if (bp.pow2) { k_xi_direct<true><<<dgrid, 256, 0, s>>>(P, region); lya_note_launch(); }
+        else { k_xi_direct<false><<<dgrid, 256, 0, s>>>(P, region); lya_note_launch(); }
         e = cudaGetLastError();
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_direct launch"); }
     }
@@ -733,7 +714,7 @@ static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *
         if (launches > 100000) { cleanup(); return lya_fail(ctx, LYA_ERR_CUDA, "k_xi made no progress"); }
     }
     cudaEventRecord(ctx->ev[1], s);
-    k_xi_finalize<<<(unsigned)((nbt + 255) / 256), 256, 0, s>>>(P.S, P.W, P.N, (int)nbt, S, W, (unsigned long long *)N, xi);
+    { k_xi_finalize<<<(unsigned)((nbt + 255) / 256), 256, 0, s>>>(P.S, P.W, P.N, (int)nbt, S, W, (unsigned long long *)N, xi); lya_note_launch(); }
     cudaEventRecord(ctx->ev[2], s);
     e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
@@ -741,8 +722,8 @@ static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *
     if (h[3] != 0) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
     if (stats) {
         memset(stats, 0, sizeof(*stats));
-        stats->n_forest_pairs = (uint64_t)pairs->n;
-        stats->n_visited = use_fast ? bk.visited : h[1];
+        stats->n_forest_pairs = (uint64_t)pl->n_pairs;
+        stats->n_visited = use_fast ? pl->visited : h[1];
         stats->n_evaluated = h[2];
         // n_binned = sum N: small D2H
         unsigned long long *hN = (unsigned long long *)malloc(sizeof(unsigned long long) * nbt);
@@ -756,10 +737,21 @@ static lya_status xi_run(lya_ctx *ctx, const lya_forests *f, const lya_binning *
     return LYA_OK;
 }
 
+extern "C" lya_status lya_xi2pcf_plan(lya_ctx *ctx, const lya_plan *plan,
+                                      double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
+{
+    return xi_run(ctx, plan, NULL, 1, S, W, N, xi, stats);
+}
+
 extern "C" lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
                                  double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
 {
-    return xi_run(ctx, f, b, pairs, NULL, 1, S, W, N, xi, stats);
+    lya_plan *pl = NULL;
+    lya_status st = lya_plan_create(ctx, f, b, pairs, 1, 0, &pl);
+    if (st) return st;
+    st = xi_run(ctx, pl, NULL, 1, S, W, N, xi, stats);
+    lya_plan_free(ctx, pl);
+    return st;
 }
 
 extern "C" lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
@@ -768,7 +760,12 @@ extern "C" lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const l
 {
     if (!ctx) return LYA_ERR_INVALID_ARG;
     if (!region) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_sub: region is NULL");
-    return xi_run(ctx, f, b, pairs, region, n_region, S, W, N, NULL, stats);
+    lya_plan *pl = NULL;
+    lya_status st = lya_plan_create(ctx, f, b, pairs, 1, 0, &pl);
+    if (st) return st;
+    st = xi_run(ctx, pl, region, n_region, S, W, N, NULL, stats);
+    lya_plan_free(ctx, pl);
+    return st;
 }
 
 // xi_A = S_A / W_A (0 where W_A == 0) from already-summed numerators (section 8(e): after the all-reduce).
@@ -779,7 +776,7 @@ extern "C" lya_status lya_xi_normalise(lya_ctx *ctx, int64_t n, const double *S,
     if (n > ((int64_t)1 << 30)) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_xi_normalise: n above 2^30");
     LYA_CUDA(cudaSetDevice(ctx->device));
     if (n > 0) {
-        k_xi_finalize<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(S, W, NULL, (int)n, NULL, NULL, NULL, xi);
+        { k_xi_finalize<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(S, W, NULL, (int)n, NULL, NULL, NULL, xi); lya_note_launch(); }
         LYA_CUDA(cudaGetLastError());
     }
     return LYA_OK;

@@ -94,8 +94,8 @@ def sharded_step(ctx, forests, b, reject_fraction: float, seed: int, rank: int, 
                  do_dmat: bool = True, lens=None):
     """One pass of the hot path over ONE catalogue split across `world` ranks.
 
-    Every rank: lya_neighbours (replicated: 0.5 % of the step) -> its chunk of the list ->
-    lya_xi2pcf (S, W, N) and lya_dmat (Dn, Wd) -> all_reduce(SUM) -> lya_xi_normalise /
+    Every rank: lya_neighbours (replicated: 0.5 % of the step) -> its chunk of the list -> one
+    lya_plan -> lya_xi2pcf_plan (S, W, N) and lya_dmat_plan (Dn, Wd) -> all_reduce(SUM) -> lya_xi_normalise /
     lya_dmat_normalise.  Returns the reduced outputs (identical on every rank) plus this rank's
     stats.  `ctx`, `forests`, `b` are binding.Context / DeviceForests / CBinning."""
     import torch
@@ -108,9 +108,11 @@ def sharded_step(ctx, forests, b, reject_fraction: float, seed: int, rank: int, 
         pairs.free()
         pairs = ctx.lya_pairs_import(mine)
         del pq
-    x = ctx.lya_xi2pcf(forests, b, pairs)
-    dm = ctx.lya_dmat(forests, b, pairs, reject_fraction, seed, want_Dn=True, want_D=False) if do_dmat else None
+    plan = ctx.lya_plan_create(forests, b, pairs, want_xi=True, want_dmat=do_dmat)     # prepared once for both stages
     pairs.free()
+    x = ctx.lya_xi2pcf_plan(plan)
+    dm = ctx.lya_dmat_plan(plan, reject_fraction, seed, want_Dn=True, want_D=False) if do_dmat else None
+    plan.free()
     allreduce_sum(x["S"], x["W"], x["N"])
     out = dict(S=x["S"], W=x["W"], N=x["N"], xi=ctx.lya_xi_normalise(x["S"], x["W"]), stats_xi=x["stats"])
     if dm is not None:
