@@ -248,6 +248,51 @@ void orc_xi(const orc_forests *f, const orc_binning *b, const int32_t *pq, int64
     free(gS); free(gW); free(gA); free(gQ);
 }
 
+/* Per-bin weighted sums of the pixel-pair coordinates (NEXT-1, second half; "mimics PICCA":
+ * the correlation is tabulated with the weighted mean r_par, r_perp and redshift of the pairs of each
+ * bin).  For every listed forest pair and every in-grid pixel pair (i, j), A = its bin,
+ * om = w_i w_j (the weight of eq. 2.4's denominator):
+ *     Rpar[A] += om * r_par,   Rperp[A] += om * r_perp,   Z[A] += om * 0.5 * (z_i + z_j),   W[A] += om
+ * with r_par = |chi_i - chi_j| c and r_perp = (chi_i + chi_j) s exactly as binned (reading G5) and z the
+ * caller's per-pixel redshift (reading R-19: the pair redshift is the mean of the two pixel redshifts).
+ * The outputs are SUMS; the weighted means are Rpar[A] / W[A] etc. */
+void orc_xi_means(const orc_forests *f, const orc_binning *b, const int32_t *pq, int64_t n_pairs, const double *z,
+                  double *Rpar, double *Rperp, double *Z, double *W)
+{
+    int32_t nb = b->n_par * b->n_perp;
+    long double *g = (long double *)calloc((size_t)nb * 4, sizeof(long double));
+#pragma omp parallel
+    {
+        long double *t = (long double *)calloc((size_t)nb * 4, sizeof(long double));
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t k = 0; k < n_pairs; ++k) {
+            int64_t p = pq[2 * k], q = pq[2 * k + 1];
+            double s, c;
+            orc_pair_sc(f, p, q, &s, &c);
+            for (int64_t i = f->pix_off[p]; i < f->pix_off[p + 1]; ++i)
+                for (int64_t j = f->pix_off[q]; j < f->pix_off[q + 1]; ++j) {
+                    int32_t A = pix_bin(b, s, c, f->chi[i], f->chi[j]);
+                    if (A < 0) continue;
+                    double om = f->w[i] * f->w[j];
+                    double rpar = fabs(f->chi[i] - f->chi[j]) * c;
+                    double rperp = (f->chi[i] + f->chi[j]) * s;
+                    double zz = 0.5 * (z[i] + z[j]);
+                    t[4 * A + 0] += (long double)om * rpar;
+                    t[4 * A + 1] += (long double)om * rperp;
+                    t[4 * A + 2] += (long double)om * zz;
+                    t[4 * A + 3] += om;
+                }
+        }
+#pragma omp critical
+        for (int32_t a = 0; a < 4 * nb; ++a) g[a] += t[a];
+        free(t);
+    }
+    for (int32_t a = 0; a < nb; ++a) {
+        Rpar[a] = (double)g[4 * a]; Rperp[a] = (double)g[4 * a + 1]; Z[a] = (double)g[4 * a + 2]; W[a] = (double)g[4 * a + 3];
+    }
+    free(g);
+}
+
 /* ---- eq. 2.7: explicit eta for one forest (reading R-10) -------------------- */
 /*
  * eta[i*n+k] = delta^K_ik - w_k/sum(w) - (L_i-Lbar) w_k (L_k-Lbar) / sum_m w_m (L_m-Lbar)^2

@@ -137,6 +137,19 @@ def xi(f, pairs, b=None):
     return dict(S=S, W=W, N=N, xi=x, Sabs=Sabs, Q=Q, n_out=int(n_out[0]))
 
 
+def xi_means(f, pairs, z, b=None):
+    """NEXT-1: per-bin weighted SUMS of r_par, r_perp, z (weights w_i w_j) and W; means = sums / W."""
+    cat = f if isinstance(f, Catalogue) else Catalogue(f)
+    b = b or binning()
+    pq = _pq(pairs)
+    z = _c(z, np.float64)
+    nb = b.n_par * b.n_perp
+    out = [np.zeros(nb) for _ in range(4)]
+    lib().orc_xi_means(C.byref(cat.c), C.byref(b), C.c_void_p(pq.ctypes.data), C.c_int64(len(pq)),
+                       C.c_void_p(z.ctypes.data), *[C.c_void_p(a.ctypes.data) for a in out])
+    return dict(Rpar=out[0], Rperp=out[1], Z=out[2], W=out[3])
+
+
 def eta(w, loglam):
     """eq. 2.7: explicit n x n eta of one forest (raises on a degenerate forest)."""
     w = _c(w, np.float64); ll = _c(loglam, np.float64)

@@ -439,3 +439,60 @@ def test_region_subsamples_partition_the_full_result(cfg0, xi0):
     subs2 = orc.xi_sub(cfg0, pq, region2, 4)
     only0 = orc.xi(cfg0, pq[pq[:, 0] == 0])
     assert np.array_equal(subs2[3]["N"], only0["N"])
+
+
+# ---------------------------------------------------------------- NEXT-1: weighted mean r_par, r_perp, z per bin
+def test_PM1_means_numpy_enumeration(cfg0):
+    """Sums of om r_par, om r_perp, om z per bin against numpy's histogram2d with weights over every
+    pixel pair of the neighbour list (an independent library routine, not the oracle's loop)."""
+    pq = orc.pairs_brute(cfg0)
+    z = 10.0 ** cfg0.loglam / 1215.67 - 1.0
+    m = orc.xi_means(cfg0, pq, z)
+    edges = np.linspace(0.0, 200.0, 51)
+    R1 = np.zeros((50, 50)); R2 = np.zeros((50, 50)); Z = np.zeros((50, 50)); W = np.zeros((50, 50))
+    f = cfg0
+    for p, q in pq:
+        s = 0.5 * np.sqrt((f.ux[p] - f.ux[q]) ** 2 + (f.uy[p] - f.uy[q]) ** 2 + (f.uz[p] - f.uz[q]) ** 2)
+        c = np.sqrt(1.0 - s * s)
+        a, b = f.pix_off[p], f.pix_off[p + 1]; d, e = f.pix_off[q], f.pix_off[q + 1]
+        rpar = (np.abs(f.chi[a:b, None] - f.chi[None, d:e]) * c).ravel()
+        rperp = ((f.chi[a:b, None] + f.chi[None, d:e]) * s).ravel()
+        om = (f.w[a:b, None] * f.w[None, d:e]).ravel()
+        zz = (0.5 * (z[a:b, None] + z[None, d:e])).ravel()
+        ok = (rpar < 200.0) & (rperp < 200.0)
+        for acc, wt in ((R1, om * rpar), (R2, om * rperp), (Z, om * zz), (W, om)):
+            acc += np.histogram2d(rpar[ok], rperp[ok], bins=[edges, edges], weights=wt[ok])[0]
+    for got, want in ((m["Rpar"], R1), (m["Rperp"], R2), (m["Z"], Z), (m["W"], W)):
+        assert np.allclose(got, want.ravel(), rtol=1e-12, atol=0)
+
+
+def test_PM2_means_lie_inside_their_bin_and_special_cases(cfg0):
+    pq = orc.pairs_brute(cfg0)
+    z = 10.0 ** cfg0.loglam / 1215.67 - 1.0
+    m = orc.xi_means(cfg0, pq, z)
+    x = orc.xi(cfg0, pq)
+    assert np.allclose(m["W"], x["W"], rtol=1e-14)                       # the same denominator as eq. 2.4
+    nz = m["W"] > 0
+    A = np.arange(2500)[nz]
+    rp, rt, zb = m["Rpar"][nz] / m["W"][nz], m["Rperp"][nz] / m["W"][nz], m["Z"][nz] / m["W"][nz]
+    assert np.all((rp >= 4.0 * (A // 50)) & (rp < 4.0 * (A // 50) + 4.0))   # a weighted mean stays inside its bin
+    assert np.all((rt >= 4.0 * (A % 50)) & (rt < 4.0 * (A % 50) + 4.0))
+    assert np.all((zb > z.min()) & (zb < z.max()))
+    # constant z: the mean redshift of every bin is that constant
+    mc = orc.xi_means(cfg0, pq, np.full_like(z, 2.25))
+    assert np.allclose(mc["Z"][nz] / mc["W"][nz], 2.25, rtol=1e-13)
+    # one pixel pair: the sums are that pair's coordinates times its weight (50-digit arithmetic)
+    from decimal import Decimal, getcontext
+    getcontext().prec = 50
+    s_txt = "0.0123"
+    uq = (1.0 - 2.0 * float(s_txt) ** 2, 2.0 * float(s_txt) * float((1 - Decimal(s_txt) ** 2).sqrt()), 0.0)
+    f2 = gen.two_forests([4000.0], [4070.5], (1.0, 0.0, 0.0), uq, w_p=[1.5], w_q=[0.25])
+    s, c = orc.pair_sc(f2, 0, 1)
+    m2 = orc.xi_means(f2, [[0, 1]], np.array([2.0, 3.0]))
+    A2 = int(np.nonzero(m2["W"])[0][0])
+    rpar = Decimal(70.5) * Decimal(c); rperp = Decimal(8070.5) * Decimal(s)
+    assert A2 == 50 * int(rpar / 4) + int(rperp / 4)
+    assert abs(m2["W"][A2] - 0.375) < 1e-15
+    assert abs(Decimal(float(m2["Rpar"][A2])) / Decimal("0.375") - rpar) < Decimal("1e-11")
+    assert abs(Decimal(float(m2["Rperp"][A2])) / Decimal("0.375") - rperp) < Decimal("1e-11")
+    assert abs(m2["Z"][A2] / 0.375 - 2.5) < 1e-14
