@@ -169,6 +169,17 @@ lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const lya_binning 
                           const lya_pairs *pairs, const int32_t *region, int32_t n_region,
                           double *S, double *W, uint64_t *N, lya_stats *stats);
 
+/* NEXT-1, second half: the weighted mean coordinates of every bin, as the PICCA-like correlation table carries
+ * them ("mimics PICCA", 261-263).  For every in-grid pixel pair (i, j) of the listed forest pairs,
+ * A = its bin, om = w_i w_j:  Rpar[A] += om r_par,  Rperp[A] += om r_perp,  Z[A] += om (z_i + z_j) / 2,
+ * W[A] += om, with r_par, r_perp exactly as binned (geometry above) and z a device array [n_pix] of pixel
+ * redshifts (reading R-19: the redshift of a pair is the mean of its two pixels').  The outputs are SUMS (device
+ * double [n_par*n_perp], additive over forest pairs and ranks); the means are lya_xi_normalise(Rpar, W) etc.
+ * W may be NULL.  delta and loglam are not read.  A second, cheap mode (shared-memory CAS histogram), not the
+ * tuned pair kernel.  Synchronises the ctx stream. */
+lya_status lya_xi2pcf_means(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                            const double *z, double *Rpar, double *Rperp, double *Z, double *W);
+
 /* ---- stages 3+4: distortion matrix, eqs. 2.6-2.7 ----------------- */
 /* eta_ii' = delta^K_ii' - w_i'/sum_k w_k - (L_i-Lbar) w_i' (L_i'-Lbar) / sum_k w_k (L_k-Lbar)^2
  * inside a forest (0 across forests), L = loglam, Lbar the w-weighted mean (R-10).

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "liblya.so")
 
 EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_launch_count", "lya_set_option", "lya_neighbours",
            "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
-           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_dmat", "lya_run_host", "lya_xi_normalise", "lya_dmat_normalise",
+           "lya_xi2pcf", "lya_xi2pcf_sub", "lya_xi2pcf_means", "lya_dmat", "lya_run_host", "lya_xi_normalise", "lya_dmat_normalise",
            "lya_plan_create", "lya_plan_free", "lya_xi2pcf_plan", "lya_dmat_plan"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
@@ -80,6 +80,8 @@ def load():
                                    C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
         lib.lya_xi2pcf_sub.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
                                        C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
+        lib.lya_xi2pcf_means.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.lya_dmat.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p,
                                  C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
         lib.lya_run_host.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_int, C.c_int,
@@ -298,6 +300,18 @@ class Context:
         self._check(load().lya_xi2pcf_sub(self.h, C.byref(cf), C.byref(b), pairs.handle, _ptr(region), int(n_region),
                                           _ptr(S), _ptr(W), _ptr(N), C.byref(stats)))
         return dict(S=S, W=W, N=N, stats=stats.as_dict())
+
+    def lya_xi2pcf_means(self, forests: DeviceForests, b: CBinning, pairs: Pairs, z):
+        """z: per-pixel redshift (numpy or torch, [n_pix]).  Returns the SUMS Rpar, Rperp, Z and W."""
+        torch = self.torch
+        if not torch.is_tensor(z):
+            z = torch.from_numpy(np.ascontiguousarray(z, dtype=np.float64))
+        z = z.to(self.device, dtype=torch.float64).contiguous()
+        nb = b.n_par * b.n_perp
+        out = [torch.empty(nb, dtype=torch.float64, device=self.device) for _ in range(4)]
+        cf = forests.c()
+        self._check(load().lya_xi2pcf_means(self.h, C.byref(cf), C.byref(b), pairs.handle, _ptr(z), *[_ptr(o) for o in out]))
+        return dict(Rpar=out[0], Rperp=out[1], Z=out[2], W=out[3])
 
     # ---- lya_dmat ----
     def lya_dmat(self, forests: DeviceForests, b: CBinning, pairs: Pairs, reject_fraction: float, seed: int,

@@ -768,6 +768,116 @@ extern "C" lya_status lya_xi2pcf_sub(lya_ctx *ctx, const lya_forests *f, const l
     return st;
 }
 
+// ======================= NEXT-1, second half: weighted sums of r_par, r_perp, z per bin ==================
+// Rpar_A = sum om r_par, Rperp_A = sum om r_perp, Z_A = sum om (z_i + z_j) / 2, W_A = sum om over the in-grid
+// pixel pairs of bin A, om = w_i w_j (the PICCA-like table carries the weighted mean
+// coordinates of every bin; the means are these sums over W_A).  A second, cheap mode next to the pair kernel:
+// one warp per forest pair, lanes over the pixel pairs, block-level shared histogram (fp64 shared atomics are a
+// CAS loop here -- acceptable for an output computed once per analysis), merged with global fp64 atomics.
+namespace {
+constexpr int MEAN_THREADS = 256;
+template <bool POW2>
+__global__ void __launch_bounds__(MEAN_THREADS) k_xi_means(XiParams P, const double *z, double *out /* [4][nb] */)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const BinParams bp = P.bp;
+    const int nb = bp.n_par * bp.n_perp;
+    double *h = (double *)smem_raw;                                   // [4][nb]
+    for (int k = threadIdx.x; k < 4 * nb; k += MEAN_THREADS) h[k] = 0.0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int64_t n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t k = warp; k < P.n_pairs; k += n_warps) {
+        const int p = P.pq[2 * k], q = P.pq[2 * k + 1];
+        if ((unsigned)p >= (unsigned)P.n_forest || (unsigned)q >= (unsigned)P.n_forest) {
+            if (lane == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_BAD_PAIR);
+            continue;
+        }
+        const int64_t op = P.pix_off[p], oq = P.pix_off[q];
+        const int np = (int)(P.pix_off[p + 1] - op), nq = (int)(P.pix_off[q + 1] - oq);
+        if (np == 0 || nq == 0) continue;
+        double s, c;
+        lya_pair_sc(P.ux[p], P.uy[p], P.uz[p], P.ux[q], P.uy[q], P.uz[q], s, c);
+        const PairBin g = lya_make_pairbin(bp, s, c);
+        int i = 0, j = lane;                                           // lanes over the pixel pairs, row-major
+        while (j >= nq) { j -= nq; ++i; }
+        while (i < np) {
+            const double ci = P.chi[op + i], cj = P.chi[oq + j];
+            const int A = lya_pix_bin<POW2>(bp, g, ci, cj);
+            if (A >= 0) {
+                const double om = P.w[op + i] * P.w[oq + j];
+                const double rpar = __dmul_rn(fabs(__dsub_rn(ci, cj)), g.c), rperp = __dmul_rn(__dadd_rn(ci, cj), g.s);
+                atomicAdd(&h[A], om * rpar);
+                atomicAdd(&h[nb + A], om * rperp);
+                atomicAdd(&h[2 * nb + A], om * (0.5 * (z[op + i] + z[oq + j])));
+                atomicAdd(&h[3 * nb + A], om);
+            }
+            j += 32;
+            while (j >= nq) { j -= nq; ++i; }
+        }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < 4 * nb; k += MEAN_THREADS)
+        if (h[k] != 0.0) atomicAdd(&out[k], h[k]);
+}
+}  // namespace
+
+extern "C" lya_status lya_xi2pcf_means(lya_ctx *ctx, const lya_forests *f, const lya_binning *b, const lya_pairs *pairs,
+                                       const double *z, double *Rpar, double *Rperp, double *Z, double *W)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (!pairs || !Rpar || !Rperp || !Z) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_means: NULL argument");
+    lya_status st = lya_check_binning(ctx, b);
+    if (st) return st;
+    st = lya_check_forests_host(ctx, f, true, false, false);
+    if (st) return st;
+    if (f->n_forest > 0 && !(f->ux && f->uy && f->uz)) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_means needs ux,uy,uz (device)");
+    if (f->n_pix > 0 && !z) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_means: z is NULL");
+    LYA_CUDA(cudaSetDevice(ctx->device));
+    st = lya_validate_forests(ctx, f, false, false, NULL);
+    if (st) return st;
+    const int nb = b->n_par * b->n_perp;
+    cudaStream_t s = ctx->stream;
+    double *acc = NULL;
+    LYA_CUDA(cudaMalloc(&acc, sizeof(double) * 4 * (size_t)nb));
+    cudaMemsetAsync(acc, 0, sizeof(double) * 4 * (size_t)nb, s);
+    cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
+    XiParams P;
+    memset(&P, 0, sizeof(P));
+    P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.delta = NULL;
+    P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
+    P.pq = pairs->pq; P.n_pairs = pairs->n; P.n_forest = f->n_forest;
+    P.bp = lya_make_binparams(b);
+    P.counters = ctx->d_counters;
+    cudaError_t e = cudaSuccess;
+    if (pairs->n > 0) {
+        const size_t smem = sizeof(double) * 4 * (size_t)nb;
+        const int64_t want = (pairs->n + 7) / 8;
+        const int grid = (int)(want < (int64_t)ctx->sm_count * 2 ? want : (int64_t)ctx->sm_count * 2);
+        if (P.bp.pow2) {
+            e = cudaFuncSetAttribute(k_xi_means<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess) { k_xi_means<true><<<grid, MEAN_THREADS, smem, s>>>(P, z, acc); lya_note_launch(); }
+        } else {
+            e = cudaFuncSetAttribute(k_xi_means<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess) { k_xi_means<false><<<grid, MEAN_THREADS, smem, s>>>(P, z, acc); lya_note_launch(); }
+        }
+        if (e == cudaSuccess) e = cudaGetLastError();
+    }
+    const size_t bytes = sizeof(double) * (size_t)nb;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(Rpar, acc, bytes, cudaMemcpyDeviceToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(Rperp, acc + nb, bytes, cudaMemcpyDeviceToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(Z, acc + 2 * nb, bytes, cudaMemcpyDeviceToDevice, s);
+    if (e == cudaSuccess && W) e = cudaMemcpyAsync(W, acc + 3 * nb, bytes, cudaMemcpyDeviceToDevice, s);
+    unsigned long long h[4] = {0, 0, 0, 0};
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(acc);
+    if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "lya_xi2pcf_means");
+    if (h[3] != 0) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)");
+    return LYA_OK;
+}
+
 // xi_A = S_A / W_A (0 where W_A == 0) from already-summed numerators (section 8(e): after the all-reduce).
 extern "C" lya_status lya_xi_normalise(lya_ctx *ctx, int64_t n, const double *S, const double *W, double *xi)
 {

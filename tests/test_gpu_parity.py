@@ -364,6 +364,27 @@ def test_sharded_halves_sum_to_full(ctx, B, orc):
     check_dmat(dict(D=st["D"], Dn=st["Dn"], Wd=st["Wd"], stats=st["stats_dmat"]), od, "sharded_step D")
 
 
+def test_weighted_mean_coordinates_next1(ctx, B, orc):
+    """lya_xi2pcf_means against the oracle: sums of om r_par, om r_perp, om z and W per bin to 1e-9, on a
+    power-of-two and a generic grid; the means come out of lya_xi_normalise."""
+    f = gen.make_config(1, n_forest=500)
+    d = B.DeviceForests(f)
+    z = 10.0 ** f.loglam / 1215.67 - 1.0
+    for grid in ((200.0, 200.0, 50, 50), (150.0, 90.0, 30, 40)):
+        b, ob = B.binning(*grid), orc.binning(*grid)
+        pairs = ctx.lya_neighbours(d, b)
+        pq = pairs.export().cpu().numpy()
+        g = ctx.lya_xi2pcf_means(d, b, pairs, z)
+        o = orc.xi_means(f, pq, z, ob)
+        for k in ("Rpar", "Rperp", "Z", "W"):
+            assert np.all(np.abs(g[k].cpu().numpy() - o[k]) <= 1e-9 * np.abs(o[k])), k
+        nz = o["W"] > 0
+        zbar = ctx.lya_xi_normalise(g["Z"], g["W"]).cpu().numpy()
+        assert np.all(np.abs(zbar[nz] - o["Z"][nz] / o["W"][nz]) <= 1e-9) and np.all(zbar[~nz] == 0.0)
+        x = ctx.lya_xi2pcf(d, b, pairs)
+        assert np.allclose(g["W"].cpu().numpy(), x["W"].cpu().numpy(), rtol=1e-12)      # eq. 2.4's denominator
+
+
 # ------------------------------------------------------------------ invariances and edge cases
 def test_P7_pair_order_and_swap(ctx, B, orc, cfg0):
     d = B.DeviceForests(cfg0)
