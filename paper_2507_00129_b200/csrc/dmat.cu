@@ -460,7 +460,7 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
     P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.loglam = f->loglam;
     P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
     P.f_invS = scal; P.f_lbar = scal + nf; P.f_invV = scal + 2 * nf;
-    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pl->pq;
+    P.pq = use_fast ? bk.pq + 2 * (bk.n_fast + bk.n_fast2) : pl->pq;
     P.n_pairs = use_fast ? bk.n_generic : pl->n_pairs;
     P.n_forest = nf;
     P.bp = bp;
@@ -471,19 +471,33 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
     if (P.LC > b->n_perp) P.LC = b->n_perp;
 
     cudaEventRecord(ctx->ev[0], s);
-    if (use_fast && bk.n_fast > 0) {
+    if (use_fast && bk.n_fast + bk.n_fast2 > 0) {
         DmFastParams F;
-        F.prep = pl->prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp; F.seed = seed; F.thr = thr;
+        F.prep = pl->prep; F.bp = bp; F.seed = seed; F.thr = thr;
         F.Dn = Dn; F.Wd = Wd; F.counters = ctx->d_counters;
-        const size_t fsmem = FD_SMEM_BYTES;
         const int fgrid = ctx->sm_count;
-        auto launch = [&](auto kern) {
+        auto launch = [&](auto kern, int threads, size_t fsmem) {
             cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (le == cudaSuccess) { kern<<<fgrid, FD_THREADS, fsmem, s>>>(F); lya_note_launch(); }
+            if (le == cudaSuccess) { kern<<<fgrid, threads, fsmem, s>>>(F); lya_note_launch(); }
             return le;
         };
-        if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_fast<true, true>) : launch(k_dmat_fast<false, true>);
-        else e = bp.pow2 ? launch(k_dmat_fast<true, false>) : launch(k_dmat_fast<false, false>);
+        e = cudaSuccess;
+        if (bk.n_fast > 0) {                                  // class 0: forests of up to 72 pixels, spacing above the bin width
+            F.pq = bk.pq; F.n_pairs = bk.n_fast;
+            const int th = DmCfg<0>::WARPS * 32;
+            const size_t sm = DmPool<0>::SMEM_BYTES;
+            if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_fast<true, true, 0>, th, sm) : launch(k_dmat_fast<false, true, 0>, th, sm);
+            else e = bp.pow2 ? launch(k_dmat_fast<true, false, 0>, th, sm) : launch(k_dmat_fast<false, false, 0>, th, sm);
+        }
+        if (e == cudaSuccess && bk.n_fast2 > 0) {             // class 1: up to 144 pixels, diagonal stride up to 8
+            // (its own work counter: counters[4] is reset between the two launches on the stream)
+            cudaMemsetAsync(ctx->d_counters + 4, 0, sizeof(unsigned long long), s);
+            F.pq = bk.pq + 2 * bk.n_fast; F.n_pairs = bk.n_fast2;
+            const int th = DmCfg<1>::WARPS * 32;
+            const size_t sm = DmPool<1>::SMEM_BYTES;
+            if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_fast<true, true, 1>, th, sm) : launch(k_dmat_fast<false, true, 1>, th, sm);
+            else e = bp.pow2 ? launch(k_dmat_fast<true, false, 1>, th, sm) : launch(k_dmat_fast<false, false, 1>, th, sm);
+        }
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_dmat_fast launch"); }
     }

@@ -20,24 +20,41 @@
 
 namespace {
 
+// Two size classes of the same kernel (template parameter CLS):
+//   class 0: forests of up to LYA_FAST_TILE (72) pixels -- the BASELINE configs; 15 warps per SM;
+//   class 1: forests of up to LYA_FAST_TILE2 (144) pixels -- native-resolution shapes (DESIGN.md NEXT-3): longer
+//            staging tiles and kept-pair queue, 10 warps per SM.
+// In both, pass A takes a DIAGONAL STRIDE ds: a pass covers the diagonals d0 + ds * lane, so the lanes of a row
+// step sit ds pixels of q apart; ds is the smallest integer with ds * (q's pixel spacing) > r_par bin width, which
+// keeps "one holder per table entry" true when the pixels are finer than the bins (ds passes, one per residue,
+// cover every diagonal; the number of lane-slots walked is the same).
 #ifndef LYA_FD_WARPS
 #define LYA_FD_WARPS 15
 #endif
-constexpr int FD_WARPS = LYA_FD_WARPS;       // one CTA per SM; 5.6 KB of private shared memory per warp + the table pool
-constexpr int FD_THREADS = FD_WARPS * 32;
+#ifndef LYA_FD_WARPS2
+#define LYA_FD_WARPS2 10
+#endif
+template <int CLS> struct DmCfg;
+template <> struct DmCfg<0> { static constexpr int T = LYA_FAST_TILE, WARPS = LYA_FD_WARPS, KCAP = 48; };
+template <> struct DmCfg<1> { static constexpr int T = LYA_FAST_TILE2, WARPS = LYA_FD_WARPS2, KCAP = 192; };
+// (the FD_* names below depend on the template parameter CLS of the struct / function they are used in)
+#define FD_WARPS (DmCfg<CLS>::WARPS)         // one CTA per SM; private shared memory per warp + the table pool
+#define FD_THREADS (DmCfg<CLS>::WARPS * 32)
+#define FD_T (DmCfg<CLS>::T)
+#define FD_TP (((DmCfg<CLS>::T + 15) / 16) * 16 + 2)
+#define FD_TQ (DmCfg<CLS>::T + 2 * FD_PAD)
+#define FD_KCAP (DmCfg<CLS>::KCAP)           // kept pairs queued per forest pair
+#define FD_RPL ((DmCfg<CLS>::T + 31) / 32)   // rows of p per lane in the mask scan's prefix sum
 constexpr int FD_SMEM_MAX = 232448;          // 227 KB: the most a CTA can have on sm_100
-constexpr int FD_T = LYA_FAST_TILE;
 #ifndef LYA_FD_ROWS
 #define LYA_FD_ROWS 16
 #endif
 constexpr int FD_ROWS = LYA_FD_ROWS;         // rows of p per pass-A group
-constexpr int FD_TP = ((FD_T + 15) / 16) * 16 + 2;
 constexpr int FD_PAD = 2;
-constexpr int FD_TQ = FD_T + 2 * FD_PAD;
 constexpr int FD_SLOTS = 302;                // n_par * LYA_NCOL + 1 <= FD_SLOTS (the last slot used is garbage)
-constexpr int FD_KCAP = 48;                  // kept pairs queued per forest pair
 constexpr int FD_KBATCH = 24;                // kept pairs drained together (coefficient tables)
 constexpr int FD_CHUNK = 8;
+constexpr int FD_DS_MAX = 8;                 // largest diagonal stride the fast kernel takes
 // Profiling aids (compile-time, off by default; results are WRONG with any of them): -DLYA_ABL_NO_T23,
 // -DLYA_ABL_NO_T4, -DLYA_ABL_NO_MASK, -DLYA_ABL_NO_WALK drop one phase so that its share of the kernel time can
 // be measured as a difference (profiles/r2*_dmat_ablation.md).
@@ -52,7 +69,7 @@ struct DmFastParams {
     unsigned long long *counters;   // [4] next chunk, [2] evaluated, [3] error, [5] kept, [6] binned, [7] scatter-adds, [10] holder conflicts (CHECK)
 };
 
-struct DmKeysA {                                                             // mask scan
+template <int CLS> struct DmKeysA {                                          // mask scan
     unsigned long long qk[FD_T], pk[FD_T];       // stage-4 keys of the pixels of q and p
     unsigned short pre[FD_T + 2];                // pre[i] = in-window pairs of the rows before i
 };
@@ -60,30 +77,33 @@ struct DmDrainBC {                                                            //
     double2 kc01[FD_KBATCH], kc23[FD_KBATCH];    // per kept pair of a batch: om (1, u_j), om (u_i, u_i u_j)
     unsigned short nz[FD_SLOTS];                 // non-zero slots
 };
-// H tables live in a POOL shared by the warps of the CTA: a warp needs one only from pass A to the end of T4
-// (about a third of its time on a forest pair), so fewer tables than warps are enough and the shared memory
-// saved buys resident warps (the kernel is latency-bound: IPC follows the warp count).  A free table is all zero.
+// H tables live in a POOL shared by the warps of the CTA (a warp holds one from pass A to the end of T4; a free
+// table is all zero).  With as many tables as warps (the default) nobody ever waits; fewer tables than warps
+// were measured to lose more to waiting than extra warps bring (profiles/r2b_dmat_ablation.md).
 struct __align__(16) DmTable {
     double2 H01[FD_SLOTS], H23[FD_SLOTS];    // (H_aa, H_ag), (H_ga, H_gg) per slot = col_rel * n_par + b_par; slot LYA_NCOL * n_par = garbage
 };
-struct __align__(16) DmFastWarp {
+template <int CLS> struct __align__(16) DmFastWarp {
     double2 pce[FD_TP];                      // (chi, ea) of p; rows >= len are sentinels
     double2 qce[FD_TQ];                      // (chi, ea) of q, FD_PAD sentinels either side
     double peg[FD_TP], qeg[FD_TQ];           // eg
-    union { DmKeysA a; DmDrainBC b; } u;     // the keys are dead once the mask scan is done (shared memory buys occupancy)
+    union { DmKeysA<CLS> a; DmDrainBC b; } u;     // the keys are dead once the mask scan is done (shared memory buys occupancy)
     unsigned kept[FD_KCAP];                  // (A << 16) | (i << 8) | j   (A is filled in by the drain)
     unsigned char jlo[FD_T + 4], jx[FD_T + 4], jhi[FD_T + 4];   // (row len = a stop row for the mask scan)
     unsigned nkept, pad_[1];
 };
 constexpr int FD_POOL_HDR = 128;             // owner flags of the tables (one int each)
+template <int CLS> struct DmPool {
+    static constexpr int FIT = (FD_SMEM_MAX - FD_POOL_HDR - (int)sizeof(DmFastWarp<CLS>) * FD_WARPS) / (int)sizeof(DmTable);
 #ifdef LYA_FD_NTABLES
-constexpr int FD_NTABLES = LYA_FD_NTABLES;
+    static constexpr int NTABLES = LYA_FD_NTABLES;
 #else
-constexpr int FD_NTABLES = (FD_SMEM_MAX - FD_POOL_HDR - (int)sizeof(DmFastWarp) * FD_WARPS) / (int)sizeof(DmTable) < FD_WARPS
-                               ? (FD_SMEM_MAX - FD_POOL_HDR - (int)sizeof(DmFastWarp) * FD_WARPS) / (int)sizeof(DmTable) : FD_WARPS;
+    static constexpr int NTABLES = FIT < FD_WARPS ? FIT : FD_WARPS;
 #endif
-static_assert(FD_NTABLES >= 2 && FD_NTABLES * 4 <= FD_POOL_HDR, "table pool");
-constexpr size_t FD_SMEM_BYTES = FD_POOL_HDR + sizeof(DmTable) * FD_NTABLES + sizeof(DmFastWarp) * FD_WARPS;
+    static constexpr size_t SMEM_BYTES = FD_POOL_HDR + sizeof(DmTable) * NTABLES + sizeof(DmFastWarp<CLS>) * FD_WARPS;
+    static_assert(NTABLES >= 2 && NTABLES * 4 <= FD_POOL_HDR && SMEM_BYTES <= (size_t)FD_SMEM_MAX, "table pool");
+};
+#define FD_NTABLES (DmPool<CLS>::NTABLES)
 
 // shared-memory ADDRESS of the H01 entry of a pixel pair in THIS walk (inside the grid and on the walk's
 // side of chi_i = chi_j: sgn = 0 for chi_i >= chi_j, -1 otherwise); everything else -> the garbage entry.
@@ -115,8 +135,8 @@ __device__ __forceinline__ unsigned dm_key(const BinParams &bp, const PairBin &g
 
 // pass A over rows [r0, r1] (a multiple of D rows; rows >= len are sentinels) and diagonals [dlo, dhi].
 // `key`/`cur` are shared-memory addresses of H01 entries; H23 sits at a fixed offset.
-template <int D, bool POW2, bool CHECK>
-__device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi,
+template <int D, bool POW2, bool CHECK, int CLS>
+__device__ __forceinline__ void dm_walk(DmFastWarp<CLS> &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi, int ds,
                                         int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned npar,
                                         int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
@@ -124,8 +144,14 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, int r0, in
     const double2 *qce = ws.qce + FD_PAD;
     const double *qeg = ws.qeg + FD_PAD;
     const unsigned garbage = h01 + ((npar * LYA_NCOL) << 4);
-    for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
-        const int dl = d0 + lane * D;
+    // D == 1: blocks of 32 * ds diagonals, ds passes per block (one per residue), lane l on diagonal d0 + ds * l;
+    // D == 2 (ds == 1 only): blocks of 64 diagonals, lane l on diagonals d0 + 2 l and d0 + 2 l + 1.
+    const int step = (D == 1) ? ds : D, n_res = (D == 1) ? ds : 1;
+    const int n_pass = ((dhi - dlo) / (32 * step) + 1) * n_res;
+    for (int pass = 0; pass < n_pass; ++pass) {
+        const int d0 = dlo + (pass / n_res) * (32 * step) + pass % n_res;
+        if (d0 > dhi) continue;
+        const int dl = d0 + lane * step;
         unsigned cur[D], key[D];
         double h0[D], h1[D], h2[D], h3[D], fa[D], fg[D];
         double wc[D], wa[D], wg[D];                         // sliding window over q: chi, ea, eg
@@ -210,15 +236,15 @@ __device__ __forceinline__ void dm_walk(DmFastWarp &ws, unsigned h01, int r0, in
     }
 }
 
-template <bool POW2, bool CHECK>
-__device__ __forceinline__ void dm_walk_any(DmFastWarp &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi,
+template <bool POW2, bool CHECK, int CLS>
+__device__ __forceinline__ void dm_walk_any(DmFastWarp<CLS> &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi, int ds,
                                             int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned npar,
                                             int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
     if (dhi < dlo) return;
     const int nd = dhi - dlo + 1;
-    if (nd <= 32) dm_walk<1, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
-    else dm_walk<2, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
+    if (nd <= 32 || ds > 1) dm_walk<1, POW2, CHECK, CLS>(ws, h01, r0, r1, mq, dlo, dhi, ds, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
+    else dm_walk<2, POW2, CHECK, CLS>(ws, h01, r0, r1, mq, dlo, dhi, 1, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
 }
 
 // transposed bin index b_perp * n_par + b_par of a pixel pair KNOWN to be inside the grid (exact windows)
@@ -251,8 +277,8 @@ __device__ __forceinline__ void dm_red(double *addr, double v)
 // Dn has n_bins^2 <= 2^24 entries, so element indices are 32-bit and an address is one IMAD.WIDE away.
 // (Tried and dropped: keeping each lane's rows / columns in registers for the whole drain -- fewer shared-memory
 // wavefronts, but the extra live registers spilled and it was 3-9 % slower.)
-template <bool POW2>
-__device__ __forceinline__ void dm_drain_t123(DmFastWarp &ws, unsigned *kept, int n, int mp, const DmFastParams &P,
+template <bool POW2, int CLS>
+__device__ __forceinline__ void dm_drain_t123(DmFastWarp<CLS> &ws, unsigned *kept, int n, int mp, const DmFastParams &P,
                                               const PairBin &g, long long offp, long long offq, int lane,
                                               bool scatter, unsigned &n_red)
 {
@@ -315,7 +341,8 @@ __device__ __forceinline__ void dm_drain_t123(DmFastWarp &ws, unsigned *kept, in
 #define LYA_FD_T4B 4
 #endif
 constexpr int FD_T4B = LYA_FD_T4B;
-__device__ __forceinline__ void dm_drain_t4(DmFastWarp &ws, DmTable &tb, const unsigned *kept, int n, int nnz,
+template <int CLS>
+__device__ __forceinline__ void dm_drain_t4(DmFastWarp<CLS> &ws, DmTable &tb, const unsigned *kept, int n, int nnz,
                                             const DmFastParams &P, int c0, int lane, bool wipe_after, unsigned &n_red)
 {
     const unsigned nb = (unsigned)(P.bp.n_par * P.bp.n_perp);
@@ -350,6 +377,7 @@ __device__ __forceinline__ void dm_drain_t4(DmFastWarp &ws, DmTable &tb, const u
 }
 
 // table pool: lane 0 claims a free table (owner flag 0 -> 1), probing round-robin from the warp's own slot
+template <int CLS>
 __device__ __forceinline__ int dm_table_acquire(int *owner, int wid, int lane)
 {
     int t = 0;
@@ -370,14 +398,14 @@ __device__ __forceinline__ void dm_table_release(int *owner, int t, int lane)
     if (lane == 0) { __threadfence_block(); atomicExch(&owner[t], 0); }
 }
 
-template <bool POW2, bool CHECK>
+template <bool POW2, bool CHECK, int CLS>
 __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     int *owner = (int *)smem_raw;
     DmTable *tables = (DmTable *)(smem_raw + FD_POOL_HDR);
-    DmFastWarp &ws = ((DmFastWarp *)(smem_raw + FD_POOL_HDR + sizeof(DmTable) * FD_NTABLES))[wid];
+    DmFastWarp<CLS> &ws = ((DmFastWarp<CLS> *)(smem_raw + FD_POOL_HDR + sizeof(DmTable) * FD_NTABLES))[wid];
     const BinParams bp = P.bp;
     const unsigned npar = (unsigned)bp.n_par;
     const int n_slots = bp.n_par * LYA_NCOL;                  // real slots; slot n_slots is the garbage entry
@@ -423,8 +451,9 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             const PairBin g = lya_make_pairbin(bp, s, c);
             int c0;
             const int key = lya_pair_key<POW2>(bp, g, hp, hq, c0);
-            if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
+            if (key >= 2 * bp.n_perp) continue;              // cannot happen in the fast ranges
             const unsigned lim = (unsigned)min(LYA_NCOL, bp.n_perp - c0);
+            const int ds = lya_pair_stride(bp, g, hq);              // lanes of a row step sit ds pixels of q apart
             __syncwarp();
             // ---- stage p (when it changes) and q: (chi, ea) pairs with 16-byte loads, eg, q's stage-4 keys ----
             if (p != cur_p) {
@@ -473,19 +502,23 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 // takes entries [l K, (l + 1) K), K = ceil(M / 32).  pre[] (rows before i) is a warp scan with three
                 // consecutive rows per lane; a lane finds its first row by binary search and then walks along,
                 // stepping to the next non-empty row when its window ends.
-                const int r3 = 3 * lane;
-                unsigned w0 = 0, w1 = 0, w2 = 0;
-                if (r3 < mp) w0 = (unsigned)ws.jhi[r3] - ws.jlo[r3];
-                if (r3 + 1 < mp) w1 = (unsigned)ws.jhi[r3 + 1] - ws.jlo[r3 + 1];
-                if (r3 + 2 < mp) w2 = (unsigned)ws.jhi[r3 + 2] - ws.jlo[r3 + 2];
-                unsigned incl = w0 + w1 + w2;
+                const int r3 = FD_RPL * lane;
+                unsigned wrow[FD_RPL], incl = 0;
+#pragma unroll
+                for (int k = 0; k < FD_RPL; ++k) {
+                    wrow[k] = (r3 + k < mp) ? (unsigned)ws.jhi[r3 + k] - ws.jlo[r3 + k] : 0u;
+                    incl += wrow[k];
+                }
+                const unsigned own = incl;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) { const unsigned v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
                 const unsigned M = __shfl_sync(0xffffffffu, incl, 31);
-                const unsigned excl = incl - (w0 + w1 + w2);
-                if (r3 <= mp) ws.u.a.pre[r3] = (unsigned short)excl;
-                if (r3 + 1 <= mp) ws.u.a.pre[r3 + 1] = (unsigned short)(excl + w0);
-                if (r3 + 2 <= mp) ws.u.a.pre[r3 + 2] = (unsigned short)(excl + w0 + w1);
+                unsigned run = incl - own;
+#pragma unroll
+                for (int k = 0; k < FD_RPL; ++k) {
+                    if (r3 + k <= mp) ws.u.a.pre[r3 + k] = (unsigned short)run;
+                    run += wrow[k];
+                }
                 for (int t = lane; t < mp; t += 32) ws.u.a.pk[t] = lya_key_lo(P.seed, (unsigned long long)(hp.pix0 + t));
                 if (lane == 0) { ws.jlo[mp] = 0; ws.jhi[mp] = 0xff; }          // stop row: never left, never counted
                 __syncwarp();
@@ -498,13 +531,13 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                     row = lo;
                 }
                 int j = (int)ws.jlo[row] + (int)(first - ws.u.a.pre[row]);
-                int jend = ws.jhi[row];
+                int jend = (row >= mp) ? (1 << 30) : (int)ws.jhi[row];
                 unsigned long long pki = ws.u.a.pk[min(row, FD_T - 1)];
                 const unsigned n_it = __reduce_max_sync(0xffffffffu, last - first);
                 for (unsigned t = 0; t < n_it; ++t) {
                     if (j >= jend) {                             // next non-empty row (the stop row ends the search)
                         do { ++row; } while (ws.jlo[row] == ws.jhi[row]);
-                        j = ws.jlo[row]; jend = ws.jhi[row];
+                        j = ws.jlo[row]; jend = (row >= mp) ? (1 << 30) : (int)ws.jhi[row];
                         pki = ws.u.a.pk[min(row, FD_T - 1)];
                     }
                     const unsigned h = lya_pair_hash32(pki, ws.u.a.qk[min(j, FD_T - 1)]);
@@ -526,11 +559,11 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             const int n_q0 = overflow ? 0 : (int)nk;
             unsigned n_red32 = 0;
             for (int e0 = 0; e0 < n_q0; e0 += FD_KBATCH) {
-                dm_drain_t123<POW2>(ws, ws.kept + e0, min(FD_KBATCH, n_q0 - e0), mp, P, g, hp.off, hq.off, lane, true, n_red32);
+                dm_drain_t123<POW2, CLS>(ws, ws.kept + e0, min(FD_KBATCH, n_q0 - e0), mp, P, g, hp.off, hq.off, lane, true, n_red32);
                 __syncwarp();
             }
             // ---- pass A: H tables, in a table of the pool ----
-            const int tix = dm_table_acquire(owner, wid, lane);
+            const int tix = dm_table_acquire<CLS>(owner, wid, lane);
             DmTable &tb = tables[tix];
             const unsigned h01 = (unsigned)__cvta_generic_to_shared(tb.H01);
             for (int i0 = 0; i0 < mp; i0 += FD_ROWS) {
@@ -553,7 +586,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
 #ifdef LYA_ABL_NO_WALK
                     continue;
 #endif
-                    dm_walk_any<POW2, CHECK>(ws, h01, r0 & ~1, r1 | 1, mq, sgn ? nlo : plo, sgn ? nhi : phi, sgn, bp, g,
+                    dm_walk_any<POW2, CHECK, CLS>(ws, h01, r0 & ~1, r1 | 1, mq, sgn ? nlo : plo, sgn ? nhi : phi, ds, sgn, bp, g,
                                              (unsigned)c0, lim, npar, lane, evaluated, conflicts);
                 }
             }
@@ -575,12 +608,12 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             // ---- pass C, second half: T4 (and, in the overflow case, the whole drain batch by batch) ----
             if (!overflow) {
                 if (n_q0 <= FD_KBATCH) {                     // the coefficients of the only batch are still in place
-                    dm_drain_t4(ws, tb, ws.kept, n_q0, nnz, P, c0, lane, true, n_red32);
+                    dm_drain_t4<CLS>(ws, tb, ws.kept, n_q0, nnz, P, c0, lane, true, n_red32);
                 } else {
                     for (int e0 = 0; e0 < n_q0; e0 += FD_KBATCH) {
                         const int nb_e = min(FD_KBATCH, n_q0 - e0);
-                        dm_drain_t123<POW2>(ws, ws.kept + e0, nb_e, mp, P, g, hp.off, hq.off, lane, false, n_red32);
-                        dm_drain_t4(ws, tb, ws.kept + e0, nb_e, nnz, P, c0, lane, e0 + FD_KBATCH >= n_q0, n_red32);
+                        dm_drain_t123<POW2, CLS>(ws, ws.kept + e0, nb_e, mp, P, g, hp.off, hq.off, lane, false, n_red32);
+                        dm_drain_t4<CLS>(ws, tb, ws.kept + e0, nb_e, nnz, P, c0, lane, e0 + FD_KBATCH >= n_q0, n_red32);
                         __syncwarp();
                     }
                 }
@@ -604,8 +637,8 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                     __syncwarp();
                     for (int e0 = 0; e0 < n_q || e0 == 0; e0 += FD_KBATCH) {
                         const int nb_e = max(min(FD_KBATCH, n_q - e0), 0);
-                        dm_drain_t123<POW2>(ws, ws.kept + e0, nb_e, mp, P, g, hp.off, hq.off, lane, true, n_red32);
-                        dm_drain_t4(ws, tb, ws.kept + e0, nb_e, nnz, P, c0, lane, done && e0 + FD_KBATCH >= n_q, n_red32);
+                        dm_drain_t123<POW2, CLS>(ws, ws.kept + e0, nb_e, mp, P, g, hp.off, hq.off, lane, true, n_red32);
+                        dm_drain_t4<CLS>(ws, tb, ws.kept + e0, nb_e, nnz, P, c0, lane, done && e0 + FD_KBATCH >= n_q, n_red32);
                         __syncwarp();
                     }
                     if (done) break;
@@ -635,3 +668,12 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
 }
 
 }  // namespace
+
+#undef FD_WARPS
+#undef FD_THREADS
+#undef FD_T
+#undef FD_TP
+#undef FD_TQ
+#undef FD_KCAP
+#undef FD_RPL
+#undef FD_NTABLES

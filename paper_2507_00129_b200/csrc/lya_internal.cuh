@@ -78,15 +78,19 @@ void lya_prep_free(LyaPrep *p);
 
 // ---- pair bucketing (prep.cu) -----------------------------------------------------------
 // Stable counting sort of the forest-pair list by the r_perp column of the pair's first
-// pixel pair (c_first).  Keys: 0..n_perp-1 = fast-path pairs whose bins lie in columns
-// [c_first, c_first + LYA_NCOL); n_perp = pairs for the generic kernels (long forests, wide
-// column span, spacing below the bin width); n_perp+1 = pairs with nothing inside the grid.
+// pixel pair (c_first).  Keys: 0..n_perp-1 = class-0 fast pairs (forests of up to LYA_FAST_TILE pixels whose
+// spacing exceeds the r_par bin width; bins in columns [c_first, c_first + LYA_NCOL)); n_perp..2 n_perp-1 =
+// class-1 fast pairs (up to LYA_FAST_TILE2 pixels, any spacing down to bin width / 8: the D kernel's second
+// size class; the xi kernel sends them to its generic kernel); 2 n_perp = pairs for the generic kernels (longer
+// forests, wider column span); 2 n_perp + 1 = pairs with nothing inside the grid.
 #define LYA_NCOL 6                  // r_perp columns of a warp-private sub-histogram
-#define LYA_FAST_TILE 72            // longest forest the fast kernels stage in one piece
+#define LYA_FAST_TILE 72            // longest forest the class-0 fast kernels stage in one piece
+#define LYA_FAST_TILE2 144          // same for class 1 (native-resolution shapes, DESIGN.md NEXT-3)
+#define LYA_DS_MAX 8                // largest diagonal stride (bin width / pixel spacing, rounded up) of class 1
 struct LyaBuckets {
     int32_t *pq;                    // device [n][2], sorted by key (stable)
     int64_t n;
-    int64_t n_fast, n_generic, n_skip;
+    int64_t n_fast, n_fast2, n_generic, n_skip;   // sizes of the four ranges of the sorted list, in this order
     unsigned long long visited;     // sum n_p * n_q over the whole list
     int bad_pair;                   // LYA_DEV_BAD_PAIR: a pair outside [0, n_forest); LYA_DEV_DEGENERATE: a listed degenerate forest
 };
@@ -246,22 +250,34 @@ __device__ __forceinline__ int lya_col_of(const BinParams &bp, const PairBin &g,
     }
 }
 
-// Can the fast kernels take this forest pair?  (warp-uniform; identical in the bucketing
-// pass and in the kernels.)  c_first: column of the pair's first pixels.  Returns the key.
+// Diagonal stride of a forest pair: the smallest ds with ds * (smallest pixel spacing of q) > r_par bin width
+// (margin 1e-6).  Lanes of one row step that sit ds pixels of q apart then hold pairs in different r_par bins on
+// each side of chi_i = chi_j.  Returns a large number for a single-pixel q.
+__device__ __forceinline__ int lya_pair_stride(const BinParams &bp, const PairBin &g, const ForestHead &hq)
+{
+    const double x = __dmul_rn(__dmul_rn(hq.dmin, g.c), bp.inv_par);     // spacing in bin widths
+    if (x > 1.000001) return 1;
+    if (!(x > 1.000001 / 64.0)) return 64;
+    return (int)(1.000001 / x) + 1;
+}
+
+// Which kernel takes this forest pair?  (warp-uniform; identical in the bucketing pass and in the kernels.)
+// c_first: column of the pair's first pixels.  Returns the bucket key (see LyaBuckets).
 template <bool POW2>
 __device__ __forceinline__ int lya_pair_key(const BinParams &bp, const PairBin &g, const ForestHead &hp,
                                             const ForestHead &hq, int &c_first)
 {
     c_first = bp.n_perp;
-    if (hp.len == 0 || hq.len == 0) return bp.n_perp + 1;
+    if (hp.len == 0 || hq.len == 0) return 2 * bp.n_perp + 1;
     c_first = lya_col_of<POW2>(bp, g, __dadd_rn(hp.chi0, hq.chi0));
-    if (c_first >= bp.n_perp) return bp.n_perp + 1;                 // r_perp grows with both pixels
+    if (c_first >= bp.n_perp) return 2 * bp.n_perp + 1;             // r_perp grows with both pixels
     int c_last = lya_col_of<POW2>(bp, g, __dadd_rn(hp.chi1, hq.chi1));
     if (c_last >= bp.n_perp) c_last = bp.n_perp - 1;
-    bool fast = (hp.len <= LYA_FAST_TILE) && (hq.len <= LYA_FAST_TILE) && (c_last - c_first < LYA_NCOL);
-    // lanes of one flush hold pixel pairs (i, j_lane) with distinct j: their r_par bins differ
-    // when the spacing of q exceeds the bin width (margin 1e-6), see DESIGN.md "conflict-free runs"
-    fast = fast && (__dmul_rn(__dmul_rn(hq.dmin, g.c), bp.inv_par) > 1.000001);
-    return fast ? c_first : bp.n_perp;
+    if (c_last - c_first >= LYA_NCOL) return 2 * bp.n_perp;
+    const int len = max(hp.len, hq.len);
+    const int ds = lya_pair_stride(bp, g, hq);
+    if (len <= LYA_FAST_TILE && ds == 1) return c_first;
+    if (len <= LYA_FAST_TILE2 && ds <= LYA_DS_MAX) return bp.n_perp + c_first;
+    return 2 * bp.n_perp;
 }
 #endif

@@ -261,6 +261,30 @@ def test_one_holder_invariant_debug_variant(B, orc):
     c.close()
 
 
+@pytest.mark.parametrize("cfg,fine,n,frac", [(2, 2, 150, 0.97), (4, 2, 120, 0.99), (0, 4, 64, 0.9), (0, 6, 40, 0.5)])
+def test_native_resolution_fast_class_next3(B, orc, cfg, fine, n, frac):
+    """NEXT-3 shapes: pixel spacing BELOW the r_par bin width (3.3 Mpc/h at fine = 2, the SDSS spacing of
+    PAPER.md:142; 1.6 / 1.1 Mpc/h at fine = 4 / 6) and forests of up to 144 pixels take the second size class of
+    the fast D kernel (diagonal stride 2..4).  D and xi against the naive oracle; the debug variant also checks
+    that no H-table entry ever has two holders."""
+    f = gen.make_config(cfg, n_forest=n, density_scale=4.0, fine=fine)
+    assert np.diff(f.pix_off).max() <= 144 and np.diff(f.chi)[np.diff(f.chi) > 0].min() < 4.0
+    seed = gen.mask_seed(cfg)
+    ref = orc.pairs_window(f)
+    od, ox = orc.dmat(f, ref, frac, seed), orc.xi(f, ref)
+    for check in (1, 0):
+        c = B.Context("cuda:0")
+        c.lya_set_option("check_holders", check)
+        d = B.DeviceForests(f)
+        pairs = c.lya_neighbours(d, B.binning())
+        assert pairs.n == len(ref)
+        g = c.lya_dmat(d, B.binning(), pairs, frac, seed)
+        check_dmat(g, od, f"cfg{cfg} fine={fine} check={check}")
+        assert g["stats"]["n_scatter"] > 0.5 * od["n_kept"]           # the fast kernel took (most of) the pairs
+        check_xi(c.lya_xi2pcf(d, B.binning(), pairs), ox, f"cfg{cfg} fine={fine} xi")
+        c.close()
+
+
 def test_forest_pair_subsampling_next2(ctx, B, orc):
     """D from a subset of FOREST pairs = lya_pairs_subsample + lya_dmat(f = 0)."""
     f = gen.make_config(1, n_forest=150, density_scale=4.0)
