@@ -58,7 +58,8 @@ typedef enum {
 
 /* Forest catalogue, CSR over pixels (a skewer = sky position + a
  * variable-length table of delta, weight, wavelength).
- *   ux,uy,uz: unit vectors of the sightlines.  They are INPUTS (like chi) so that
+ *   ux,uy,uz: unit vectors of the sightlines (|u|^2 = 1 to 1e-9, else LYA_ERR_INVALID_ARG).  They are INPUTS
+ *     (like chi) so that
  *     both this library and a checker consume identical values; pass NULL for all
  *     three to have them derived on the device from ra/dec (not bit-reproducible
  *     against a host libm).  ra/dec [radians] may be NULL when ux,uy,uz are given.
@@ -77,7 +78,8 @@ typedef struct {
 } lya_forests;
 
 /* (r_par, r_perp) grid (4 Mpc/h bins up to 200 Mpc/h -> 50 x 50).
- * Requires 0 < r*_max, 1 <= n_* and n_par*n_perp <= 4096, bin width >= 0.01. */
+ * Requires 0 < r*_max <= 1e5, 1 <= n_* and n_par*n_perp <= 4096, bin width >= 0.01 (LYA_ERR_CAPACITY
+ * otherwise); the fast kernels also need n_par <= 50 and n_perp <= 127, other grids take the generic ones. */
 typedef struct {
     double rpar_max, rperp_max;
     int32_t n_par, n_perp;
@@ -118,8 +120,14 @@ uint64_t    lya_launch_count(void);
  *                             row step that no two lanes of a warp hold the same table entry (the invariant
  *                             their atomic-free accumulation rests on).  Much slower; a
  *                             violation makes the call return LYA_ERR_CUDA with the count in lya_last_error.
+ *   LYA_OPT_XI_MERGE_EVERY    1 .. 2^31 (default 2^31): a warp of the fast xi kernel merges its private
+ *                             sub-histogram into the global accumulators after this many visited pixel pairs
+ *                             even when its bucket does not change -- the guard that keeps its 32-bit pair
+ *                             counters from overflowing.  No workload of this size reaches the default, so a
+ *                             test lowers it to drive the guard; results do not depend on it.
  * LYA_ERR_INVALID_ARG for an unknown option or value. */
-typedef enum { LYA_OPT_FORCE_GENERIC = 0, LYA_OPT_GENERIC_DIAGONALS = 1, LYA_OPT_CHECK_HOLDERS = 2 } lya_option;
+typedef enum { LYA_OPT_FORCE_GENERIC = 0, LYA_OPT_GENERIC_DIAGONALS = 1, LYA_OPT_CHECK_HOLDERS = 2,
+               LYA_OPT_XI_MERGE_EVERY = 3 } lya_option;
 lya_status  lya_set_option(lya_ctx *ctx, lya_option opt, int64_t value);
 
 /* ---- stage 1: neighbour search (north_star stage 1) ------------ */
@@ -154,7 +162,7 @@ void       lya_pairs_free(lya_ctx *ctx, lya_pairs *pairs);
 /* S, W: double [n_par*n_perp]; N: uint64 [n_par*n_perp]; xi: double [n_par*n_perp]
  * (xi_A = S_A / W_A, 0 where W_A == 0); row-major [b_par][b_perp].  Any of S, W,
  * N, xi may be NULL.  Each unordered pixel pair of each listed forest pair counts
- * once.  stats: host out, may be NULL (when non-NULL the call synchronises). */
+ * once.  stats: host out, may be NULL.  The call synchronises the ctx stream either way. */
 lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                       const lya_pairs *pairs,
                       double *S, double *W, uint64_t *N, double *xi, lya_stats *stats);

@@ -20,7 +20,7 @@ EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_la
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
           4: "LYA_ERR_CAPACITY", 5: "LYA_ERR_OOM", 6: "LYA_ERR_CUDA", 7: "LYA_ERR_UNIMPLEMENTED"}
-OPTIONS = {"force_generic": 0, "generic_diagonals": 1, "check_holders": 2}
+OPTIONS = {"force_generic": 0, "generic_diagonals": 1, "check_holders": 2, "xi_merge_every": 3}
 
 
 class LyaError(RuntimeError):

@@ -48,6 +48,7 @@ extern "C" lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     ctx->force_generic = 0;
     ctx->generic_diagonals = 2;
     ctx->check_holders = 0;
+    ctx->xi_merge_every = 1ull << 31;
     ctx->err[0] = 0;
     *out = ctx;
     return LYA_OK;
@@ -76,6 +77,10 @@ extern "C" lya_status lya_set_option(lya_ctx *ctx, lya_option opt, int64_t value
         if (value != 1 && value != 2 && value != 4) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "LYA_OPT_GENERIC_DIAGONALS takes 1, 2 or 4");
         ctx->generic_diagonals = (int)value;
         return LYA_OK;
+    case LYA_OPT_XI_MERGE_EVERY:
+        if (value < 1 || value > ((int64_t)1 << 31)) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "LYA_OPT_XI_MERGE_EVERY takes 1 .. 2^31");
+        ctx->xi_merge_every = (unsigned long long)value;
+        return LYA_OK;
     case LYA_OPT_CHECK_HOLDERS:
         if (value != 0 && value != 1) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "LYA_OPT_CHECK_HOLDERS takes 0 or 1");
         ctx->check_holders = (int)value;
@@ -96,6 +101,9 @@ lya_status lya_check_binning(lya_ctx *ctx, const lya_binning *b)
                         (long long)b->n_par * b->n_perp, LYA_MAX_BINS);
     if (b->rpar_max / b->n_par < 0.01 || b->rperp_max / b->n_perp < 0.01)
         return lya_fail(ctx, LYA_ERR_CAPACITY, "binning: bin width below 0.01");
+    // padding / sentinel pixels sit at chi = 1e7 and 2e7 and must stay far outside any grid
+    if (b->rpar_max > 1e5 || b->rperp_max > 1e5)
+        return lya_fail(ctx, LYA_ERR_CAPACITY, "binning: r*_max above 1e5");
     return LYA_OK;
 }
 
@@ -142,7 +150,8 @@ __global__ void k_validate(lya_forests f, bool need_delta, bool need_loglam, uns
         prev = c;
     }
     if (f.ux) {
-        if (!(isfinite(f.ux[p]) && isfinite(f.uy[p]) && isfinite(f.uz[p]))) err = max(err, (unsigned)LYA_DEV_NONFINITE);
+        const double n2 = f.ux[p] * f.ux[p] + f.uy[p] * f.uy[p] + f.uz[p] * f.uz[p];
+        if (!(isfinite(n2) && fabs(n2 - 1.0) <= 1e-9)) err = max(err, (unsigned)LYA_DEV_NONFINITE);   // finite and of unit length
     } else if (f.ra) {
         if (!(isfinite(f.ra[p]) && isfinite(f.dec[p]))) err = max(err, (unsigned)LYA_DEV_NONFINITE);
     }
@@ -171,7 +180,7 @@ lya_status lya_validate_forests(lya_ctx *ctx, const lya_forests *f, bool need_de
     switch (err) {
     case LYA_DEV_OK: return LYA_OK;
     case LYA_DEV_BAD_OFFSETS: return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pix_off must start at 0, be non-decreasing and end at n_pix");
-    case LYA_DEV_NONFINITE: return lya_fail(ctx, LYA_ERR_INVALID_ARG, "non-finite input, w < 0, or chi outside [0, 1e6)");
+    case LYA_DEV_NONFINITE: return lya_fail(ctx, LYA_ERR_INVALID_ARG, "non-finite input, w < 0, chi outside [0, 1e6), or a sightline vector that is not of unit length (1e-9)");
     case LYA_DEV_UNSORTED: return lya_fail(ctx, LYA_ERR_UNSORTED, "chi is not strictly increasing inside a forest");
     case LYA_DEV_TOO_LONG: return lya_fail(ctx, LYA_ERR_CAPACITY, "a forest has more than 2^20 pixels");
     default: return lya_fail(ctx, LYA_ERR_INVALID_ARG, "catalogue validation failed (%u)", err);

@@ -20,6 +20,7 @@ struct lya_ctx {
     unsigned long long *d_counters;   // [16] work counters / flags
     int force_generic;                // LYA_OPT_FORCE_GENERIC: route every pair to the generic kernels
     int check_holders;                // LYA_OPT_CHECK_HOLDERS: debug variant of the fast kernels that asserts the one-holder invariant
+    unsigned long long xi_merge_every; // LYA_OPT_XI_MERGE_EVERY: visited pairs between forced merges of a warp's sub-histogram
     int generic_diagonals;            // LYA_OPT_GENERIC_DIAGONALS: diagonals per lane of the generic xi kernel (1, 2, 4)
     cudaEvent_t ev[4];
 };

@@ -161,18 +161,38 @@ __global__ void k_cell_scatter(const int *cell_of, int64_t n, const unsigned lon
     sorted_id[cell_start[c] + slot] = (int)p;
 }
 
-// deterministic order inside a cell: insertion sort by forest id (cells are small)
+// deterministic order inside a cell: sort by forest id (insertion sort for the usual small cells, an in-place
+// heap sort for crowded ones, e.g. a whole catalogue in one cell when the admissible chord exceeds the sphere)
 __global__ void k_cell_sort(const unsigned long long *cell_start, int64_t n_cells, int *sorted_id)
 {
     int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (c >= n_cells) return;
-    int64_t a = cell_start[c], b = cell_start[c + 1];
-    if (b - a < 2 || b - a > 4096) return;
-    for (int64_t i = a + 1; i < b; ++i) {
-        int v = sorted_id[i];
-        int64_t j = i - 1;
-        while (j >= a && sorted_id[j] > v) { sorted_id[j + 1] = sorted_id[j]; --j; }
-        sorted_id[j + 1] = v;
+    const int64_t a = cell_start[c], n = (int64_t)cell_start[c + 1] - a;
+    if (n < 2) return;
+    int *v = sorted_id + a;
+    if (n <= 64) {
+        for (int64_t i = 1; i < n; ++i) {
+            const int x = v[i];
+            int64_t j = i - 1;
+            while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; --j; }
+            v[j + 1] = x;
+        }
+        return;
+    }
+    auto sift = [&](int64_t root, int64_t end) {            // max-heap on v[0, end)
+        for (;;) {
+            int64_t child = 2 * root + 1;
+            if (child >= end) break;
+            if (child + 1 < end && v[child + 1] > v[child]) ++child;
+            if (v[root] >= v[child]) break;
+            const int t = v[root]; v[root] = v[child]; v[child] = t;
+            root = child;
+        }
+    };
+    for (int64_t i = n / 2 - 1; i >= 0; --i) sift(i, n);
+    for (int64_t end = n - 1; end > 0; --end) {
+        const int t = v[0]; v[0] = v[end]; v[end] = t;
+        sift(0, end);
     }
 }
 

@@ -327,6 +327,7 @@ struct XiFastParams {
     unsigned long long *counters;            // [4] next chunk, [2] evaluated
     const int32_t *region;                   // NULL, or the sub-sample (sky region) of every forest (NEXT-1)
     int n_region;
+    unsigned long long merge_every;          // visited pixel pairs after which a warp merges its sub-histogram (u32 counters)
 };
 
 // Sub-histogram slot = col_rel * 2 (n_par + 1) + side * (n_par + 1) + row.
@@ -394,10 +395,10 @@ __device__ __forceinline__ unsigned xi_key(const BinParams &bp, const PairBin &g
 // width), so an entry has one holder at a time; all releases of a row come before its acquires (warp
 // barrier in between).  The keys of row i+1 are computed between the acquire of row i and the FMAs
 // that need it.  r1 - r0 + 1 is a multiple of D; rows >= mp of p are sentinels.
-template <int D, bool POW2>
+template <int D, bool POW2, bool CHECK>
 __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
                                         int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
-                                        unsigned np1, int lane, unsigned long long &evaluated)
+                                        unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
     const double *qc = ws.qc + FPAD, *qa = ws.qa + FPAD, *qw = ws.qw + FPAD;
     const unsigned garbage = (np1 - 1u) * 16u;              // entry (column 0, side 0, row n_par)
@@ -426,6 +427,17 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
             for (int u = 0; u < D; ++u) {
                 const int i = ib + u;                       // window slot of q[i + dl + k] is (k + u) % D
                 bool ch[D];
+                if (CHECK) {                                // invariant: a non-garbage entry has one holder (debug runs only)
+                    for (int src = 0; src < 32; ++src)
+#pragma unroll
+                        for (int k2 = 0; k2 < D; ++k2) {
+                            const unsigned other = __shfl_sync(0xffffffffu, key[k2], src);
+#pragma unroll
+                            for (int k = 0; k < D; ++k)
+                                if (other == key[k] && key[k] != garbage && key[k] != garbage + np1 * 16u &&   // (row n_par of either side is garbage)
+                                    (src < lane || (src == lane && k2 < k))) conflicts += 1u;
+                        }
+                }
 #pragma unroll
                 for (int k = 0; k < D; ++k) {
                     ch[k] = key[k] != cur[k];
@@ -473,15 +485,15 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
     }
 }
 
-template <bool POW2>
+template <bool POW2, bool CHECK>
 __device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
                                             int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
-                                            unsigned np1, int lane, unsigned long long &evaluated)
+                                            unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
     const int nd = dhi - dlo + 1;
-    if (nd <= 32) xi_walk<1, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
-    else if (nd <= 64) xi_walk<2, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
-    else xi_walk<4, POW2>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated);
+    if (nd <= 32) xi_walk<1, POW2, CHECK>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts);
+    else if (nd <= 64) xi_walk<2, POW2, CHECK>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts);
+    else xi_walk<4, POW2, CHECK>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts);
 }
 
 // merge a warp's sub-histogram (first column c0) into the global accumulators and clear it
@@ -509,7 +521,7 @@ __device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, in
     __syncwarp();
 }
 
-template <bool POW2>
+template <bool POW2, bool CHECK>
 __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -524,6 +536,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
     const double *qc = ws.qc + FPAD;
     const unsigned sw_base = (unsigned)__cvta_generic_to_shared(ws.SW), n_base = (unsigned)__cvta_generic_to_shared(ws.N);
     unsigned long long evaluated = 0, since_merge = 0;
+    unsigned conflicts = 0;
     int cur_p = -1, head_p = -1, win_c0 = -1, win_reg = 0;
     ForestHead hp;
     hp.len = 0;
@@ -548,7 +561,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
             if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
             since_merge += (unsigned long long)mp * mq;
             const int reg = P.region ? P.region[p] : 0;       // a pixel pair belongs to the sub-sample of forest p
-            if (c0 != win_c0 || reg != win_reg || since_merge > (1ull << 31)) {
+            if (c0 != win_c0 || reg != win_reg || since_merge > P.merge_every) {
                 if (win_c0 >= 0) xi_merge(ws, P, win_c0, win_reg, lane);
                 win_c0 = c0; win_reg = reg; since_merge = (unsigned long long)mp * mq;
             }
@@ -603,7 +616,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
                 }
                 dlo = __reduce_min_sync(0xffffffffu, dlo); dhi = __reduce_max_sync(0xffffffffu, dhi);
                 r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
-                if (r1 >= r0) xi_walk_any<POW2>(ws, sw_base, n_base, r0 & ~3, r1 | 3, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated);
+                if (r1 >= r0) xi_walk_any<POW2, CHECK>(ws, sw_base, n_base, r0 & ~3, r1 | 3, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated, conflicts);
             }
         }
     }
@@ -611,6 +624,11 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) evaluated += __shfl_xor_sync(0xffffffffu, evaluated, o);
     if (lane == 0 && evaluated) atomicAdd(&P.counters[2], evaluated);
+    if (CHECK) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) conflicts += __shfl_xor_sync(0xffffffffu, conflicts, o);
+        if (lane == 0 && conflicts) atomicAdd(&P.counters[5], (unsigned long long)conflicts);
+    }
 }
 
 }  // namespace
@@ -675,15 +693,16 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
         F.prep = pl->prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
         F.S = P.S; F.W = P.W; F.N = P.N; F.counters = ctx->d_counters;
         F.region = region; F.n_region = n_reg;
+        F.merge_every = ctx->xi_merge_every;
         const size_t fsmem = sizeof(FastWarp) * FW;
         const int fgrid = ctx->sm_count;
-        if (bp.pow2) {
-            e = cudaFuncSetAttribute(k_xi_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (e == cudaSuccess) { k_xi_fast<true><<<fgrid, FTHREADS, fsmem, s>>>(F); lya_note_launch(); }
-        } else {
-            e = cudaFuncSetAttribute(k_xi_fast<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (e == cudaSuccess) { k_xi_fast<false><<<fgrid, FTHREADS, fsmem, s>>>(F); lya_note_launch(); }
-        }
+        auto launch = [&](auto kern) {
+            cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
+            if (le == cudaSuccess) { kern<<<fgrid, FTHREADS, fsmem, s>>>(F); lya_note_launch(); }
+            return le;
+        };
+        if (ctx->check_holders) e = bp.pow2 ? launch(k_xi_fast<true, true>) : launch(k_xi_fast<false, true>);
+        else e = bp.pow2 ? launch(k_xi_fast<true, false>) : launch(k_xi_fast<false, false>);
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_fast launch"); }
     }
@@ -691,7 +710,7 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
     const int grid = ctx->sm_count * 2;
     const int64_t n_chunks = (P.n_pairs + CHUNK - 1) / CHUNK;
     int launches = 0;
-    unsigned long long h[4] = {0, 0, 0, 0};
+    unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     if (region && P.n_pairs > 0) {                 // sub-sample mode: the block-level histogram of k_xi cannot be used
         const int dgrid = (int)((P.n_pairs + 7) / 8 < (int64_t)ctx->sm_count * 8 ? (P.n_pairs + 7) / 8 : (int64_t)ctx->sm_count * 8);
         if (bp.pow2) { k_xi_direct<true><<<dgrid, 256, 0, s>>>(P, region); lya_note_launch(); }
@@ -707,7 +726,7 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
         }
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi launch"); }
         ++launches;
-        e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
+        e = cudaMemcpyAsync(h, ctx->d_counters, 4 * sizeof(h[0]), cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi"); }
         if ((int64_t)h[0] >= n_chunks) break;      // every chunk claimed (warps stop at their u32 budget)
@@ -720,6 +739,7 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "lya_xi2pcf"); }
     if (h[3] != 0) { cleanup(); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)"); }
+    if (h[5] != 0) { cleanup(); return lya_fail(ctx, LYA_ERR_CUDA, "k_xi_fast: %llu sub-histogram entries had two holders (LYA_OPT_CHECK_HOLDERS)", h[5]); }
     if (stats) {
         memset(stats, 0, sizeof(*stats));
         stats->n_forest_pairs = (uint64_t)pl->n_pairs;

@@ -254,11 +254,25 @@ def test_one_holder_invariant_debug_variant(B, orc):
     c.lya_set_option("check_holders", 1)
     d = B.DeviceForests(f)
     pairs = c.lya_neighbours(d, B.binning())
+    check_xi(c.lya_xi2pcf(d, B.binning(), pairs), orc.xi(f, orc.pairs_window(f)), "check_holders xi")   # same check in k_xi_fast
     g = c.lya_dmat(d, B.binning(), pairs, 0.9, seed)          # raises LYA_ERR_CUDA on a violation
     ref = orc.pairs_window(f)
     check_dmat(g, orc.dmat(f, ref, 0.9, seed), "check_holders")
     assert g["stats"]["n_scatter"] > 0                        # the fast kernel ran
     c.close()
+
+
+def test_xi_merge_guard(B, orc):
+    """The guard that merges a warp's sub-histogram before its 32-bit pair counters can overflow (default: every
+    2^31 visited pairs, which no workload here reaches) is driven by lowering it: N stays bit-exact."""
+    f = gen.make_config(4, n_forest=800)
+    ref = orc.pairs_window(f)
+    o = orc.xi(f, ref)
+    for every in (1, 5000, 1 << 31):
+        c = B.Context("cuda:0")
+        c.lya_set_option("xi_merge_every", every)
+        check_xi(c.lya_xi2pcf(B.DeviceForests(f), B.binning(), c.lya_pairs_import(ref)), o, f"merge every {every}")
+        c.close()
 
 
 @pytest.mark.parametrize("cfg,fine,n,frac", [(2, 2, 150, 0.97), (4, 2, 120, 0.99), (0, 4, 64, 0.9), (0, 6, 40, 0.5)])
@@ -481,6 +495,21 @@ def test_error_statuses(ctx, B, cfg0):
     assert e.value.name == "LYA_ERR_INVALID_ARG"
     with pytest.raises(B.LyaError):
         ctx.lya_pairs_import([[3, 3]])
+    with pytest.raises(B.LyaError) as e:                               # sentinel pixels must stay outside any grid
+        ctx.lya_neighbours(B.DeviceForests(cfg0), B.binning(2.0e5, 200.0, 50, 50))
+    assert e.value.name == "LYA_ERR_CAPACITY"
+    notunit = gen.make_config(0); notunit.ux[3] *= 1.001
+    with pytest.raises(B.LyaError) as e:
+        ctx.lya_neighbours(B.DeviceForests(notunit), B.binning())
+    assert e.value.name == "LYA_ERR_INVALID_ARG"
+    # the degenerate-forest rule (reading R-7) is the same on the generic route: all L equal up to rounding
+    deg2 = gen.make_config(0); deg2.loglam[:24] = 3.6 + 4.5e-16 * np.arange(24)
+    cg = B.Context("cuda:0")
+    cg.lya_set_option("force_generic", 1)
+    with pytest.raises(B.LyaError) as e:
+        cg.lya_dmat(B.DeviceForests(deg2), B.binning(), cg.lya_pairs_import([[0, 1]]), 0.0, 1)
+    assert e.value.name == "LYA_ERR_DEGENERATE_FOREST"
+    cg.close()
 
 
 def test_zero_weights_count_geometrically(ctx, B, orc):
