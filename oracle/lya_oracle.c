@@ -541,3 +541,120 @@ int orc_dmat_collapsed(const orc_forests *f, const orc_binning *b, const int32_t
     if (n_kept) n_kept[0] = kept;
     return bad;
 }
+
+/* ==========================================================================================
+ * NEXT-4: brute-force anisotropic three-point correlation function, eq. 2.8:
+ *     xi3_A = sum_A (d_i w_i)(d_j w_j)(d_k w_k) / sum_A w_i w_j w_k,   i, j, k in DISTINCT quasars,
+ * binned in the five triangle variables of PAPER.md:108 and Fig. 2 / Fig. 5: the two
+ * sides r1, r2 from a main vertex, the inner angle alpha (binned in cos alpha) and the angles theta1,
+ * theta2 of the two sides to the line of sight.  "The same triangle is recorded ... depending on which
+ * point is taken as the main vertex".
+ *
+ * The paper fixes neither the vertex convention, nor the line of sight, nor the flattening; the readings
+ * (T1-T7), each operation one separately rounded binary64 operation, no FMA:
+ *  T1 position of a pixel: X = (chi ux, chi uy, chi uz) (flat universe, comoving Cartesian).
+ *  T2 every ORDERED triple (i; j, k) counts: i the main vertex, j the end of side 1, k the end of side 2,
+ *     the three pixels in three distinct forests (so a triangle enters 6 times: 3 vertices x 2 orders).
+ *  T3 side vectors d1 = X_j - X_i, d2 = X_k - X_i; r = sqrt(((dx dx) + (dy dy)) + (dz dz));
+ *     a side takes part iff 0 < r < r_max.
+ *  T4 line of sight = the unit vector u of the main vertex's forest;
+ *     cos theta = (((dx ux) + (dy uy)) + (dz uz)) / r;   cos alpha = (((d1x d2x) + (d1y d2y)) + (d1z d2z)) / (r1 r2).
+ *  T5 bins: b_r = (int)(r (n_r / r_max)) clamped to n_r - 1;
+ *     b_theta = number of m in 1..n_theta-1 with cos theta <= C_m, C_m = cos(m pi / n_theta) -- equal steps in
+ *     theta over [0, pi] without an arccos (libm's differs between host and device in the last bit); the
+ *     table C is an INPUT computed once by the caller, like chi;
+ *     b_alpha = (int)((cos alpha + 1) (n_cosa / 2)) clamped to [0, n_cosa - 1].
+ *  T6 triangle index A = (((b_r1 n_r + b_r2) n_cosa + b_alpha) n_theta + b_theta1) n_theta + b_theta2.
+ *  T7 sums: S3 += ((a_i a_j) a_k) with a = w d;  W3 += ((w_i w_j) w_k);  N3 += 1.
+ * The forest-pair list pq (p < q) only has to hold every pair of forests with two pixels closer than
+ * r_max (any superset gives the same sums); adjacency is taken from it in both directions. */
+typedef struct { double r_max; int32_t n_r, n_theta, n_cosa; } orc_tri_binning;
+
+static inline int tri_side(const orc_tri_binning *tb, const double *cosedge, const double xi[3], const double ui[3],
+                           double chi_j, const double uj[3], double d[3], double *r, int32_t *b_r, int32_t *b_t)
+{
+    double xj0 = chi_j * uj[0], xj1 = chi_j * uj[1], xj2 = chi_j * uj[2];
+    d[0] = xj0 - xi[0]; d[1] = xj1 - xi[1]; d[2] = xj2 - xi[2];
+    double r2 = ((d[0] * d[0]) + (d[1] * d[1])) + (d[2] * d[2]);
+    *r = sqrt(r2);
+    if (!(*r > 0.0) || !(*r < tb->r_max)) return 0;
+    double inv = (double)tb->n_r / tb->r_max;
+    int32_t br = (int32_t)(*r * inv);
+    if (br > tb->n_r - 1) br = tb->n_r - 1;
+    double ct = (((d[0] * ui[0]) + (d[1] * ui[1])) + (d[2] * ui[2])) / *r;
+    int32_t bt = 0;
+    for (int32_t m = 0; m < tb->n_theta - 1; ++m) bt += (ct <= cosedge[m]) ? 1 : 0;
+    *b_r = br; *b_t = bt;
+    return 1;
+}
+
+int64_t orc_tri_nbins(const orc_tri_binning *tb)
+{
+    return (int64_t)tb->n_r * tb->n_r * tb->n_cosa * tb->n_theta * tb->n_theta;
+}
+
+void orc_xi3(const orc_forests *f, const orc_tri_binning *tb, const double *cosedge, const int32_t *pq, int64_t n_pairs,
+             double *S3, double *W3, uint64_t *N3)
+{
+    int64_t nf = f->n_forest, nb = orc_tri_nbins(tb);
+    /* adjacency in both directions from the pair list */
+    int64_t *deg = (int64_t *)calloc((size_t)nf + 1, sizeof(int64_t));
+    for (int64_t k = 0; k < n_pairs; ++k) { deg[pq[2 * k] + 1]++; deg[pq[2 * k + 1] + 1]++; }
+    for (int64_t p = 0; p < nf; ++p) deg[p + 1] += deg[p];
+    int32_t *adj = (int32_t *)malloc(sizeof(int32_t) * (size_t)(2 * n_pairs + 1));
+    int64_t *cur = (int64_t *)malloc(sizeof(int64_t) * (size_t)(nf + 1));
+    memcpy(cur, deg, sizeof(int64_t) * (size_t)(nf + 1));
+    for (int64_t k = 0; k < n_pairs; ++k) {
+        adj[cur[pq[2 * k]]++] = pq[2 * k + 1];
+        adj[cur[pq[2 * k + 1]]++] = pq[2 * k];
+    }
+    long double *gS = (long double *)calloc((size_t)nb, sizeof(long double));
+    long double *gW = (long double *)calloc((size_t)nb, sizeof(long double));
+    memset(N3, 0, sizeof(uint64_t) * (size_t)nb);
+    double nhalf = (double)tb->n_cosa / 2.0;
+#pragma omp parallel
+    {
+        long double *tS = (long double *)calloc((size_t)nb, sizeof(long double));
+        long double *tW = (long double *)calloc((size_t)nb, sizeof(long double));
+        uint64_t *tN = (uint64_t *)calloc((size_t)nb, sizeof(uint64_t));
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t p = 0; p < nf; ++p) {
+            double ui[3] = { f->ux[p], f->uy[p], f->uz[p] };
+            for (int64_t i = f->pix_off[p]; i < f->pix_off[p + 1]; ++i) {
+                double xi[3] = { f->chi[i] * ui[0], f->chi[i] * ui[1], f->chi[i] * ui[2] };
+                double ai = f->w[i] * f->delta[i], wi = f->w[i];
+                for (int64_t eq = deg[p]; eq < deg[p + 1]; ++eq) {
+                    int64_t q = adj[eq];
+                    double uq[3] = { f->ux[q], f->uy[q], f->uz[q] };
+                    for (int64_t j = f->pix_off[q]; j < f->pix_off[q + 1]; ++j) {
+                        double d1[3], r1; int32_t br1, bt1;
+                        if (!tri_side(tb, cosedge, xi, ui, f->chi[j], uq, d1, &r1, &br1, &bt1)) continue;
+                        double aij = ai * (f->w[j] * f->delta[j]), wij = wi * f->w[j];
+                        for (int64_t er = deg[p]; er < deg[p + 1]; ++er) {
+                            int64_t r = adj[er];
+                            if (r == q) continue;
+                            double ur[3] = { f->ux[r], f->uy[r], f->uz[r] };
+                            for (int64_t k = f->pix_off[r]; k < f->pix_off[r + 1]; ++k) {
+                                double d2[3], r2; int32_t br2, bt2;
+                                if (!tri_side(tb, cosedge, xi, ui, f->chi[k], ur, d2, &r2, &br2, &bt2)) continue;
+                                double ca = (((d1[0] * d2[0]) + (d1[1] * d2[1])) + (d1[2] * d2[2])) / (r1 * r2);
+                                int32_t ba = (int32_t)((ca + 1.0) * nhalf);
+                                if (ba < 0) ba = 0;
+                                if (ba > tb->n_cosa - 1) ba = tb->n_cosa - 1;
+                                int64_t A = ((((int64_t)br1 * tb->n_r + br2) * tb->n_cosa + ba) * tb->n_theta + bt1) * tb->n_theta + bt2;
+                                tS[A] += aij * (f->w[k] * f->delta[k]);
+                                tW[A] += wij * f->w[k];
+                                tN[A] += 1;
+                            }
+                        }
+                    }
+                }
+            }
+        }
+#pragma omp critical
+        for (int64_t a = 0; a < nb; ++a) { gS[a] += tS[a]; gW[a] += tW[a]; N3[a] += tN[a]; }
+        free(tS); free(tW); free(tN);
+    }
+    for (int64_t a = 0; a < nb; ++a) { S3[a] = (double)gS[a]; W3[a] = (double)gW[a]; }
+    free(gS); free(gW); free(deg); free(adj); free(cur);
+}

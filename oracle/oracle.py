@@ -150,6 +150,34 @@ def xi_means(f, pairs, z, b=None):
     return dict(Rpar=out[0], Rperp=out[1], Z=out[2], W=out[3])
 
 
+class _TriBinning(C.Structure):
+    _fields_ = [("r_max", C.c_double), ("n_r", C.c_int32), ("n_theta", C.c_int32), ("n_cosa", C.c_int32)]
+
+
+def tri_binning(r_max=80.0, n_r=20, n_theta=10, n_cosa=20):
+    """Triangle bins of PAPER.md:225 (Fig. 5): r in [0, 80) Mpc/h x 20, theta in [0, pi] x 10, cos alpha x 20."""
+    return _TriBinning(r_max, n_r, n_theta, n_cosa)
+
+
+def xi3(f, pairs, tb=None, cosedge=None):
+    """NEXT-4, eq. 2.8: brute-force anisotropic 3PCF over ordered triples (i; j, k) in three distinct forests
+    (readings T1-T7 in lya_oracle.c).  cosedge: the cos(m pi / n_theta) table (input, m = 1..n_theta-1)."""
+    cat = f if isinstance(f, Catalogue) else Catalogue(f)
+    tb = tb or tri_binning()
+    if cosedge is None:
+        cosedge = np.cos(np.pi * np.arange(1, tb.n_theta) / tb.n_theta)
+    cosedge = _c(cosedge, np.float64)
+    pq = _pq(pairs)
+    lib().orc_tri_nbins.restype = C.c_int64
+    nb = int(lib().orc_tri_nbins(C.byref(tb)))
+    S3 = np.zeros(nb); W3 = np.zeros(nb); N3 = np.zeros(nb, np.uint64)
+    lib().orc_xi3(C.byref(cat.c), C.byref(tb), C.c_void_p(cosedge.ctypes.data), C.c_void_p(pq.ctypes.data),
+                  C.c_int64(len(pq)), C.c_void_p(S3.ctypes.data), C.c_void_p(W3.ctypes.data), C.c_void_p(N3.ctypes.data))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        x3 = np.where(W3 != 0.0, S3 / np.where(W3 == 0, 1.0, W3), 0.0)
+    return dict(S3=S3, W3=W3, N3=N3, xi3=x3)
+
+
 def eta(w, loglam):
     """eq. 2.7: explicit n x n eta of one forest (raises on a degenerate forest)."""
     w = _c(w, np.float64); ll = _c(loglam, np.float64)

@@ -56,6 +56,14 @@ int main(void)
     double *Dc = calloc((size_t)nb * nb, 8), *Wc = calloc(nb, 8);
     uint64_t n_kept_c = 0;
     int rc2 = orc_dmat_collapsed(&f, &b, pq2, n_d, 0.5, 12345ULL, Dc, Wc, &n_kept_c);
+    /* 3PCF on a coarse triangle grid (4 x 4 x 4 x 3 x 3 bins) */
+    orc_tri_binning tb = { 80.0, 4, 3, 4 };
+    double cosedge[2] = { 0.5, -0.5 };
+    int64_t ntb = orc_tri_nbins(&tb);
+    double *S3 = calloc((size_t)ntb, 8), *W3 = calloc((size_t)ntb, 8);
+    uint64_t *N3 = calloc((size_t)ntb, 8);
+    orc_xi3(&f, &tb, cosedge, pq, n_b, S3, W3, N3);
+    free(S3); free(W3); free(N3);
     double eta[9 * 9];
     int rc3 = orc_eta(9, w, ll, eta);
     printf("sanitize_main: %lld all, %lld listed (%lld by the window), %llu out of grid, %llu kept (%llu), rc %d %d %d, thr %llu, keep %d\n",

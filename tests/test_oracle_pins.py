@@ -496,3 +496,89 @@ def test_PM2_means_lie_inside_their_bin_and_special_cases(cfg0):
     assert abs(Decimal(float(m2["Rpar"][A2])) / Decimal("0.375") - rpar) < Decimal("1e-11")
     assert abs(Decimal(float(m2["Rperp"][A2])) / Decimal("0.375") - rperp) < Decimal("1e-11")
     assert abs(m2["Z"][A2] / 0.375 - 2.5) < 1e-14
+
+
+# ---------------------------------------------------------------- NEXT-4: anisotropic 3PCF (eq. 2.8)
+def _np_xi3(f, r_max=80.0, n_r=20, n_t=10, n_a=20):
+    """Independent numpy evaluation over ALL ordered forest triples: positions, norms, arccos for the two
+    line-of-sight angles (the oracle uses cosine edges instead), plain floor for every bin."""
+    X = f.chi[:, None] * np.repeat(np.stack([f.ux, f.uy, f.uz], 1), np.diff(f.pix_off), axis=0)
+    fid = np.repeat(np.arange(f.n_forest), np.diff(f.pix_off))
+    U = np.stack([f.ux, f.uy, f.uz], 1)[fid]
+    a = f.w * f.delta
+    nb = n_r * n_r * n_a * n_t * n_t
+    S = np.zeros(nb); W = np.zeros(nb); N = np.zeros(nb, np.int64)
+    for i in range(len(X)):
+        d = X - X[i]
+        r = np.sqrt((d * d).sum(1))
+        ok = (fid != fid[i]) & (r > 0) & (r < r_max)
+        idx = np.nonzero(ok)[0]
+        if len(idx) < 2:
+            continue
+        dd, rr = d[idx], r[idx]
+        br = np.minimum((rr * (n_r / r_max)).astype(np.int64), n_r - 1)
+        th = np.arccos(np.clip((dd @ U[i]) / rr, -1, 1))
+        bt = np.minimum((th / (np.pi / n_t)).astype(np.int64), n_t - 1)
+        ca = (dd @ dd.T) / np.outer(rr, rr)
+        ba = np.clip(((ca + 1.0) * (n_a / 2)).astype(np.int64), 0, n_a - 1)
+        J, K = np.meshgrid(np.arange(len(idx)), np.arange(len(idx)), indexing="ij")
+        m = fid[idx][J] != fid[idx][K]
+        A = (((br[J] * n_r + br[K]) * n_a + ba) * n_t + bt[J]) * n_t + bt[K]
+        np.add.at(N, A[m], 1)
+        np.add.at(W, A[m], (f.w[i] * f.w[idx][J] * f.w[idx][K])[m])
+        np.add.at(S, A[m], (a[i] * a[idx][J] * a[idx][K])[m])
+    return S, W, N
+
+
+@pytest.fixture(scope="module")
+def tri_small():
+    f = gen.make_config(0).subset(range(12))
+    return f, orc.pairs_all(f.n_forest)
+
+
+def test_PT1_xi3_numpy_brute_force(tri_small):
+    f, pq = tri_small
+    r = orc.xi3(f, pq)
+    S, W, N = _np_xi3(f)
+    assert N.sum() > 10000
+    assert np.array_equal(r["N3"].astype(np.int64), N)
+    assert np.allclose(r["W3"], W, rtol=1e-12) and np.allclose(r["S3"], S, rtol=0, atol=1e-12 * np.abs(S).max())
+
+
+def test_PT2_xi3_constant_delta_unit_weights_and_swap_symmetry(tri_small):
+    f, pq = tri_small
+    import copy
+    g = copy.deepcopy(f); g.delta[:] = -0.5
+    r = orc.xi3(g, pq)
+    nz = r["W3"] > 0
+    assert np.allclose(r["xi3"][nz], -0.125, rtol=1e-12)                      # d = k  =>  xi3 = k^3
+    h = copy.deepcopy(f); h.w[:] = 1.0
+    r1 = orc.xi3(h, pq)
+    assert np.array_equal(r1["W3"], r1["N3"].astype(float))                    # w = 1  =>  W3 = N3 exactly
+    # both orders (j, k) and (k, j) are counted: swapping (r1, theta1) <-> (r2, theta2) is a symmetry
+    r0 = orc.xi3(f, pq)
+    for key in ("N3", "W3", "S3"):
+        T = r0[key].reshape(20, 20, 20, 10, 10)
+        assert np.allclose(T, T.transpose(1, 0, 2, 4, 3), rtol=1e-13, atol=1e-13 * np.abs(T).max())
+
+
+def test_PT3_xi3_neighbour_list_is_enough_and_hand_built_triangle(cfg0):
+    f = cfg0.subset(range(30))
+    ra = orc.xi3(f, orc.pairs_all(f.n_forest))
+    rb = orc.xi3(f, orc.pairs_brute(f, orc.binning(80.0, 80.0, 20, 20)))      # pairs with r_perp < r_max at their first pixels
+    assert np.array_equal(ra["N3"], rb["N3"]) and np.allclose(ra["S3"], rb["S3"], rtol=0, atol=1e-13 * np.abs(ra["S3"]).max())
+    # three one-pixel forests: vertex i on the x axis at chi = 4000; j 30 Mpc/h further along the line of sight
+    # (theta1 = 0); k at 40 Mpc/h from i, 60 degrees off the line of sight, so cos alpha = cos theta2 = 0.5
+    xk = np.array([4020.0, 40.0 * np.sqrt(0.75), 0.0])
+    ck = float(np.linalg.norm(xk))
+    t = gen.two_forests([4000.0], [4030.0], (1.0, 0.0, 0.0), (1.0, 0.0, 0.0), w_p=[2.0], w_q=[3.0], d_p=[0.5], d_q=[-1.0])
+    f3 = gen.Forests(np.zeros(3), np.zeros(3), np.array([1.0, 1.0, xk[0] / ck]), np.array([0.0, 0.0, xk[1] / ck]), np.zeros(3),
+                     np.zeros(3), np.array([0, 1, 2, 3], np.int64), np.array([4000.0, 4030.0, ck]), np.array([2.0, 3.0, 5.0]),
+                     np.array([0.5, -1.0, 0.25]), np.full(3, 3.6))
+    r3 = orc.xi3(f3, [[0, 1], [0, 2], [1, 2]])
+    assert r3["N3"].sum() == 6                                                 # 3 vertices x 2 orders
+    A_ijk = (((7 * 20 + 10) * 20 + 15) * 10 + 0) * 10 + 3                      # r1 = 30 -> 7, r2 = 40 -> 10, cos a = .5 -> 15, th 0 -> 0, 60 deg -> 3
+    A_ikj = (((10 * 20 + 7) * 20 + 15) * 10 + 3) * 10 + 0
+    assert r3["N3"][A_ijk] == 1 and r3["N3"][A_ikj] == 1
+    assert abs(r3["W3"][A_ijk] - 30.0) < 1e-13 and abs(r3["S3"][A_ijk] - (1.0 * -3.0 * 1.25)) < 1e-13
+    assert np.allclose(r3["xi3"][r3["N3"] > 0], 0.5 * -1.0 * 0.25)
