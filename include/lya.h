@@ -211,6 +211,28 @@ lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                     const lya_pairs *pairs, double reject_fraction, uint64_t seed,
                     double *D, double *Dn, double *Wd, lya_stats *stats);
 
+/* ---- NEXT-4: brute-force anisotropic three-point correlation function, eq. 2.8 ------ */
+/* xi3_A = sum_A (d_i w_i)(d_j w_j)(d_k w_k) / sum_A w_i w_j w_k over pixels of three DISTINCT forests, binned in the
+ * five triangle variables of PAPER.md:108 / Fig. 2 / Fig. 5: the sides r1, r2 from a main vertex, cos(alpha) of the
+ * inner angle, and the angles theta1, theta2 of the sides to the line of sight.  The paper leaves the conventions
+ * open; the readings (T1-T7), each step one rounded binary64 operation:
+ *   every ORDERED triple (i; j, k) counts (a triangle enters 6 times: 3 main vertices x 2 orders of the sides);
+ *   X = chi u;  d1 = X_j - X_i, d2 = X_k - X_i;  r = sqrt(dx dx + dy dy + dz dz);  a side takes part iff 0 < r < r_max;
+ *   line of sight = unit vector of the main vertex's forest;  cos theta = (d . u_i) / r;  cos alpha = (d1 . d2) / (r1 r2);
+ *   b_r = (int)(r n_r / r_max) (clamped);  b_theta = number of m in 1..n_theta-1 with cos theta <= cos_theta_edges[m-1],
+ *   the table cos(m pi / n_theta) being an INPUT (device double [n_theta-1]) so that no arccos enters;
+ *   b_alpha = (int)((cos alpha + 1) n_cosa / 2) clamped to [0, n_cosa-1];
+ *   A = (((b_r1 n_r + b_r2) n_cosa + b_alpha) n_theta + b_theta1) n_theta + b_theta2   (lya_tri_nbins entries).
+ * pairs: any list holding every pair of forests with two pixels closer than r_max -- lya_neighbours with
+ * rperp_max = r_max is one (r_perp never exceeds the 3-D separation).  S3, W3, xi3: device double [n_bins]; N3:
+ * device uint64 [n_bins] (ordered triples per bin); any may be NULL.  stats: n_binned = triples counted.
+ * Limits (LYA_ERR_CAPACITY): at most 255 bins per variable and 2^24 bins in all; at most 2048 pixels of other
+ * forests inside the sphere of radius r_max around one pixel.  Synchronises the ctx stream. */
+typedef struct { double r_max; int32_t n_r, n_theta, n_cosa; } lya_tri_binning;   /* 80, 20, 10, 20 */
+int64_t    lya_tri_nbins(const lya_tri_binning *tb);
+lya_status lya_xi3pcf(lya_ctx *ctx, const lya_forests *f, const lya_tri_binning *tb, const double *cos_theta_edges,
+                      const lya_pairs *pairs, double *S3, double *W3, uint64_t *N3, double *xi3, lya_stats *stats);
+
 /* ---- plans: prepare once, run stages 2 and 3+4 on the same catalogue and list -------------------- */
 /* lya_xi2pcf and lya_dmat each validate the catalogue, build a padded 16-byte-aligned copy of it (with the
  * per-pixel products of eq. 2.4 / eq. 2.7) and bucket-sort the forest-pair list by r_perp column before

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "liblya.so")
 EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_launch_count", "lya_set_option", "lya_neighbours",
            "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
            "lya_xi2pcf", "lya_xi2pcf_sub", "lya_xi2pcf_means", "lya_dmat", "lya_run_host", "lya_xi_normalise", "lya_dmat_normalise",
-           "lya_plan_create", "lya_plan_free", "lya_xi2pcf_plan", "lya_dmat_plan"]
+           "lya_plan_create", "lya_plan_free", "lya_xi2pcf_plan", "lya_dmat_plan", "lya_tri_nbins", "lya_xi3pcf"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
           4: "LYA_ERR_CAPACITY", 5: "LYA_ERR_OOM", 6: "LYA_ERR_CUDA", 7: "LYA_ERR_UNIMPLEMENTED"}
@@ -40,6 +40,10 @@ class CForests(C.Structure):
 
 class CBinning(C.Structure):
     _fields_ = [("rpar_max", C.c_double), ("rperp_max", C.c_double), ("n_par", C.c_int32), ("n_perp", C.c_int32)]
+
+
+class CTriBinning(C.Structure):
+    _fields_ = [("r_max", C.c_double), ("n_r", C.c_int32), ("n_theta", C.c_int32), ("n_cosa", C.c_int32)]
 
 
 class CStats(C.Structure):
@@ -87,6 +91,10 @@ def load():
         lib.lya_run_host.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_int, C.c_int,
                                      C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.POINTER(C.c_int64), C.POINTER(CStats), C.POINTER(CStats)]
+        lib.lya_tri_nbins.restype = C.c_int64
+        lib.lya_tri_nbins.argtypes = [C.POINTER(CTriBinning)]
+        lib.lya_xi3pcf.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CTriBinning), C.c_void_p, C.c_void_p,
+                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
         lib.lya_plan_create.argtypes = [C.c_void_p, C.POINTER(CForests), C.POINTER(CBinning), C.c_void_p, C.c_int, C.c_int,
                                         C.POINTER(C.c_void_p)]
         lib.lya_plan_free.argtypes = [C.c_void_p, C.c_void_p]
@@ -104,6 +112,10 @@ def load():
 def launch_count() -> int:
     """Kernels launched by liblya.so in this process so far."""
     return int(load().lya_launch_count())
+
+
+def tri_binning(r_max=80.0, n_r=20, n_theta=10, n_cosa=20) -> CTriBinning:
+    return CTriBinning(r_max, n_r, n_theta, n_cosa)
 
 
 def binning(rpar_max=200.0, rperp_max=200.0, n_par=50, n_perp=50) -> CBinning:
@@ -312,6 +324,22 @@ class Context:
         cf = forests.c()
         self._check(load().lya_xi2pcf_means(self.h, C.byref(cf), C.byref(b), pairs.handle, _ptr(z), *[_ptr(o) for o in out]))
         return dict(Rpar=out[0], Rperp=out[1], Z=out[2], W=out[3])
+
+    def lya_xi3pcf(self, forests: DeviceForests, tb: CTriBinning, cos_theta_edges, pairs: Pairs):
+        """cos_theta_edges: cos(m pi / n_theta), m = 1..n_theta-1 (numpy or torch): an input, like chi."""
+        torch = self.torch
+        if not torch.is_tensor(cos_theta_edges):
+            cos_theta_edges = torch.from_numpy(np.ascontiguousarray(cos_theta_edges, dtype=np.float64))
+        ce = cos_theta_edges.to(self.device, dtype=torch.float64).contiguous()
+        nb = int(load().lya_tri_nbins(C.byref(tb)))
+        S3 = torch.empty(nb, dtype=torch.float64, device=self.device)
+        W3 = torch.empty_like(S3); x3 = torch.empty_like(S3)
+        N3 = torch.empty(nb, dtype=torch.int64, device=self.device)      # uint64 payload
+        stats = CStats()
+        cf = forests.c()
+        self._check(load().lya_xi3pcf(self.h, C.byref(cf), C.byref(tb), _ptr(ce) if ce.numel() else None, pairs.handle,
+                                      _ptr(S3), _ptr(W3), _ptr(N3), _ptr(x3), C.byref(stats)))
+        return dict(S3=S3, W3=W3, N3=N3, xi3=x3, stats=stats.as_dict())
 
     # ---- lya_dmat ----
     def lya_dmat(self, forests: DeviceForests, b: CBinning, pairs: Pairs, reject_fraction: float, seed: int,

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblya.so")
 LIB_PEAKS = os.path.join(HERE, "liblya_peaks.so")
-SOURCES = ["lya_api.cu", "neighbours.cu", "prep.cu", "xi2pcf.cu", "dmat.cu"]
+SOURCES = ["lya_api.cu", "neighbours.cu", "prep.cu", "xi2pcf.cu", "dmat.cu", "xi3pcf.cu"]
 HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cuh", ".h")))
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]

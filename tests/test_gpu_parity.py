@@ -423,6 +423,29 @@ def test_weighted_mean_coordinates_next1(ctx, B, orc):
         assert np.allclose(g["W"].cpu().numpy(), x["W"].cpu().numpy(), rtol=1e-12)      # eq. 2.4's denominator
 
 
+def test_anisotropic_3pcf_next4(ctx, B, orc):
+    """lya_xi3pcf (eq. 2.8) against the brute-force oracle: ordered-triple counts per triangle bin bit-exact,
+    S3 and W3 to 1e-9, on configs[0] with the paper's 20 x 20 x 20 x 10 x 10 bins up to 80 Mpc/h (Fig. 5) and on
+    a denser configs[1]-shaped patch with the 40 Mpc/h of Tables 2-3 and a coarser grid."""
+    for f, grid in ((gen.make_config(0), (80.0, 20, 10, 20)), (gen.make_config(1, n_forest=250, density_scale=6.0), (40.0, 8, 5, 6))):
+        d = B.DeviceForests(f)
+        tb, otb = B.tri_binning(*grid), orc.tri_binning(*grid)
+        ce = np.cos(np.pi * np.arange(1, grid[2]) / grid[2])
+        b2 = B.binning(grid[0], grid[0], 20, 20)
+        pairs = ctx.lya_neighbours(d, b2)                                  # r_perp < r_max: a superset of what is needed
+        g = ctx.lya_xi3pcf(d, tb, ce, pairs)
+        o = orc.xi3(f, pairs.export().cpu().numpy(), otb, ce)
+        N3 = g["N3"].cpu().numpy().view(np.uint64)
+        assert int(o["N3"].sum()) > 100000
+        assert np.array_equal(N3, o["N3"]), f"{(N3 != o['N3']).sum()} triangle bins differ"
+        assert g["stats"]["n_binned"] == int(o["N3"].sum())
+        assert np.all(np.abs(g["W3"].cpu().numpy() - o["W3"]) <= 1e-9 * o["W3"])
+        S3 = g["S3"].cpu().numpy()
+        assert np.all(np.abs(S3 - o["S3"]) <= 1e-9 * np.maximum(np.abs(o["S3"]), 1e-6 * np.abs(o["S3"]).max()))
+        nz = o["W3"] > 0
+        assert np.all(g["xi3"].cpu().numpy()[~nz] == 0.0)
+
+
 # ------------------------------------------------------------------ invariances and edge cases
 def test_P7_pair_order_and_swap(ctx, B, orc, cfg0):
     d = B.DeviceForests(cfg0)
