@@ -301,6 +301,20 @@ def main():
     barrier()
     launches = B.launch_count() - launches0          # kernels this rank's library launched inside the timed region
     clocks = sampler.stop() if rank == 0 else None
+    # one more, untimed, step with CUDA events around every stage (where the step's time goes)
+    stage_ms = None
+    if not strong:
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+        evs[0].record()
+        pairs = ctx.lya_neighbours(d, b); evs[1].record()
+        plan = ctx.lya_plan_create(d, b, pairs, want_xi=True, want_dmat=do_d); pairs.free(); evs[2].record()
+        ctx.lya_xi2pcf_plan(plan); evs[3].record()
+        if do_d:
+            ctx.lya_dmat_plan(plan, frac, mseed, want_Dn=False)
+        plan.free(); evs[4].record()
+        torch.cuda.synchronize()
+        stage_ms = {"lya_neighbours": evs[0].elapsed_time(evs[1]), "lya_plan_create": evs[1].elapsed_time(evs[2]),
+                    "lya_xi2pcf_plan": evs[2].elapsed_time(evs[3]), "lya_dmat_plan": evs[3].elapsed_time(evs[4])}
     ms = ev0.elapsed_time(ev1)
     ms, pairs_all = shard.aggregate(ms, float(pairs_total), device=f"cuda:{local}")
     value = pairs_all / (ms * 1e-3)
@@ -398,7 +412,7 @@ def main():
                                                          "larger than L2" if f.n_pix * 32 + sx["n_forest_pairs"] * 8 > 126e6
                                                          else "NOT larger than L2: use the default workload for a valid number"),
                        "parallelism": par},
-            "roofline": roof, "clocks": clocks, "gpu_launches": int(launches), "e2e": e2e, **extra,
+            "roofline": roof, "clocks": clocks, "gpu_launches": int(launches), "stage_ms": stage_ms, "e2e": e2e, **extra,
         }
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(wl, args.cpu_forests, args.cpu_dmat_div)

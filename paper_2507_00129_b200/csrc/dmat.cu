@@ -377,7 +377,7 @@ extern "C" lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, 
     if (!(reject_fraction >= 0.0 && reject_fraction <= 1.0))
         return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_pairs_subsample: reject_fraction must be in [0,1]");
     *out = NULL; *n_kept = 0;
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     lya_pairs *pl = (lya_pairs *)calloc(1, sizeof(lya_pairs));
     if (!pl) return lya_fail(ctx, LYA_ERR_OOM, "host allocation failed");
     const int64_t n = pairs->n;
@@ -389,11 +389,11 @@ extern "C" lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, 
     cudaStream_t s = ctx->stream;
     unsigned *flag = NULL;
     unsigned long long *pos = NULL, *tmp = NULL;
-    cudaError_t e = cudaMalloc(&flag, sizeof(unsigned) * (size_t)n);
-    if (e == cudaSuccess) e = cudaMalloc(&pos, sizeof(unsigned long long) * (size_t)(n + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&tmp, sizeof(unsigned long long) * (size_t)(n / 2048 + 4));
-    auto drop = [&]() { cudaFree(flag); cudaFree(pos); cudaFree(tmp); };
-    if (e != cudaSuccess) { drop(); free(pl); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_pairs_subsample)"); }
+    cudaError_t e = lya_malloc(&flag, sizeof(unsigned) * (size_t)n);
+    if (e == cudaSuccess) e = lya_malloc(&pos, sizeof(unsigned long long) * (size_t)(n + 1));
+    if (e == cudaSuccess) e = lya_malloc(&tmp, sizeof(unsigned long long) * (size_t)(n / 2048 + 4));
+    auto drop = [&]() { lya_free(flag); lya_free(pos); lya_free(tmp); };
+    if (e != cudaSuccess) { drop(); free(pl); return lya_cuda_fail(ctx, e, "lya_malloc(lya_pairs_subsample)"); }
     const unsigned blocks = (unsigned)((n + 255) / 256);
     { k_fp_flag<<<blocks, 256, 0, s>>>(pairs->pq, n, seed, thr, flag); lya_note_launch(); }
     e = lya_exclusive_scan(flag, pos, n, tmp, s);
@@ -403,13 +403,13 @@ extern "C" lya_status lya_pairs_subsample(lya_ctx *ctx, const lya_pairs *pairs, 
     if (e != cudaSuccess) { drop(); free(pl); return lya_cuda_fail(ctx, e, "lya_pairs_subsample"); }
     pl->n = (int64_t)total;
     if (total > 0) {
-        e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)total);
+        e = lya_malloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)total);
         if (e == cudaSuccess) {
             { k_fp_compact<<<blocks, 256, 0, s>>>(pairs->pq, n, flag, pos, pl->pq); lya_note_launch(); }
             e = cudaGetLastError();
             if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         }
-        if (e != cudaSuccess) { if (pl->pq) cudaFree(pl->pq); drop(); free(pl); return lya_cuda_fail(ctx, e, "lya_pairs_subsample"); }
+        if (e != cudaSuccess) { if (pl->pq) lya_free(pl->pq); drop(); free(pl); return lya_cuda_fail(ctx, e, "lya_pairs_subsample"); }
     }
     drop();
     *out = pl; *n_kept = pl->n;
@@ -430,7 +430,7 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
     if (b->n_par > H_SLOTS) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_dmat: n_par above %d", H_SLOTS);
     if (pl->listed_degenerate)
         return lya_fail(ctx, LYA_ERR_DEGENERATE_FOREST, "a listed forest has sum w == 0 or sum w (L-Lbar)^2 == 0");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
 
     const int nb = b->n_par * b->n_perp;
     cudaStream_t s = ctx->stream;
@@ -439,12 +439,12 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
     const LyaBuckets &bk = pl->bk;
     double *scal = NULL, *Dn = NULL, *Wd = NULL;          // internal accumulators (transposed bin order)
     const int64_t nf = f->n_forest;
-    auto cleanup = [&]() { cudaFree(scal); cudaFree(Dn); cudaFree(Wd); };
+    auto cleanup = [&]() { lya_free(scal); lya_free(Dn); lya_free(Wd); };
     cudaEventRecord(ctx->ev[3], s);
-    cudaError_t e = cudaMalloc(&scal, sizeof(double) * 3 * (size_t)(nf ? nf : 1));
-    if (e == cudaSuccess) e = cudaMalloc(&Dn, sizeof(double) * (size_t)nb * nb);
-    if (e == cudaSuccess) e = cudaMalloc(&Wd, sizeof(double) * (size_t)nb);
-    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_dmat)"); }
+    cudaError_t e = lya_malloc(&scal, sizeof(double) * 3 * (size_t)(nf ? nf : 1));
+    if (e == cudaSuccess) e = lya_malloc(&Dn, sizeof(double) * (size_t)nb * nb);
+    if (e == cudaSuccess) e = lya_malloc(&Wd, sizeof(double) * (size_t)nb);
+    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "lya_malloc(lya_dmat)"); }
     cudaMemsetAsync(Dn, 0, sizeof(double) * (size_t)nb * nb, s);
     cudaMemsetAsync(Wd, 0, sizeof(double) * (size_t)nb, s);
     cudaMemsetAsync(ctx->d_counters, 0, 16 * sizeof(unsigned long long), s);
@@ -575,7 +575,7 @@ extern "C" lya_status lya_dmat_normalise(lya_ctx *ctx, const lya_binning *b, con
     lya_status st = lya_check_binning(ctx, b);
     if (st) return st;
     if (!Dn || !Wd || !D) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_dmat_normalise: NULL argument");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     const int nb = b->n_par * b->n_perp;
     { k_dmat_divide<<<(unsigned)(((int64_t)nb * nb + 255) / 256), 256, 0, ctx->stream>>>(Dn, Wd, nb, D); lya_note_launch(); }
     LYA_CUDA(cudaGetLastError());

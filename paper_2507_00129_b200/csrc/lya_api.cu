@@ -6,6 +6,16 @@
 #include "lya_internal.cuh"
 
 unsigned long long g_lya_launches = 0;
+thread_local cudaStream_t tl_lya_stream = 0;
+thread_local bool tl_lya_pool = false;
+
+cudaError_t lya_enter(lya_ctx *ctx)
+{
+    cudaError_t e = cudaSetDevice(ctx->device);
+    tl_lya_stream = ctx->stream;
+    tl_lya_pool = ctx->use_pool != 0;
+    return e;
+}
 extern "C" uint64_t lya_launch_count(void) { return g_lya_launches; }
 
 extern "C" const char *lya_version(void) { return "lya-b200 0.1 (sm_100a)"; }
@@ -39,6 +49,18 @@ extern "C" lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     ctx->device = device;
     ctx->stream = (cudaStream_t)cuda_stream;
     if (cudaSetDevice(device) != cudaSuccess) { free(ctx); return LYA_ERR_CUDA; }
+    {   // stream-ordered scratch allocation with a pool that keeps freed blocks (see lya_internal.cuh)
+        int has_pools = 0;
+        cudaMemPool_t pool;
+        if (cudaDeviceGetAttribute(&has_pools, cudaDevAttrMemoryPoolsSupported, device) == cudaSuccess && has_pools &&
+            cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            ctx->use_pool = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep) == cudaSuccess;
+        }
+        cudaGetLastError();
+        tl_lya_stream = ctx->stream;
+        tl_lya_pool = ctx->use_pool != 0;
+    }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { free(ctx); return LYA_ERR_CUDA; }
     ctx->sm_count = prop.multiProcessorCount;
@@ -57,9 +79,14 @@ extern "C" lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
 extern "C" void lya_destroy(lya_ctx *ctx)
 {
     if (!ctx) return;
-    cudaSetDevice(ctx->device);
+    lya_enter(ctx);
     for (int i = 0; i < 4; ++i) cudaEventDestroy(ctx->ev[i]);
     cudaFree(ctx->d_counters);
+    if (ctx->use_pool) {                              // hand the cached scratch back to the driver
+        cudaMemPool_t pool;
+        cudaStreamSynchronize(ctx->stream);
+        if (cudaDeviceGetDefaultMemPool(&pool, ctx->device) == cudaSuccess) cudaMemPoolTrimTo(pool, 0);
+    }
     free(ctx);
 }
 
@@ -203,13 +230,13 @@ extern "C" lya_status lya_pairs_import(lya_ctx *ctx, const int32_t *pq, int64_t 
     if (!ctx) return LYA_ERR_INVALID_ARG;
     if (!out || n_pairs < 0 || (n_pairs > 0 && !pq)) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_pairs_import: bad arguments");
     *out = NULL;
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     lya_pairs *pl = (lya_pairs *)calloc(1, sizeof(lya_pairs));
     if (!pl) return lya_fail(ctx, LYA_ERR_OOM, "host allocation failed");
     pl->n = n_pairs;
     if (n_pairs > 0) {
-        cudaError_t e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)n_pairs);
-        if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "cudaMalloc(pair list)"); }
+        cudaError_t e = lya_malloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)n_pairs);
+        if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "lya_malloc(pair list)"); }
         unsigned *d_err = (unsigned *)(ctx->d_counters + 8);
         cudaMemsetAsync(d_err, 0, sizeof(unsigned long long), ctx->stream);
         int threads = 256;
@@ -217,8 +244,8 @@ extern "C" lya_status lya_pairs_import(lya_ctx *ctx, const int32_t *pq, int64_t 
         unsigned long long h = 0;
         e = cudaMemcpyAsync(&h, d_err, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-        if (e != cudaSuccess) { cudaFree(pl->pq); free(pl); return lya_cuda_fail(ctx, e, "lya_pairs_import"); }
-        if ((unsigned)h != 0) { cudaFree(pl->pq); free(pl); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list has p == q or a negative index"); }
+        if (e != cudaSuccess) { lya_free(pl->pq); free(pl); return lya_cuda_fail(ctx, e, "lya_pairs_import"); }
+        if ((unsigned)h != 0) { lya_free(pl->pq); free(pl); return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list has p == q or a negative index"); }
     }
     *out = pl;
     return LYA_OK;
@@ -228,7 +255,7 @@ extern "C" lya_status lya_pairs_export(lya_ctx *ctx, const lya_pairs *pairs, int
 {
     if (!ctx) return LYA_ERR_INVALID_ARG;
     if (!pairs || (pairs->n > 0 && !pq)) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_pairs_export: bad arguments");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     if (pairs->n > 0)
         LYA_CUDA(cudaMemcpyAsync(pq, pairs->pq, sizeof(int32_t) * 2 * (size_t)pairs->n, cudaMemcpyDeviceToDevice, ctx->stream));
     return LYA_OK;
@@ -239,8 +266,8 @@ extern "C" int64_t lya_pairs_count(const lya_pairs *pairs) { return pairs ? pair
 extern "C" void lya_pairs_free(lya_ctx *ctx, lya_pairs *pairs)
 {
     if (!pairs) return;
-    if (ctx) cudaSetDevice(ctx->device);
-    if (pairs->pq) cudaFree(pairs->pq);
+    if (ctx) lya_enter(ctx);
+    if (pairs->pq) lya_free(pairs->pq);
     free(pairs);
 }
 
@@ -248,8 +275,8 @@ extern "C" void lya_pairs_free(lya_ctx *ctx, lya_pairs *pairs)
 namespace {
 struct DevBuf {
     void *p = nullptr;
-    ~DevBuf() { if (p) cudaFree(p); }
-    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 1); }
+    ~DevBuf() { if (p) lya_free(p); }
+    cudaError_t alloc(size_t bytes) { return lya_malloc(&p, bytes ? bytes : 1); }
 };
 }
 
@@ -264,7 +291,7 @@ extern "C" lya_status lya_run_host(lya_ctx *ctx, const lya_forests *fh, const ly
     st = lya_check_forests_host(ctx, fh, true, do_xi != 0, do_dmat != 0);
     if (st) return st;
     if (!(fh->ux && fh->uy && fh->uz)) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_run_host needs ux,uy,uz");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     const int64_t nf = fh->n_forest, np = fh->n_pix;
     const int64_t nb = (int64_t)b->n_par * b->n_perp;
     DevBuf ux, uy, uz, off, chi, w, delta, loglam, dS, dW, dN, dxi, dD, dWd;
@@ -303,7 +330,7 @@ extern "C" lya_status lya_run_host(lya_ctx *ctx, const lya_forests *fh, const ly
         if (e == cudaSuccess) e = dW.alloc(8 * nb);
         if (e == cudaSuccess) e = dN.alloc(8 * nb);
         if (e == cudaSuccess) e = dxi.alloc(8 * nb);
-        if (e != cudaSuccess) { lya_plan_free(ctx, plan); return lya_cuda_fail(ctx, e, "cudaMalloc(xi outputs)"); }
+        if (e != cudaSuccess) { lya_plan_free(ctx, plan); return lya_cuda_fail(ctx, e, "lya_malloc(xi outputs)"); }
         st = lya_xi2pcf_plan(ctx, plan, (double *)dS.p, (double *)dW.p, (uint64_t *)dN.p, (double *)dxi.p, stats_xi);
         if (st) { lya_plan_free(ctx, plan); return st; }
         if (S) cudaMemcpyAsync(S, dS.p, 8 * nb, cudaMemcpyDeviceToHost, s);
@@ -314,7 +341,7 @@ extern "C" lya_status lya_run_host(lya_ctx *ctx, const lya_forests *fh, const ly
     if (do_dmat) {
         cudaError_t e = dD.alloc(8 * nb * nb);
         if (e == cudaSuccess) e = dWd.alloc(8 * nb);
-        if (e != cudaSuccess) { lya_plan_free(ctx, plan); return lya_cuda_fail(ctx, e, "cudaMalloc(D outputs)"); }
+        if (e != cudaSuccess) { lya_plan_free(ctx, plan); return lya_cuda_fail(ctx, e, "lya_malloc(D outputs)"); }
         st = lya_dmat_plan(ctx, plan, reject_fraction, seed, (double *)dD.p, NULL, (double *)dWd.p, stats_dmat);
         if (st) { lya_plan_free(ctx, plan); return st; }
         if (D) cudaMemcpyAsync(D, dD.p, 8 * nb * nb, cudaMemcpyDeviceToHost, s);

@@ -23,6 +23,7 @@ struct lya_ctx {
     unsigned long long xi_merge_every; // LYA_OPT_XI_MERGE_EVERY: visited pairs between forced merges of a warp's sub-histogram
     int generic_diagonals;            // LYA_OPT_GENERIC_DIAGONALS: diagonals per lane of the generic xi kernel (1, 2, 4)
     cudaEvent_t ev[4];
+    int use_pool;                     // scratch from the stream-ordered allocator (memory pools supported)
 };
 
 struct lya_pairs {
@@ -38,6 +39,24 @@ enum { LYA_DEV_OK = 0, LYA_DEV_BAD_OFFSETS = 1, LYA_DEV_NONFINITE = 2, LYA_DEV_U
 // process-wide count of kernel launches made by the library (lya_launch_count): every launch site notes itself
 extern unsigned long long g_lya_launches;
 static inline void lya_note_launch() { ++g_lya_launches; }
+
+// Device scratch comes from CUDA's stream-ordered allocator on the ctx stream: the device's default memory pool
+// keeps freed blocks (release threshold raised in lya_create), so the multi-GB pair lists and catalogue copies of
+// one step are re-used by the next instead of being mapped and unmapped every call (0.3 s per step at configs[4]).
+// lya_enter(ctx) is called by every entry point: it selects the device and makes the ctx stream the thread's
+// allocation stream.
+extern thread_local cudaStream_t tl_lya_stream;
+extern thread_local bool tl_lya_pool;
+cudaError_t lya_enter(lya_ctx *ctx);
+template <class T> static inline cudaError_t lya_malloc(T **p, size_t bytes)
+{
+    return tl_lya_pool ? cudaMallocAsync((void **)p, bytes ? bytes : 1, tl_lya_stream) : cudaMalloc((void **)p, bytes ? bytes : 1);
+}
+static inline cudaError_t lya_free(void *p)
+{
+    if (!p) return cudaSuccess;
+    return tl_lya_pool ? cudaFreeAsync(p, tl_lya_stream) : cudaFree(p);
+}
 
 lya_status lya_fail(lya_ctx *ctx, lya_status st, const char *fmt, ...);
 lya_status lya_cuda_fail(lya_ctx *ctx, cudaError_t e, const char *what);

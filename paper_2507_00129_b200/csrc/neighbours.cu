@@ -261,10 +261,10 @@ __global__ void k_pairs(SortedForests sf, int64_t m, const unsigned long long *c
 struct Scratch {
     void *ptrs[24];
     int n = 0;
-    ~Scratch() { for (int i = 0; i < n; ++i) cudaFree(ptrs[i]); }
+    ~Scratch() { for (int i = 0; i < n; ++i) lya_free(ptrs[i]); }
     template <class T> cudaError_t alloc(T **p, size_t count)
     {
-        cudaError_t e = cudaMalloc((void **)p, sizeof(T) * (count ? count : 1));
+        cudaError_t e = lya_malloc(p, sizeof(T) * (count ? count : 1));
         if (e == cudaSuccess) ptrs[n++] = *p;
         return e;
     }
@@ -288,7 +288,7 @@ extern "C" lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const l
     if (st) return st;
     st = lya_check_forests_host(ctx, f, true, false, false);
     if (st) return st;
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     st = lya_validate_forests(ctx, f, false, false, NULL);
     if (st) return st;
 
@@ -304,7 +304,7 @@ extern "C" lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const l
     unsigned *counts;
     unsigned long long *offsets, *scan_tmp;
     SortedForests sf;
-#define NB_ALLOC(ptr, cnt) do { cudaError_t e_ = sc.alloc(&(ptr), (size_t)(cnt)); if (e_ != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e_, "cudaMalloc(neighbour scratch)"); } } while (0)
+#define NB_ALLOC(ptr, cnt) do { cudaError_t e_ = sc.alloc(&(ptr), (size_t)(cnt)); if (e_ != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e_, "lya_malloc(neighbour scratch)"); } } while (0)
     NB_ALLOC(ux, n); NB_ALLOC(uy, n); NB_ALLOC(uz, n); NB_ALLOC(chimin, n);
     NB_ALLOC(cell_of, n); NB_ALLOC(sorted_id, n);
     NB_ALLOC(sf.ux, n); NB_ALLOC(sf.uy, n); NB_ALLOC(sf.uz, n); NB_ALLOC(sf.chimin, n); NB_ALLOC(sf.id, n);
@@ -366,12 +366,12 @@ extern "C" lya_status lya_neighbours(lya_ctx *ctx, const lya_forests *f, const l
     if (total >= (1ULL << 40)) { free(pl); return lya_fail(ctx, LYA_ERR_CAPACITY, "more than 2^40 forest pairs"); }
     pl->n = (int64_t)total;
     if (total > 0) {
-        e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)total);
-        if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "cudaMalloc(pair list)"); }
+        e = lya_malloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)total);
+        if (e != cudaSuccess) { free(pl); return lya_cuda_fail(ctx, e, "lya_malloc(pair list)"); }
         { k_pairs<true><<<wblk, T, 0, s>>>(sf, m, cell_start, G, b->rperp_max, NULL, offsets, pl->pq); lya_note_launch(); }
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-        if (e != cudaSuccess) { cudaFree(pl->pq); free(pl); return lya_cuda_fail(ctx, e, "k_pairs<fill>"); }
+        if (e != cudaSuccess) { lya_free(pl->pq); free(pl); return lya_cuda_fail(ctx, e, "k_pairs<fill>"); }
     }
     *out = pl;
     *n_pairs = pl->n;

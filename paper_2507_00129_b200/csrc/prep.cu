@@ -179,7 +179,7 @@ __global__ void k_bucket_scatter(const int32_t *pq, const unsigned char *keys, i
 
 void lya_prep_free(LyaPrep *p)
 {
-    if (p && p->base) { cudaFree(p->base); p->base = NULL; }
+    if (p && p->base) { lya_free(p->base); p->base = NULL; }
 }
 
 lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool want_dmat, LyaPrep *out)
@@ -191,11 +191,11 @@ lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool
     cudaStream_t s = ctx->stream;
     unsigned *padlen = NULL;
     unsigned long long *off2 = NULL, *tmp = NULL;
-    LYA_CUDA(cudaMalloc(&padlen, sizeof(unsigned) * (size_t)n));
-    cudaError_t e = cudaMalloc(&off2, sizeof(unsigned long long) * (size_t)(n + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&tmp, sizeof(unsigned long long) * (size_t)(n / 2048 + 4));
-    if (e != cudaSuccess) { cudaFree(padlen); cudaFree(off2); return lya_cuda_fail(ctx, e, "cudaMalloc(prep scratch)"); }
-    auto drop = [&]() { cudaFree(padlen); cudaFree(off2); cudaFree(tmp); };
+    LYA_CUDA(lya_malloc(&padlen, sizeof(unsigned) * (size_t)n));
+    cudaError_t e = lya_malloc(&off2, sizeof(unsigned long long) * (size_t)(n + 1));
+    if (e == cudaSuccess) e = lya_malloc(&tmp, sizeof(unsigned long long) * (size_t)(n / 2048 + 4));
+    if (e != cudaSuccess) { lya_free(padlen); lya_free(off2); return lya_cuda_fail(ctx, e, "lya_malloc(prep scratch)"); }
+    auto drop = [&]() { lya_free(padlen); lya_free(off2); lya_free(tmp); };
     { k_pad_len<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(f->pix_off, n, padlen); lya_note_launch(); }
     e = lya_exclusive_scan(padlen, off2, n, tmp, s);
     unsigned long long total = 0;
@@ -206,8 +206,8 @@ lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool
     const int n_arr = 1 + (want_xi ? 2 : 0) + (want_dmat ? 4 : 0);
     const size_t head_bytes = sizeof(ForestHead) * (size_t)n;
     const size_t arr_bytes = ((size_t)total * 8 + 255) & ~(size_t)255;
-    e = cudaMalloc(&out->base, head_bytes + arr_bytes * n_arr + 256);
-    if (e != cudaSuccess) { drop(); out->base = NULL; return lya_cuda_fail(ctx, e, "cudaMalloc(prepared catalogue)"); }
+    e = lya_malloc(&out->base, head_bytes + arr_bytes * n_arr + 256);
+    if (e != cudaSuccess) { drop(); out->base = NULL; return lya_cuda_fail(ctx, e, "lya_malloc(prepared catalogue)"); }
     char *b = (char *)out->base;
     out->head = (ForestHead *)b; b += (head_bytes + 255) & ~(size_t)255;
     out->w = (double *)b; b += arr_bytes;
@@ -227,7 +227,7 @@ lya_status lya_prep_build(lya_ctx *ctx, const lya_forests *f, bool want_xi, bool
 
 void lya_buckets_free(LyaBuckets *b)
 {
-    if (b && b->pq) { cudaFree(b->pq); b->pq = NULL; }
+    if (b && b->pq) { lya_free(b->pq); b->pq = NULL; }
 }
 
 // counters[1] += visited, counters[3] = error flag (the caller zeroes ctx->d_counters first)
@@ -246,13 +246,13 @@ lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *
     unsigned char *keys = NULL;
     unsigned *counts = NULL;
     unsigned long long *offsets = NULL, *tmp = NULL;
-    cudaError_t e = cudaMalloc(&keys, (size_t)n);
-    if (e == cudaSuccess) e = cudaMalloc(&counts, sizeof(unsigned) * (size_t)n_cnt);
-    if (e == cudaSuccess) e = cudaMalloc(&offsets, sizeof(unsigned long long) * (size_t)(n_cnt + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&tmp, sizeof(unsigned long long) * (size_t)(n_cnt / 2048 + 4));
-    if (e == cudaSuccess) e = cudaMalloc(&out->pq, sizeof(int32_t) * 2 * (size_t)n);
-    auto drop = [&]() { cudaFree(keys); cudaFree(counts); cudaFree(offsets); cudaFree(tmp); };
-    if (e != cudaSuccess) { drop(); cudaFree(out->pq); out->pq = NULL; return lya_cuda_fail(ctx, e, "cudaMalloc(bucketing)"); }
+    cudaError_t e = lya_malloc(&keys, (size_t)n);
+    if (e == cudaSuccess) e = lya_malloc(&counts, sizeof(unsigned) * (size_t)n_cnt);
+    if (e == cudaSuccess) e = lya_malloc(&offsets, sizeof(unsigned long long) * (size_t)(n_cnt + 1));
+    if (e == cudaSuccess) e = lya_malloc(&tmp, sizeof(unsigned long long) * (size_t)(n_cnt / 2048 + 4));
+    if (e == cudaSuccess) e = lya_malloc(&out->pq, sizeof(int32_t) * 2 * (size_t)n);
+    auto drop = [&]() { lya_free(keys); lya_free(counts); lya_free(offsets); lya_free(tmp); };
+    if (e != cudaSuccess) { drop(); lya_free(out->pq); out->pq = NULL; return lya_cuda_fail(ctx, e, "lya_malloc(bucketing)"); }
     const unsigned blocks = (unsigned)((n_tiles + 3) / 4);
     if (bp->pow2)
         { k_bucket_count<true><<<blocks, 128, 0, s>>>(prep->head, prep->n_forest, *bp, pairs->pq, n, n_tiles, force_generic, keys, counts, ctx->d_counters); lya_note_launch(); }
@@ -285,10 +285,10 @@ lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *
 extern "C" void lya_plan_free(lya_ctx *ctx, lya_plan *pl)
 {
     if (!pl) return;
-    if (ctx) cudaSetDevice(ctx->device);
+    if (ctx) lya_enter(ctx);
     lya_prep_free(&pl->prep);
     lya_buckets_free(&pl->bk);
-    if (pl->pq) cudaFree(pl->pq);
+    if (pl->pq) lya_free(pl->pq);
     free(pl);
 }
 
@@ -306,7 +306,7 @@ extern "C" lya_status lya_plan_create(lya_ctx *ctx, const lya_forests *f, const 
     if (st) return st;
     if (f->n_forest > 0 && !(f->ux && f->uy && f->uz))
         return lya_fail(ctx, LYA_ERR_INVALID_ARG, "the pair kernels need ux,uy,uz (device); derive them once with the catalogue");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     int max_len = 0;
     st = lya_validate_forests(ctx, f, want_xi != 0, want_dmat != 0, &max_len);
     if (st) return st;
@@ -330,7 +330,7 @@ extern "C" lya_status lya_plan_create(lya_ctx *ctx, const lya_forests *f, const 
         pl->listed_degenerate = pl->bk.bad_pair == LYA_DEV_DEGENERATE;
         pl->visited = pl->bk.visited;
     } else if (pairs->n > 0) {
-        cudaError_t e = cudaMalloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)pairs->n);
+        cudaError_t e = lya_malloc(&pl->pq, sizeof(int32_t) * 2 * (size_t)pairs->n);
         if (e == cudaSuccess) e = cudaMemcpyAsync(pl->pq, pairs->pq, sizeof(int32_t) * 2 * (size_t)pairs->n, cudaMemcpyDeviceToDevice, s);
         if (e != cudaSuccess) { lya_plan_free(ctx, pl); return lya_cuda_fail(ctx, e, "lya_plan_create (pair list copy)"); }
     }

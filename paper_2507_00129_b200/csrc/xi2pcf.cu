@@ -648,7 +648,7 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
     if (!ctx) return LYA_ERR_INVALID_ARG;
     if (!pl) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf: plan is NULL");
     if (!pl->has_xi) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf: the plan was created without want_xi");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     const lya_forests *f = &pl->f;
     const lya_binning *b = &pl->b;
     const int nb = b->n_par * b->n_perp;
@@ -670,10 +670,10 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
     const bool use_fast = pl->use_fast;
     const LyaBuckets &bk = pl->bk;
     double *acc = NULL;                         // [S | W | N] accumulators
-    auto cleanup = [&]() { cudaFree(acc); };
+    auto cleanup = [&]() { lya_free(acc); };
     cudaEventRecord(ctx->ev[3], s);
-    cudaError_t e = cudaMalloc(&acc, nbt * 24);
-    if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "cudaMalloc(xi accumulators)");
+    cudaError_t e = lya_malloc(&acc, nbt * 24);
+    if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "lya_malloc(xi accumulators)");
     cudaMemsetAsync(acc, 0, nbt * 24, s);
     cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
 
@@ -854,13 +854,13 @@ extern "C" lya_status lya_xi2pcf_means(lya_ctx *ctx, const lya_forests *f, const
     if (st) return st;
     if (f->n_forest > 0 && !(f->ux && f->uy && f->uz)) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_means needs ux,uy,uz (device)");
     if (f->n_pix > 0 && !z) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_means: z is NULL");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     st = lya_validate_forests(ctx, f, false, false, NULL);
     if (st) return st;
     const int nb = b->n_par * b->n_perp;
     cudaStream_t s = ctx->stream;
     double *acc = NULL;
-    LYA_CUDA(cudaMalloc(&acc, sizeof(double) * 4 * (size_t)nb));
+    LYA_CUDA(lya_malloc(&acc, sizeof(double) * 4 * (size_t)nb));
     cudaMemsetAsync(acc, 0, sizeof(double) * 4 * (size_t)nb, s);
     cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
     XiParams P;
@@ -892,7 +892,7 @@ extern "C" lya_status lya_xi2pcf_means(lya_ctx *ctx, const lya_forests *f, const
     unsigned long long h[4] = {0, 0, 0, 0};
     if (e == cudaSuccess) e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    cudaFree(acc);
+    lya_free(acc);
     if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "lya_xi2pcf_means");
     if (h[3] != 0) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)");
     return LYA_OK;
@@ -904,7 +904,7 @@ extern "C" lya_status lya_xi_normalise(lya_ctx *ctx, int64_t n, const double *S,
     if (!ctx) return LYA_ERR_INVALID_ARG;
     if (n < 0 || (n > 0 && (!S || !W || !xi))) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi_normalise: bad arguments");
     if (n > ((int64_t)1 << 30)) return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_xi_normalise: n above 2^30");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     if (n > 0) {
         { k_xi_finalize<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(S, W, NULL, (int)n, NULL, NULL, NULL, xi); lya_note_launch(); }
         LYA_CUDA(cudaGetLastError());

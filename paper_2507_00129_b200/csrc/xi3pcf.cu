@@ -175,7 +175,7 @@ extern "C" lya_status lya_xi3pcf(lya_ctx *ctx, const lya_forests *f, const lya_t
     lya_status st = lya_check_forests_host(ctx, f, true, true, false);
     if (st) return st;
     if (f->n_forest > 0 && !(f->ux && f->uy && f->uz)) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi3pcf needs ux,uy,uz (device)");
-    LYA_CUDA(cudaSetDevice(ctx->device));
+    LYA_CUDA(lya_enter(ctx));
     st = lya_validate_forests(ctx, f, true, false, NULL);
     if (st) return st;
     const int64_t nb = lya_tri_nbins(tb), nf = f->n_forest, n = pairs->n;
@@ -184,14 +184,14 @@ extern "C" lya_status lya_xi3pcf(lya_ctx *ctx, const lya_forests *f, const lya_t
     unsigned *deg = NULL, *cursor = NULL;
     unsigned long long *off = NULL, *tmp = NULL;
     int32_t *adj = NULL;
-    auto cleanup = [&]() { cudaFree(acc); cudaFree(deg); cudaFree(cursor); cudaFree(off); cudaFree(tmp); cudaFree(adj); };
-    cudaError_t e = cudaMalloc(&acc, sizeof(double) * 3 * (size_t)nb);
-    if (e == cudaSuccess) e = cudaMalloc(&deg, sizeof(unsigned) * (size_t)(nf + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&cursor, sizeof(unsigned) * (size_t)(nf + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&off, sizeof(unsigned long long) * (size_t)(nf + 2));
-    if (e == cudaSuccess) e = cudaMalloc(&tmp, sizeof(unsigned long long) * (size_t)(nf / 2048 + 4));
-    if (e == cudaSuccess) e = cudaMalloc(&adj, sizeof(int32_t) * (size_t)(2 * n + 1));
-    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "cudaMalloc(lya_xi3pcf)"); }
+    auto cleanup = [&]() { lya_free(acc); lya_free(deg); lya_free(cursor); lya_free(off); lya_free(tmp); lya_free(adj); };
+    cudaError_t e = lya_malloc(&acc, sizeof(double) * 3 * (size_t)nb);
+    if (e == cudaSuccess) e = lya_malloc(&deg, sizeof(unsigned) * (size_t)(nf + 1));
+    if (e == cudaSuccess) e = lya_malloc(&cursor, sizeof(unsigned) * (size_t)(nf + 1));
+    if (e == cudaSuccess) e = lya_malloc(&off, sizeof(unsigned long long) * (size_t)(nf + 2));
+    if (e == cudaSuccess) e = lya_malloc(&tmp, sizeof(unsigned long long) * (size_t)(nf / 2048 + 4));
+    if (e == cudaSuccess) e = lya_malloc(&adj, sizeof(int32_t) * (size_t)(2 * n + 1));
+    if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "lya_malloc(lya_xi3pcf)"); }
     cudaEventRecord(ctx->ev[3], s);
     cudaMemsetAsync(acc, 0, sizeof(double) * 3 * (size_t)nb, s);
     cudaMemsetAsync(deg, 0, sizeof(unsigned) * (size_t)(nf + 1), s);
