@@ -30,7 +30,7 @@
 // Geometry is exact binary64, operation by operation (lya_internal.cuh), so N is
 // bit-identical to the oracle for any traversal order.
 #include <stdlib.h>
-#include "lya_internal.cuh"
+#include "lya_walk.cuh"
 
 namespace {
 
@@ -342,27 +342,7 @@ struct __align__(16) FastWarp {
     unsigned char jlo[FT], jhi[FT];          // per row of p: window [jlo, jhi) of q that can be in the grid
 };
 
-// ---- predicated shared-memory accesses (no divergence in the pair loop) ----
-__device__ __forceinline__ void sts_v2_if(bool p, unsigned addr, double x, double y)
-{
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q st.shared.v2.f64 [%1], {%2, %3};\n}"
-                 :: "r"((unsigned)p), "r"(addr), "d"(x), "d"(y) : "memory");
-}
-__device__ __forceinline__ void lds_v2_if(bool p, unsigned addr, double &x, double &y)
-{
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %2, 0;\n @q ld.shared.v2.f64 {%0, %1}, [%3];\n}"
-                 : "+d"(x), "+d"(y) : "r"((unsigned)p), "r"(addr) : "memory");
-}
-__device__ __forceinline__ void sts_u32_if(bool p, unsigned addr, unsigned v)
-{
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %0, 0;\n @q st.shared.u32 [%1], %2;\n}"
-                 :: "r"((unsigned)p), "r"(addr), "r"(v) : "memory");
-}
-__device__ __forceinline__ void lds_u32_if(bool p, unsigned addr, unsigned &v)
-{
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %1, 0;\n @q ld.shared.u32 %0, [%2];\n}"
-                 : "+r"(v) : "r"((unsigned)p), "r"(addr) : "memory");
-}
+// (predicated shared-memory accesses: lya_walk.cuh)
 
 // byte offset (16 * slot) of a pixel pair's sub-histogram entry
 template <bool POW2>
