@@ -240,9 +240,17 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    # functional dry runs of the N > 1 path on a box with ONE GPU (never a performance number): LYA_BENCH_BACKEND=gloo
+    # LYA_BENCH_ONE_DEVICE=1 put every rank on cuda:0 and reduce through the host
+    backend = os.environ.get("LYA_BENCH_BACKEND", "nccl")
+    if os.environ.get("LYA_BENCH_ONE_DEVICE"):
+        local = 0
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+        else:
+            dist.init_process_group(backend)
     if rank == 0:
         build.build()
     if world > 1:

@@ -12,14 +12,8 @@ __device__ __forceinline__ void sts_v2_if(bool p, unsigned addr, double x, doubl
 }
 __device__ __forceinline__ void lds_v2_if(bool p, unsigned addr, double &x, double &y)
 {
-#ifdef LYA_LDS_SPLIT
-    // two 64-bit loads: the destinations need not be an aligned register quad, so no moves follow
-    asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %2, 0;\n @q ld.shared.f64 %0, [%3];\n @q ld.shared.f64 %1, [%3+8];\n}"
-                 : "+d"(x), "+d"(y) : "r"((unsigned)p), "r"(addr) : "memory");
-#else
     asm volatile("{\n .reg .pred q;\n setp.ne.u32 q, %2, 0;\n @q ld.shared.v2.f64 {%0, %1}, [%3];\n}"
                  : "+d"(x), "+d"(y) : "r"((unsigned)p), "r"(addr) : "memory");
-#endif
 }
 __device__ __forceinline__ void sts_u32_if(bool p, unsigned addr, unsigned v)
 {
