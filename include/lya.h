@@ -203,10 +203,11 @@ lya_status lya_xi2pcf_means(lya_ctx *ctx, const lya_forests *f, const lya_binnin
  * D: double [NB*NB] row-major [A][B], NB = n_par*n_perp (NULL to skip the final
  * division); Dn: double [NB*NB] un-normalised sums (may be NULL if D is given; at
  * least one of D, Dn); Wd: double [NB] (may be NULL); stats as above (n_kept).
- * Every forest on the list must be non-degenerate (LYA_ERR_DEGENERATE_FOREST).  Forests of any
- * length (< 2^20 pixels) and any pixel spacing are accepted; forests of up to 72 pixels whose spacing
- * exceeds the r_par bin width take the fast kernel, the others a slower generic one.
- * LYA_ERR_CAPACITY if n_par > 512. */
+ * Every forest on the list must be non-degenerate (LYA_ERR_DEGENERATE_FOREST: sum w == 0, or all L equal up to
+ * rounding -- sum w (L-Lbar)^2 <= sum w (1e-12 |Lbar|)^2).  Forests of any length (< 2^20 pixels) and any pixel
+ * spacing are accepted; forests of up to 72 pixels whose spacing exceeds the r_par bin width take the fast kernel
+ * (the BASELINE shapes), forests of up to 144 pixels with a spacing down to an eighth of the bin width its second
+ * size class (native-resolution shapes), everything else a slower generic kernel.  LYA_ERR_CAPACITY if n_par > 512. */
 lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                     const lya_pairs *pairs, double reject_fraction, uint64_t seed,
                     double *D, double *Dn, double *Wd, lya_stats *stats);

@@ -53,7 +53,10 @@ constexpr int FD_ROWS = LYA_FD_ROWS;         // rows of p per pass-A group
 constexpr int FD_PAD = 2;
 constexpr int FD_SLOTS = 302;                // n_par * LYA_NCOL + 1 <= FD_SLOTS (the last slot used is garbage)
 constexpr int FD_KBATCH = 24;                // kept pairs drained together (coefficient tables)
-constexpr int FD_CHUNK = 8;
+#ifndef LYA_FD_CHUNK
+#define LYA_FD_CHUNK 8
+#endif
+constexpr int FD_CHUNK = LYA_FD_CHUNK;    // forest pairs claimed per atomic
 constexpr int FD_DS_MAX = 8;                 // largest diagonal stride the fast kernel takes
 // Profiling aids (compile-time, off by default; results are WRONG with any of them): -DLYA_ABL_NO_T23,
 // -DLYA_ABL_NO_T4, -DLYA_ABL_NO_MASK, -DLYA_ABL_NO_WALK drop one phase so that its share of the kernel time can
