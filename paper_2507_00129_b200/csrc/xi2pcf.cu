@@ -309,9 +309,10 @@ constexpr int FW = 14;                       // warps per block, one block per S
 constexpr int FTHREADS = FW * 32;
 constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
 #ifndef LYA_FROWS
-#define LYA_FROWS 16
+#define LYA_FROWS 12
 #endif
 constexpr int FROWS = LYA_FROWS;             // rows of p walked per pass (keeps lanes busy: DESIGN.md)
+static_assert(FROWS % 12 == 0 && FROWS <= 32, "a row group holds whole blocks of 1, 2, 3 or 4 rows");
 constexpr int FTP = ((FT + 15) / 16) * 16 + 2;   // p rows incl. sentinel rows
 constexpr int FPAD = 2;                      // sentinel pixels either side of q (reads are clamped)
 constexpr int FSLOTS = 612;                  // 2 * (n_par + 1) * LYA_NCOL <= FSLOTS
@@ -466,14 +467,20 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
 }
 
 template <bool POW2, bool CHECK>
-__device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
+__device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsigned n_base, int i0, int r0, int r1, int mq,
                                             int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
                                             unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
+    // D diagonals per lane, the smallest that covers the group in one pass; the rows [r0, r1] (inside one group of
+    // FROWS rows, i0 its first) are widened to a multiple of D rows aligned to the group
     const int nd = dhi - dlo + 1;
-    if (nd <= 32) xi_walk<1, POW2, CHECK>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts);
-    else if (nd <= 64) xi_walk<2, POW2, CHECK>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts);
-    else xi_walk<4, POW2, CHECK>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts);
+#define XI_WALK_D(D_) do { const int a = i0 + ((r0 - i0) / D_) * D_, b = a + ((r1 - a) / D_ + 1) * D_ - 1; \
+        xi_walk<D_, POW2, CHECK>(ws, sw_base, n_base, a, b, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts); } while (0)
+    if (nd <= 32) XI_WALK_D(1);
+    else if (nd <= 64) XI_WALK_D(2);
+    else if (nd <= 96) XI_WALK_D(3);
+    else XI_WALK_D(4);
+#undef XI_WALK_D
 }
 
 // merge a warp's sub-histogram (first column c0) into the global accumulators and clear it
@@ -596,7 +603,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
                 }
                 dlo = __reduce_min_sync(0xffffffffu, dlo); dhi = __reduce_max_sync(0xffffffffu, dhi);
                 r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
-                if (r1 >= r0) xi_walk_any<POW2, CHECK>(ws, sw_base, n_base, r0 & ~3, r1 | 3, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated, conflicts);
+                if (r1 >= r0) xi_walk_any<POW2, CHECK>(ws, sw_base, n_base, i0, r0, r1, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated, conflicts);
             }
         }
     }
