@@ -351,6 +351,7 @@ __global__ void k_dmat_divide(const double *Dn, const double *Wd, int nb, double
 }  // namespace
 
 #include "dmat_fast.cuh"
+#include "dmat_long.cuh"
 
 namespace {
 __global__ void k_fp_flag(const int32_t *pq, int64_t n, unsigned long long seed, unsigned long long thr, unsigned *flag)
@@ -460,7 +461,7 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
     P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.loglam = f->loglam;
     P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
     P.f_invS = scal; P.f_lbar = scal + nf; P.f_invV = scal + 2 * nf;
-    P.pq = use_fast ? bk.pq + 2 * (bk.n_fast + bk.n_fast2) : pl->pq;
+    P.pq = use_fast ? bk.pq + 2 * (bk.n_fast + bk.n_fast2 + bk.n_long) : pl->pq;
     P.n_pairs = use_fast ? bk.n_generic : pl->n_pairs;
     P.n_forest = nf;
     P.bp = bp;
@@ -471,7 +472,7 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
     if (P.LC > b->n_perp) P.LC = b->n_perp;
 
     cudaEventRecord(ctx->ev[0], s);
-    if (use_fast && bk.n_fast + bk.n_fast2 > 0) {
+    if (use_fast && bk.n_fast + bk.n_fast2 + bk.n_long > 0) {
         DmFastParams F;
         F.prep = pl->prep; F.bp = bp; F.seed = seed; F.thr = thr;
         F.Dn = Dn; F.Wd = Wd; F.counters = ctx->d_counters;
@@ -497,6 +498,12 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
             const size_t sm = DmPool<1>::SMEM_BYTES;
             if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_fast<true, true, 1>, th, sm) : launch(k_dmat_fast<false, true, 1>, th, sm);
             else e = bp.pow2 ? launch(k_dmat_fast<true, false, 1>, th, sm) : launch(k_dmat_fast<false, false, 1>, th, sm);
+        }
+        if (e == cudaSuccess && bk.n_long > 0) {              // long forests: up to 768 pixels, one CTA per forest pair
+            cudaMemsetAsync(ctx->d_counters + 4, 0, sizeof(unsigned long long), s);
+            F.pq = bk.pq + 2 * (bk.n_fast + bk.n_fast2); F.n_pairs = bk.n_long;
+            if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_long<true, true>, DL_THREADS, DL_SMEM_BYTES) : launch(k_dmat_long<false, true>, DL_THREADS, DL_SMEM_BYTES);
+            else e = bp.pow2 ? launch(k_dmat_long<true, false>, DL_THREADS, DL_SMEM_BYTES) : launch(k_dmat_long<false, false>, DL_THREADS, DL_SMEM_BYTES);
         }
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_dmat_fast launch"); }

@@ -138,8 +138,9 @@ __device__ __forceinline__ unsigned dm_key(const BinParams &bp, const PairBin &g
 
 // pass A over rows [r0, r1] (a multiple of D rows; rows >= len are sentinels) and diagonals [dlo, dhi].
 // `key`/`cur` are shared-memory addresses of H01 entries; H23 sits at a fixed offset.
-template <int D, bool POW2, bool CHECK, int CLS>
-__device__ __forceinline__ void dm_walk(DmFastWarp<CLS> &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi, int ds,
+// (WS: the staging area -- pce, peg, qce, qeg -- of a warp, DmFastWarp, or of a CTA, dmat_long.cuh)
+template <int D, bool POW2, bool CHECK, class WS>
+__device__ __forceinline__ void dm_walk(WS &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi, int ds,
                                         int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned npar,
                                         int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
@@ -239,15 +240,15 @@ __device__ __forceinline__ void dm_walk(DmFastWarp<CLS> &ws, unsigned h01, int r
     }
 }
 
-template <bool POW2, bool CHECK, int CLS>
-__device__ __forceinline__ void dm_walk_any(DmFastWarp<CLS> &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi, int ds,
+template <bool POW2, bool CHECK, class WS>
+__device__ __forceinline__ void dm_walk_any(WS &ws, unsigned h01, int r0, int r1, int mq, int dlo, int dhi, int ds,
                                             int sgn, const BinParams &bp, const PairBin &g, unsigned c0, unsigned lim, unsigned npar,
                                             int lane, unsigned long long &evaluated, unsigned &conflicts)
 {
     if (dhi < dlo) return;
     const int nd = dhi - dlo + 1;
-    if (nd <= 32 || ds > 1) dm_walk<1, POW2, CHECK, CLS>(ws, h01, r0, r1, mq, dlo, dhi, ds, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
-    else dm_walk<2, POW2, CHECK, CLS>(ws, h01, r0, r1, mq, dlo, dhi, 1, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
+    if (nd <= 32 || ds > 1) dm_walk<1, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, ds, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
+    else dm_walk<2, POW2, CHECK>(ws, h01, r0, r1, mq, dlo, dhi, 1, sgn, bp, g, c0, lim, npar, lane, evaluated, conflicts);
 }
 
 // transposed bin index b_perp * n_par + b_par of a pixel pair KNOWN to be inside the grid (exact windows)
@@ -589,7 +590,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
 #ifdef LYA_ABL_NO_WALK
                     continue;
 #endif
-                    dm_walk_any<POW2, CHECK, CLS>(ws, h01, r0 & ~1, r1 | 1, mq, sgn ? nlo : plo, sgn ? nhi : phi, ds, sgn, bp, g,
+                    dm_walk_any<POW2, CHECK>(ws, h01, r0 & ~1, r1 | 1, mq, sgn ? nlo : plo, sgn ? nhi : phi, ds, sgn, bp, g,
                                              (unsigned)c0, lim, npar, lane, evaluated, conflicts);
                 }
             }

@@ -106,11 +106,18 @@ void lya_prep_free(LyaPrep *p);
 #define LYA_NCOL 6                  // r_perp columns of a warp-private sub-histogram
 #define LYA_FAST_TILE 72            // longest forest the class-0 fast kernels stage in one piece
 #define LYA_FAST_TILE2 144          // same for class 1 (native-resolution shapes, DESIGN.md NEXT-3)
-#define LYA_DS_MAX 8                // largest diagonal stride (bin width / pixel spacing, rounded up) of class 1
+#define LYA_DS_MAX 8                // largest diagonal stride (bin width / pixel spacing, rounded up) of class 1 and of the long kernel
+#define LYA_LONG_TILE 768           // longest forest of the long-forest D kernel (one CTA per forest pair, dmat_long.cuh)
+// Bucket keys of the sorted forest-pair list: [0, n_perp) class 0 by first column, [n_perp, 2 n_perp) class 1 by
+// first column, then one key each for the long-forest D kernel, the generic kernels and the pairs with nothing in the grid.
+#define LYA_KEY_LONG(n_perp) (2 * (n_perp))
+#define LYA_KEY_GENERIC(n_perp) (2 * (n_perp) + 1)
+#define LYA_KEY_SKIP(n_perp) (2 * (n_perp) + 2)
+#define LYA_N_KEYS(n_perp) (2 * (n_perp) + 3)
 struct LyaBuckets {
     int32_t *pq;                    // device [n][2], sorted by key (stable)
     int64_t n;
-    int64_t n_fast, n_fast2, n_generic, n_skip;   // sizes of the four ranges of the sorted list, in this order
+    int64_t n_fast, n_fast2, n_long, n_generic, n_skip;   // sizes of the five ranges of the sorted list, in this order
     unsigned long long visited;     // sum n_p * n_q over the whole list
     int bad_pair;                   // LYA_DEV_BAD_PAIR: a pair outside [0, n_forest); LYA_DEV_DEGENERATE: a listed degenerate forest
 };
@@ -288,16 +295,17 @@ __device__ __forceinline__ int lya_pair_key(const BinParams &bp, const PairBin &
                                             const ForestHead &hq, int &c_first)
 {
     c_first = bp.n_perp;
-    if (hp.len == 0 || hq.len == 0) return 2 * bp.n_perp + 1;
+    if (hp.len == 0 || hq.len == 0) return LYA_KEY_SKIP(bp.n_perp);
     c_first = lya_col_of<POW2>(bp, g, __dadd_rn(hp.chi0, hq.chi0));
-    if (c_first >= bp.n_perp) return 2 * bp.n_perp + 1;             // r_perp grows with both pixels
+    if (c_first >= bp.n_perp) return LYA_KEY_SKIP(bp.n_perp);       // r_perp grows with both pixels
     int c_last = lya_col_of<POW2>(bp, g, __dadd_rn(hp.chi1, hq.chi1));
     if (c_last >= bp.n_perp) c_last = bp.n_perp - 1;
-    if (c_last - c_first >= LYA_NCOL) return 2 * bp.n_perp;
+    if (c_last - c_first >= LYA_NCOL) return LYA_KEY_GENERIC(bp.n_perp);
     const int len = max(hp.len, hq.len);
     const int ds = lya_pair_stride(bp, g, hq);
     if (len <= LYA_FAST_TILE && ds == 1) return c_first;
     if (len <= LYA_FAST_TILE2 && ds <= LYA_DS_MAX) return bp.n_perp + c_first;
-    return 2 * bp.n_perp;
+    if (len <= LYA_LONG_TILE && ds <= LYA_DS_MAX) return LYA_KEY_LONG(bp.n_perp);
+    return LYA_KEY_GENERIC(bp.n_perp);
 }
 #endif

@@ -95,13 +95,13 @@ __global__ void k_pack(lya_forests f, const unsigned long long *off2, LyaPrep P)
 
 // ---- (2) bucketing ------------------------------------------------------------------
 constexpr int BK_TILE = 2048;            // pairs per tile (one warp walks a tile in order)
-constexpr int BK_MAX_KEYS = 64 * 4 + 2;  // 2 n_perp + 2 <= this
+constexpr int BK_MAX_KEYS = 64 * 4 + 3;  // LYA_N_KEYS(n_perp) <= this
 
 template <bool POW2>
 __device__ __forceinline__ int pair_key(const ForestHead *head, int64_t n_forest, const BinParams &bp, int p, int q,
                                         unsigned long long &visited, int &bad)
 {
-    if ((unsigned)p >= (unsigned)n_forest || (unsigned)q >= (unsigned)n_forest) { bad = max(bad, (int)LYA_DEV_BAD_PAIR); return 2 * bp.n_perp + 1; }
+    if ((unsigned)p >= (unsigned)n_forest || (unsigned)q >= (unsigned)n_forest) { bad = max(bad, (int)LYA_DEV_BAD_PAIR); return LYA_KEY_SKIP(bp.n_perp); }
     const ForestHead hp = head[p], hq = head[q];
     if ((hp.flags | hq.flags) & 1) bad = max(bad, (int)LYA_DEV_DEGENERATE);   // (only set by a dmat catalogue)
     visited += (unsigned long long)hp.len * (unsigned long long)hq.len;
@@ -122,7 +122,7 @@ __global__ void k_bucket_count(const ForestHead *head, int64_t n_forest, BinPara
     __shared__ unsigned hist[4][BK_MAX_KEYS];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t tile = blockIdx.x * (int64_t)(blockDim.x >> 5) + w;
-    const int nk = 2 * bp.n_perp + 2;
+    const int nk = LYA_N_KEYS(bp.n_perp);
     for (int k = lane; k < nk; k += 32) hist[w][k] = 0;
     __syncwarp();
     unsigned long long visited = 0;
@@ -132,7 +132,7 @@ __global__ void k_bucket_count(const ForestHead *head, int64_t n_forest, BinPara
         for (int64_t k = k0 + lane; k < k1; k += 32) {
             const int2 e = ((const int2 *)pq)[k];
             int key = pair_key<POW2>(head, n_forest, bp, e.x, e.y, visited, bad);
-            if (force_generic && key < 2 * bp.n_perp) key = 2 * bp.n_perp;
+            if (force_generic && key < LYA_KEY_GENERIC(bp.n_perp)) key = LYA_KEY_GENERIC(bp.n_perp);
             keys[k] = (unsigned char)min(key, 255);
             atomicAdd(&hist[w][key], 1u);
         }
@@ -238,8 +238,8 @@ lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *
     const int64_t n = pairs->n;
     out->n = n;
     if (n == 0) return LYA_OK;
-    const int nk = 2 * bp->n_perp + 2;
-    if (nk > BK_MAX_KEYS || nk > 256) return lya_fail(ctx, LYA_ERR_CAPACITY, "n_perp above %d", 127);
+    const int nk = LYA_N_KEYS(bp->n_perp);
+    if (nk > BK_MAX_KEYS || nk > 256) return lya_fail(ctx, LYA_ERR_CAPACITY, "n_perp above %d", 126);
     cudaStream_t s = ctx->stream;
     const int64_t n_tiles = (n + BK_TILE - 1) / BK_TILE;
     const int64_t n_cnt = n_tiles * nk;
@@ -263,19 +263,20 @@ lya_status lya_bucket_pairs(lya_ctx *ctx, const LyaPrep *prep, const BinParams *
         { k_bucket_scatter<<<blocks, 128, 0, s>>>(pairs->pq, keys, n, n_tiles, nk, offsets, out->pq); lya_note_launch(); }
         e = cudaGetLastError();
     }
-    unsigned long long h_start[3] = {0, 0, 0};     // start of key n_perp (class 1), 2 n_perp (generic), 2 n_perp + 1 (skip)
+    unsigned long long h_start[4] = {0, 0, 0, 0};     // start of class 1, of the long range, of the generic range, of the skipped pairs
     unsigned long long h_cnt[4];
-    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_start[0], offsets + (int64_t)bp->n_perp * n_tiles, 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_start[1], offsets + (int64_t)(2 * bp->n_perp) * n_tiles, 8, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_start[2], offsets + (int64_t)(2 * bp->n_perp + 1) * n_tiles, 8, cudaMemcpyDeviceToHost, s);
+    const int first_key[4] = {bp->n_perp, LYA_KEY_LONG(bp->n_perp), LYA_KEY_GENERIC(bp->n_perp), LYA_KEY_SKIP(bp->n_perp)};
+    for (int k = 0; k < 4 && e == cudaSuccess; ++k)
+        e = cudaMemcpyAsync(&h_start[k], offsets + (int64_t)first_key[k] * n_tiles, 8, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h_cnt, ctx->d_counters, sizeof(h_cnt), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     drop();
     if (e != cudaSuccess) { lya_buckets_free(out); return lya_cuda_fail(ctx, e, "pair bucketing"); }
     out->n_fast = (int64_t)h_start[0];
     out->n_fast2 = (int64_t)(h_start[1] - h_start[0]);
-    out->n_generic = (int64_t)(h_start[2] - h_start[1]);
-    out->n_skip = n - (int64_t)h_start[2];
+    out->n_long = (int64_t)(h_start[2] - h_start[1]);
+    out->n_generic = (int64_t)(h_start[3] - h_start[2]);
+    out->n_skip = n - (int64_t)h_start[3];
     out->visited = h_cnt[1];
     out->bad_pair = (int)h_cnt[3];
     return LYA_OK;
@@ -315,7 +316,7 @@ extern "C" lya_status lya_plan_create(lya_ctx *ctx, const lya_forests *f, const 
     pl->f = *f; pl->b = *b; pl->bp = lya_make_binparams(b);
     pl->has_xi = want_xi != 0; pl->has_dmat = want_dmat != 0;
     pl->n_pairs = pairs->n; pl->max_len = max_len;
-    pl->use_fast = pairs->n > 0 && b->n_par <= LYA_FAST_NPAR_MAX && 2 * b->n_perp + 2 <= 256 && !ctx->force_generic;
+    pl->use_fast = pairs->n > 0 && b->n_par <= LYA_FAST_NPAR_MAX && LYA_N_KEYS(b->n_perp) <= 256 && !ctx->force_generic;
     cudaStream_t s = ctx->stream;
     if (pl->use_fast) {
         st = lya_prep_build(ctx, f, pl->has_xi, pl->has_dmat, &pl->prep);

@@ -668,7 +668,7 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
     P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.delta = f->delta;
     P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
     P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pl->pq;
-    P.n_pairs = use_fast ? bk.n_fast2 + bk.n_generic : pl->n_pairs;     // (class-1 pairs take the generic xi kernel)
+    P.n_pairs = use_fast ? bk.n_fast2 + bk.n_long + bk.n_generic : pl->n_pairs;     // (class-1 and long pairs take the generic xi kernel)
     P.n_forest = f->n_forest;
     P.bp = bp;
     P.S = acc; P.W = acc + nbt; P.N = (unsigned long long *)(acc + 2 * nbt);

@@ -299,6 +299,32 @@ def test_native_resolution_fast_class_next3(B, orc, cfg, fine, n, frac):
         c.close()
 
 
+@pytest.mark.parametrize("cfg,fine,n,frac", [(4, 5, 48, 0.99), (2, 4, 40, 0.9), (0, 12, 16, 0.98), (0, 8, 5, 0.0),
+                                             (4, 10, 12, 0.995)])
+def test_long_forest_kernel_next3(B, orc, cfg, fine, n, frac):
+    """NEXT-3 shapes with LONG forests (observed-frame 2.4 A, SDSS 3e-4 log steps, DESI 0.8 A):
+    145..768 pixels, spacing down to 0.5 Mpc/h (diagonal stride up to 8) take k_dmat_long, one CTA per forest pair
+    (per-warp H tables summed, banded stage-4 scan and drain).  f = 0.9 and f = 0 need several bands per forest
+    pair; the last case mixes in forests above 768 pixels, which stay with the generic kernel.  D and xi against
+    the naive oracle; the debug variant also checks that no H-table entry ever has two holders."""
+    f = gen.make_config(cfg, n_forest=n, density_scale=4.0, fine=fine)
+    assert np.diff(f.pix_off).max() > 144
+    seed = gen.mask_seed(cfg)
+    ref = orc.pairs_window(f)
+    od, ox = orc.dmat(f, ref, frac, seed), orc.xi(f, ref)
+    for check in (1, 0):
+        c = B.Context("cuda:0")
+        c.lya_set_option("check_holders", check)
+        d = B.DeviceForests(f)
+        pairs = c.lya_neighbours(d, B.binning())
+        assert pairs.n == len(ref)
+        g = c.lya_dmat(d, B.binning(), pairs, frac, seed)
+        check_dmat(g, od, f"long cfg{cfg} fine={fine} check={check}")
+        assert g["stats"]["n_scatter"] > 0.5 * od["n_kept"]           # k_dmat_long took (most of) the pairs
+        check_xi(c.lya_xi2pcf(d, B.binning(), pairs), ox, f"long cfg{cfg} fine={fine} xi")
+        c.close()
+
+
 def test_forest_pair_subsampling_next2(ctx, B, orc):
     """D from a subset of FOREST pairs = lya_pairs_subsample + lya_dmat(f = 0)."""
     f = gen.make_config(1, n_forest=150, density_scale=4.0)
