@@ -79,7 +79,7 @@ typedef struct {
 
 /* (r_par, r_perp) grid (4 Mpc/h bins up to 200 Mpc/h -> 50 x 50).
  * Requires 0 < r*_max <= 1e5, 1 <= n_* and n_par*n_perp <= 4096, bin width >= 0.01 (LYA_ERR_CAPACITY
- * otherwise); the fast kernels also need n_par <= 50 and n_perp <= 127, other grids take the generic ones. */
+ * otherwise); the fast kernels also need n_par <= 50 and n_perp <= 126, other grids take the generic ones. */
 typedef struct {
     double rpar_max, rperp_max;
     int32_t n_par, n_perp;
@@ -93,7 +93,7 @@ typedef struct {
     uint64_t n_evaluated;      /* pixel pairs whose separation was actually computed */
     uint64_t n_binned;         /* pixel pairs inside the grid (= sum_A N_A) */
     uint64_t n_kept;           /* lya_dmat: in-grid pixel pairs that passed the keep mask */
-    uint64_t n_scatter;        /* lya_dmat: fp64 scatter-adds into Dn/Wd issued by the fast kernel (0 for generic pairs) */
+    uint64_t n_scatter;        /* lya_dmat: fp64 scatter-adds into Dn/Wd issued by the fast and long-forest kernels (0 for generic pairs) */
     float    ms_main;          /* device time of the dominant kernel (CUDA events on the ctx stream) */
     float    ms_total;         /* device time of the whole call */
 } lya_stats;
@@ -207,7 +207,9 @@ lya_status lya_xi2pcf_means(lya_ctx *ctx, const lya_forests *f, const lya_binnin
  * rounding -- sum w (L-Lbar)^2 <= sum w (1e-12 |Lbar|)^2).  Forests of any length (< 2^20 pixels) and any pixel
  * spacing are accepted; forests of up to 72 pixels whose spacing exceeds the r_par bin width take the fast kernel
  * (the BASELINE shapes), forests of up to 144 pixels with a spacing down to an eighth of the bin width its second
- * size class (native-resolution shapes), everything else a slower generic kernel.  LYA_ERR_CAPACITY if n_par > 512. */
+ * size class, forests of up to 768 pixels at such a spacing the long-forest kernel (one thread block per forest
+ * pair; both for the native-resolution shapes of PAPER.md:79, 140-145), everything else -- longer forests, finer
+ * pixels, forest pairs spanning more than 6 r_perp columns -- a slower generic kernel.  LYA_ERR_CAPACITY if n_par > 512. */
 lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                     const lya_pairs *pairs, double reject_fraction, uint64_t seed,
                     double *D, double *Dn, double *Wd, lya_stats *stats);

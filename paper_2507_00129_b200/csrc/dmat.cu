@@ -60,9 +60,10 @@ __global__ void k_forest_scalars(const int64_t *pix_off, const double *w, const 
     int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= n_forest) return;
     int64_t a = pix_off[p], b = pix_off[p + 1];
-    double sw = 0.0, swl = 0.0;
-    for (int64_t k = a; k < b; ++k) { sw += w[k]; swl += w[k] * loglam[k]; }
-    double lb = (sw > 0.0) ? swl / sw : 0.0;
+    double sw = 0.0, swl = 0.0;                               // Lbar = L_0 + sum w (L - L_0) / sum w (exact differences: prep.cu)
+    const double l0 = (b > a) ? loglam[a] : 0.0;
+    for (int64_t k = a; k < b; ++k) { sw += w[k]; swl += w[k] * (loglam[k] - l0); }
+    double lb = (sw > 0.0) ? l0 + swl / sw : 0.0;
     double v = 0.0;
     for (int64_t k = a; k < b; ++k) { double u = loglam[k] - lb; v += w[k] * u * u; }
     const double tiny = 1e-12 * fabs(lb);                  // reading R-7: all weighted L equal up to rounding of L - Lbar

@@ -20,14 +20,17 @@
 namespace {
 
 #ifndef LYA_DL_WARPS
-#define LYA_DL_WARPS 12
+#define LYA_DL_WARPS 14
 #endif
 constexpr int DL_T = LYA_LONG_TILE;
 constexpr int DL_WARPS = LYA_DL_WARPS, DL_THREADS = DL_WARPS * 32;
 constexpr int DL_TP = ((DL_T + 15) / 16) * 16 + 2;      // rows of p incl. sentinel rows (walks cover whole row groups)
 constexpr int DL_TQ = DL_T + 2 * FD_PAD + 2;            // q incl. sentinels either side and the pad pixel of an odd forest
 constexpr int DL_KCAP = 2048;                           // kept pairs queued per band
-constexpr int DL_KBATCH = 16;                           // kept pairs a warp drains together
+#ifndef LYA_DL_KBATCH
+#define LYA_DL_KBATCH 8
+#endif
+constexpr int DL_KBATCH = LYA_DL_KBATCH;                // kept pairs a warp drains together
 constexpr int DL_RPT = (DL_T + DL_THREADS - 1) / DL_THREADS;   // rows per thread in the prefix sum
 static_assert(DL_T <= 0xffff && DL_T % 2 == 0 && DL_KBATCH <= 32, "record layout");
 
@@ -52,6 +55,22 @@ struct __align__(16) DlShared {
 constexpr size_t DL_SHARED_BYTES = (sizeof(DlShared) + 15) & ~(size_t)15;
 constexpr size_t DL_SMEM_BYTES = DL_SHARED_BYTES + sizeof(DmTable) * DL_WARPS;
 static_assert(DL_SMEM_BYTES <= (size_t)FD_SMEM_MAX, "k_dmat_long shared memory");
+
+// T2 / T3 of one kept pair over the pixels [lo, hi) of one forest (ce, eg) against the fixed pixel chi_fix of the
+// other: Dn[row][bin] += m0 * ea + mx * eg, one pixel per lane.  (With fine pixels several lanes of an instruction
+// reduce onto the same bin; adding such runs up first -- across lanes with shuffles, or with each lane on 3..8
+// consecutive pixels -- was measured no faster or slower at every spacing: profiles/r2i_next3_long_forests.md.)
+template <bool POW2>
+__device__ __forceinline__ void dl_t23(const BinParams &bp, const PairBin &g, const double2 *ce, const double *eg, int lo, int hi,
+                                       double chi_fix, double m0, double mx, double *row, int lane, unsigned &n_red)
+{
+#pragma unroll 1
+    for (int t = lo + lane; t < hi; t += 32) {
+        const double2 v = ce[t];
+        dm_red(row + (unsigned)dm_bin_in<POW2>(bp, g, chi_fix, v.x), fma(mx, eg[t], m0 * v.y));
+        n_red += 1u;
+    }
+}
 
 // drain of n <= DL_KBATCH kept pairs (kept[e] = (i << 16) | j) by one warp: T1..T4
 template <bool POW2>
@@ -97,18 +116,9 @@ __device__ __forceinline__ void dl_drain(DlShared &sh, DlDrainWarp &dw, const Dm
         const double ci = sh.pce[i].x, cj = qce[j].x;
         const unsigned row = dw.rowoff[e];
         const int jh = sh.jhi[i], ih = dw.ihi[e];
-#pragma unroll 1
-        for (int j2 = (int)sh.jlo[i] + lane; j2 < jh; j2 += 32) {                     // T2
-            const double2 q2 = qce[j2];
-            dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, ci, q2.x)), fma(m1, qeg[j2], m0 * q2.y));
-            n_red += 1u;
-        }
-#pragma unroll 1
-        for (int i2 = (int)dw.ilo[e] + lane; i2 < ih; i2 += 32) {                     // T3
-            const double2 p2 = sh.pce[i2];
-            dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, p2.x, cj)), fma(m2, sh.peg[i2], m0 * p2.y));
-            n_red += 1u;
-        }
+        const int jl = sh.jlo[i], il = dw.ilo[e];
+dl_t23<POW2>(bp, g, qce, qeg, jl, jh, ci, m0, m1, Dn + row, lane, n_red);          // T2
+        dl_t23<POW2>(bp, g, sh.pce, sh.peg, il, ih, cj, m0, m2, Dn + row, lane, n_red);    // T3
     }
     const unsigned col0 = (unsigned)(c0 * bp.n_par);
     for (int e0 = 0; e0 < n; e0 += FD_T4B) {                                          // T4

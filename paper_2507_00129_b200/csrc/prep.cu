@@ -47,18 +47,22 @@ __global__ void k_pack(lya_forests f, const unsigned long long *off2, LyaPrep P)
     const int n = (int)(f.pix_off[p + 1] - a);
     const long long o = (long long)off2[p];
     const int npad = (n + 1) & ~1;
+    // Lbar = L_0 + sum w (L - L_0) / sum w: the differences are exact, so Lbar is the correctly rounded mean but
+    // for rare ties.  (sum w L / sum w in plain fp64 can be an ulp off, and for a forest whose L spans 1e-4 an ulp
+    // of Lbar is 1e-11 of u = L - Lbar: visible in D where eta should cancel exactly, e.g. a 2-pixel forest.)
     double dmin = 1e300, sw = 0.0, swl = 0.0;
+    const double l0 = (DMAT && n > 0) ? f.loglam[a] : 0.0;
     for (int t = lane; t < n; t += 32) {
         double c = f.chi[a + t];
         if (t + 1 < n) dmin = fmin(dmin, f.chi[a + t + 1] - c);
-        if (DMAT) { double w = f.w[a + t]; sw += w; swl += w * f.loglam[a + t]; }
+        if (DMAT) { double w = f.w[a + t]; sw += w; swl += w * (f.loglam[a + t] - l0); }
     }
     dmin = warp_min(dmin);
     double lbar = 0.0, invS = 0.0, invV = 0.0;
     int flags = 0;
     if (DMAT) {
         sw = warp_sum(sw); swl = warp_sum(swl);
-        lbar = (sw > 0.0) ? swl / sw : 0.0;
+        lbar = (sw > 0.0) ? l0 + swl / sw : 0.0;
         double v = 0.0;
         for (int t = lane; t < n; t += 32) { double u = f.loglam[a + t] - lbar; v += f.w[a + t] * u * u; }
         v = warp_sum(v);
