@@ -225,6 +225,8 @@ def main():
     ap.add_argument("--cpu-dmat-div", type=int, default=20, help="naive D runs on 1/N of the sample's forest pairs")
     ap.add_argument("--forests", type=int, default=0,
                     help="profiling only: a shaped sub-catalogue of this many forests (same sky density)")
+    ap.add_argument("--force-generic", action="store_true",
+                    help="route every forest pair to the generic kernels (lya_set_option force_generic): the comparison figure for the fast / long-forest kernels")
     ap.add_argument("--fine", type=int, default=1,
                     help="NEXT-3 shapes: divide the pixel step by this factor (gen.make_config(fine=...)); throughput only")
     args = ap.parse_args()
@@ -263,6 +265,8 @@ def main():
     f = gen.make_config(wl["cfg"], n_forest=args.forests or None, fine=args.fine,
                         seed=None if strong else shard.rank_seed(gen.SEED_BASE + wl["cfg"], rank))
     ctx = B.Context(f"cuda:{local}")
+    if args.force_generic:
+        ctx.lya_set_option("force_generic", 1)
     d = B.DeviceForests(f, device=f"cuda:{local}")
     b = B.binning()
     do_d = not args.no_dmat
@@ -392,7 +396,7 @@ def main():
                  "measured_peaks": mp}
         if sd is not None:
             alg_d = 10.0 * sd["n_binned"] + 4.0 * sd["n_scatter"]
-            roof_d = {"bound": "alu", "kernel": "k_dmat_fast", "achieved": alg_d / t_dm / 1e12, "peak": peak_alu / 1e12,
+            roof_d = {"bound": "alu", "kernel": "k_dmat (generic)" if args.force_generic else ("k_dmat_fast" if args.fine == 1 else "k_dmat_fast / k_dmat_long"), "achieved": alg_d / t_dm / 1e12, "peak": peak_alu / 1e12,
                       "unit": "Tops/s (fp64 lane-operations)", "frac": alg_d / t_dm / peak_alu, "traffic": None,
                       "peak_source": peak_src,
                       "scatter_adds_per_s": sd["n_scatter"] / t_dm,
@@ -412,7 +416,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if strong else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload + (f" fine={args.fine}" if args.fine != 1 else ""), "description": wl["desc"],
+            "config": {"workload": args.workload + (f" fine={args.fine}" if args.fine != 1 else "") + (" force_generic" if args.force_generic else ""), "description": wl["desc"],
                        "n_forest": f.n_forest, "n_pix": f.n_pix,
                        "bins": "50x50x4Mpc/h", "reject_fraction": frac, "dmat": do_d,
                        "l2": ("catalogue %.2f GB + forest-pair list %.2f GB per step vs 126 MB of L2 (%s); Dn (50 MB) "

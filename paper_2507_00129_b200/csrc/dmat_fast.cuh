@@ -210,9 +210,10 @@ __device__ __forceinline__ void dm_walk(WS &ws, unsigned h01, int r0, int r1, in
                 unsigned key_n[D];
                 double fa_n[D], fg_n[D];
                 {
-                    const int j = min(max(i + dl + D, -FD_PAD), mq + FD_PAD - 1);
-                    const double2 v = qce[j];
-                    wc[u] = v.x; wa[u] = v.y; wg[u] = qeg[j];
+                    // (one unsigned min clamps both ends: a negative index wraps to the right-hand sentinel)
+                    const unsigned j = min((unsigned)(i + dl + D + FD_PAD), (unsigned)(mq + 2 * FD_PAD - 1));
+                    const double2 v = ws.qce[j];
+                    wc[u] = v.x; wa[u] = v.y; wg[u] = ws.qeg[j];
                 }
                 const double2 pv = ws.pce[i + 1];
                 const double pg_n = ws.peg[i + 1];

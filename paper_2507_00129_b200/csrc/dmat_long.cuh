@@ -31,6 +31,10 @@ constexpr int DL_KCAP = 2048;                           // kept pairs queued per
 #define LYA_DL_KBATCH 8
 #endif
 constexpr int DL_KBATCH = LYA_DL_KBATCH;                // kept pairs a warp drains together
+#ifndef LYA_DL_ROWS
+#define LYA_DL_ROWS 16
+#endif
+constexpr int DL_ROWS = LYA_DL_ROWS;                    // rows of p per pass-A task (even, <= 32)
 constexpr int DL_RPT = (DL_T + DL_THREADS - 1) / DL_THREADS;   // rows per thread in the prefix sum
 static_assert(DL_T <= 0xffff && DL_T % 2 == 0 && DL_KBATCH <= 32, "record layout");
 
@@ -251,16 +255,16 @@ __global__ void __launch_bounds__(DL_THREADS, 1) k_dmat_long(DmFastParams P)
         }
         // ---- pass A: tasks (row group, side), each warp into its own table ----
         {
-            const int n_tasks = 2 * ((mp + FD_ROWS - 1) / FD_ROWS);
+            const int n_tasks = 2 * ((mp + DL_ROWS - 1) / DL_ROWS);
             for (;;) {
                 int task = 0;
                 if (lane == 0) task = (int)atomicAdd(&sh.next_task, 1u);
                 task = __shfl_sync(0xffffffffu, task, 0);
                 if (task >= n_tasks) break;
-                const int i0 = (task >> 1) * FD_ROWS, sgn = -(task & 1);
+                const int i0 = (task >> 1) * DL_ROWS, sgn = -(task & 1);
                 const int i = i0 + lane;
                 int lo = 1 << 20, hi = -(1 << 20), r0 = 1 << 20, r1 = -1;
-                if (lane < FD_ROWS && i < mp) {
+                if (lane < DL_ROWS && i < mp) {
                     const int jl = sh.jlo[i], jh = sh.jhi[i], jx = sh.jx[i];
                     if (sgn == 0) { if (jx > jl) { lo = jl - i; hi = jx - 1 - i; r0 = i; r1 = i; } }
                     else if (jh > jx) { lo = jx - i; hi = jh - 1 - i; r0 = i; r1 = i; }

@@ -361,11 +361,13 @@ __device__ __forceinline__ unsigned xi_key(const BinParams &bp, const PairBin &g
         bx = (rpar < bp.rpar_max) ? min(lya_floor_u32(__dmul_rn(rpar, bp.inv_par)), (unsigned)(bp.n_par - 1)) : (unsigned)bp.n_par;
         by = (rperp < bp.rperp_max) ? min(lya_floor_u32(__dmul_rn(rperp, bp.inv_perp)), (unsigned)(bp.n_perp - 1)) : 0x7fffffffu;
     }
-    const bool valid = (bx < np1 - 1u) & (by - c0 < (unsigned)LYA_NCOL);   // else -> the garbage entry (0, n_par)
-    bx = valid ? bx : np1 - 1u;
-    const unsigned col = valid ? by - c0 : 0u;
+    const unsigned col = by - c0;
     const unsigned side = (unsigned)__double2hiint(d) >> 31;
-    return (col * (2u * np1) + side * np1 + bx) * 16u;
+    const unsigned off = ((col * 2u + side) * np1 + bx) << 4;
+    unsigned key;                                                           // outside the window -> the garbage entry (0, 0, n_par)
+    asm("{\n .reg .pred v;\n setp.lt.u32 v, %1, %2;\n setp.lt.and.u32 v, %3, %4, v;\n selp.u32 %0, %5, %6, v;\n}"
+        : "=r"(key) : "r"(bx), "r"(np1 - 1u), "r"(col), "r"((unsigned)LYA_NCOL), "r"(off), "r"((np1 - 1u) << 4));
+    return key;
 }
 
 // Walk rows [r0, r1] of p against the diagonals [dlo, dhi], D adjacent diagonals per lane.
@@ -436,8 +438,9 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
                 double fa_n[D], fw_n[D];
                 unsigned key_n[D];
                 {
-                    const int j = min(max(i + dl + D, -FPAD), mq + FPAD - 1);
-                    wc[u] = qc[j]; wa[u] = qa[j]; ww[u] = qw[j];
+                    // (one unsigned min clamps both ends: a negative index wraps to the right-hand sentinel)
+                    const unsigned j = min((unsigned)(i + dl + D + FPAD), (unsigned)(mq + 2 * FPAD - 1));
+                    wc[u] = ws.qc[j]; wa[u] = ws.qa[j]; ww[u] = ws.qw[j];
                     const double pci = ws.pc[i + 1];
 #pragma unroll
                     for (int k = 0; k < D; ++k) {
