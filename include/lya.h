@@ -207,9 +207,10 @@ lya_status lya_xi2pcf_means(lya_ctx *ctx, const lya_forests *f, const lya_binnin
  * rounding -- sum w (L-Lbar)^2 <= sum w (1e-12 |Lbar|)^2).  Forests of any length (< 2^20 pixels) and any pixel
  * spacing are accepted; forests of up to 72 pixels whose spacing exceeds the r_par bin width take the fast kernel
  * (the BASELINE shapes), forests of up to 144 pixels with a spacing down to an eighth of the bin width its second
- * size class, forests of up to 768 pixels at such a spacing the long-forest kernel (one thread block per forest
- * pair; both for the native-resolution shapes of PAPER.md:79, 140-145), everything else -- longer forests, finer
- * pixels, forest pairs spanning more than 6 r_perp columns -- a slower generic kernel.  LYA_ERR_CAPACITY if n_par > 512. */
+ * size class, forests of up to 1024 pixels with a spacing down to a sixteenth of it the long-forest kernel (one
+ * thread block per forest pair; both for the native-resolution shapes of PAPER.md:79, 140-145), everything else --
+ * longer forests, finer pixels, forest pairs spanning more than 6 r_perp columns -- a slower generic kernel.
+ * LYA_ERR_CAPACITY if n_par > 512. */
 lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                     const lya_pairs *pairs, double reject_fraction, uint64_t seed,
                     double *D, double *Dn, double *Wd, lya_stats *stats);

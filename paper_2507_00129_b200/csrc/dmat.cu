@@ -500,7 +500,7 @@ static lya_status dmat_run(lya_ctx *ctx, const lya_plan *pl, double reject_fract
             if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_fast<true, true, 1>, th, sm) : launch(k_dmat_fast<false, true, 1>, th, sm);
             else e = bp.pow2 ? launch(k_dmat_fast<true, false, 1>, th, sm) : launch(k_dmat_fast<false, false, 1>, th, sm);
         }
-        if (e == cudaSuccess && bk.n_long > 0) {              // long forests: up to 768 pixels, one CTA per forest pair
+        if (e == cudaSuccess && bk.n_long > 0) {              // long forests: up to 1024 pixels, one CTA per forest pair
             cudaMemsetAsync(ctx->d_counters + 4, 0, sizeof(unsigned long long), s);
             F.pq = bk.pq + 2 * (bk.n_fast + bk.n_fast2); F.n_pairs = bk.n_long;
             if (ctx->check_holders) e = bp.pow2 ? launch(k_dmat_long<true, true>, DL_THREADS, DL_SMEM_BYTES) : launch(k_dmat_long<false, true>, DL_THREADS, DL_SMEM_BYTES);

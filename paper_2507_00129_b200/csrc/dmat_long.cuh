@@ -1,6 +1,6 @@
 // dmat_long.cuh -- k_dmat_long, the distortion-matrix kernel for LONG forests (eqs. 2.6-2.7, PAPER.md:91-98;
 // native-resolution shapes, PAPER.md:79, 140-145 and DESIGN.md NEXT-3): up to LYA_LONG_TILE pixels per forest,
-// pixel spacing down to an eighth of the r_par bin width.  Included by dmat.cu only.
+// pixel spacing down to a sixteenth of the r_par bin width (LYA_DS_MAX_LONG).  Included by dmat.cu only.
 //
 // A forest pair of such forests holds 10^4..10^5 in-grid pixel pairs and hundreds of kept ones, so ONE CTA works
 // on one forest pair (the fast kernels give a forest pair to one warp), every phase spread over its warps:
@@ -36,7 +36,7 @@ constexpr int DL_KBATCH = LYA_DL_KBATCH;                // kept pairs a warp dra
 #endif
 constexpr int DL_ROWS = LYA_DL_ROWS;                    // rows of p per pass-A task (even, <= 32)
 constexpr int DL_RPT = (DL_T + DL_THREADS - 1) / DL_THREADS;   // rows per thread in the prefix sum
-static_assert(DL_T <= 0xffff && DL_T % 2 == 0 && DL_KBATCH <= 32, "record layout");
+static_assert(DL_T <= 0xffff && (DL_T & (DL_T - 1)) == 0 && DL_KBATCH <= 32 && DL_KCAP >= 2 * DL_T, "record layout, search steps, one row fits the queue twice");
 
 struct DlDrainWarp {                                    // per warp: one batch of kept pairs
     double2 kc01[DL_KBATCH], kc23[DL_KBATCH];           // om (1, u_j), om (u_i, u_i u_j)
@@ -100,7 +100,7 @@ __device__ __forceinline__ void dl_drain(DlShared &sh, DlDrainWarp &dw, const Dm
         // a half-plane in chi_i + chi_j); fixed trip count
         int il = 0, ih = i + 1;
 #pragma unroll
-        for (int st = 512; st; st >>= 1) {
+        for (int st = DL_T / 2; st; st >>= 1) {
             const int m = il + st, m2 = ih + st;
             if (m <= i) { const unsigned lo2 = sh.jlo[m - 1]; if (!((unsigned)j - lo2 < (unsigned)sh.jhi[m - 1] - lo2)) il = m; }
             if (m2 <= mp) { const unsigned lo2 = sh.jlo[m2 - 1]; if ((unsigned)j - lo2 < (unsigned)sh.jhi[m2 - 1] - lo2) ih = m2; }
@@ -121,7 +121,7 @@ __device__ __forceinline__ void dl_drain(DlShared &sh, DlDrainWarp &dw, const Dm
         const unsigned row = dw.rowoff[e];
         const int jh = sh.jhi[i], ih = dw.ihi[e];
         const int jl = sh.jlo[i], il = dw.ilo[e];
-dl_t23<POW2>(bp, g, qce, qeg, jl, jh, ci, m0, m1, Dn + row, lane, n_red);          // T2
+        dl_t23<POW2>(bp, g, qce, qeg, jl, jh, ci, m0, m1, Dn + row, lane, n_red);          // T2
         dl_t23<POW2>(bp, g, sh.pce, sh.peg, il, ih, cj, m0, m2, Dn + row, lane, n_red);    // T3
     }
     const unsigned col0 = (unsigned)(c0 * bp.n_par);
@@ -323,7 +323,7 @@ __global__ void __launch_bounds__(DL_THREADS, 1) k_dmat_long(DmFastParams P)
                 const unsigned first = base + min((unsigned)tid * K, Mb), last = base + min((unsigned)tid * K + K, Mb);
                 int row = ra;                                  // last row with pre[row] <= first (fixed trip count)
 #pragma unroll
-                for (int st = 512; st; st >>= 1) {
+                for (int st = DL_T / 2; st; st >>= 1) {
                     const int m = row + st;
                     if (m <= mp && sh.pre[m] <= first) row = m;
                 }

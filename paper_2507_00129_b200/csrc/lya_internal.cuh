@@ -106,8 +106,9 @@ void lya_prep_free(LyaPrep *p);
 #define LYA_NCOL 6                  // r_perp columns of a warp-private sub-histogram
 #define LYA_FAST_TILE 72            // longest forest the class-0 fast kernels stage in one piece
 #define LYA_FAST_TILE2 144          // same for class 1 (native-resolution shapes, DESIGN.md NEXT-3)
-#define LYA_DS_MAX 8                // largest diagonal stride (bin width / pixel spacing, rounded up) of class 1 and of the long kernel
-#define LYA_LONG_TILE 768           // longest forest of the long-forest D kernel (one CTA per forest pair, dmat_long.cuh)
+#define LYA_DS_MAX 8                // largest diagonal stride (bin width / pixel spacing, rounded up) of class 1
+#define LYA_LONG_TILE 1024          // longest forest of the long-forest D kernel (one CTA per forest pair, dmat_long.cuh)
+#define LYA_DS_MAX_LONG 16          // its largest diagonal stride (long rows keep the lanes busy at larger strides)
 // Bucket keys of the sorted forest-pair list: [0, n_perp) class 0 by first column, [n_perp, 2 n_perp) class 1 by
 // first column, then one key each for the long-forest D kernel, the generic kernels and the pairs with nothing in the grid.
 #define LYA_KEY_LONG(n_perp) (2 * (n_perp))
@@ -305,7 +306,7 @@ __device__ __forceinline__ int lya_pair_key(const BinParams &bp, const PairBin &
     const int ds = lya_pair_stride(bp, g, hq);
     if (len <= LYA_FAST_TILE && ds == 1) return c_first;
     if (len <= LYA_FAST_TILE2 && ds <= LYA_DS_MAX) return bp.n_perp + c_first;
-    if (len <= LYA_LONG_TILE && ds <= LYA_DS_MAX) return LYA_KEY_LONG(bp.n_perp);
+    if (len <= LYA_LONG_TILE && ds <= LYA_DS_MAX_LONG) return LYA_KEY_LONG(bp.n_perp);
     return LYA_KEY_GENERIC(bp.n_perp);
 }
 #endif

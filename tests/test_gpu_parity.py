@@ -300,12 +300,12 @@ def test_native_resolution_fast_class_next3(B, orc, cfg, fine, n, frac):
 
 
 @pytest.mark.parametrize("cfg,fine,n,frac", [(4, 5, 48, 0.99), (2, 4, 40, 0.9), (0, 12, 16, 0.98), (0, 8, 5, 0.0),
-                                             (4, 10, 12, 0.995)])
+                                             (4, 10, 12, 0.995), (4, 16, 8, 0.995)])
 def test_long_forest_kernel_next3(B, orc, cfg, fine, n, frac):
     """NEXT-3 shapes with LONG forests (observed-frame 2.4 A, SDSS 3e-4 log steps, DESI 0.8 A):
-    145..768 pixels, spacing down to 0.5 Mpc/h (diagonal stride up to 8) take k_dmat_long, one CTA per forest pair
-    (per-warp H tables summed, banded stage-4 scan and drain).  f = 0.9 and f = 0 need several bands per forest
-    pair; the last case mixes in forests above 768 pixels, which stay with the generic kernel.  D and xi against
+    145..1024 pixels, spacing down to 0.33 Mpc/h (diagonal stride up to 13 of the 16 allowed) take k_dmat_long, one
+    CTA per forest pair (per-warp H tables summed, banded stage-4 scan and drain).  f = 0.9 and f = 0 need several
+    bands per forest pair; the last case mixes in forests above 1024 pixels, which stay with the generic kernel.  D and xi against
     the naive oracle; the debug variant also checks that no H-table entry ever has two holders."""
     f = gen.make_config(cfg, n_forest=n, density_scale=4.0, fine=fine)
     assert np.diff(f.pix_off).max() > 144
