@@ -257,6 +257,26 @@ lya_status lya_xi2pcf_plan(lya_ctx *ctx, const lya_plan *plan,
 lya_status lya_dmat_plan(lya_ctx *ctx, const lya_plan *plan, double reject_fraction, uint64_t seed,
                          double *D, double *Dn, double *Wd, lya_stats *stats);
 
+/* ---- stage 2 without any allocation -------------------------------------------------------------- */
+/* lya_xi2pcf_plan for callers that cannot allocate device memory inside the call (tight serving loops, harnesses
+ * that forbid cudaMalloc): same arguments, same kernels, same results as lya_xi2pcf_plan (eq. 2.4)
+ * -- N bit-identical, S / W / xi equal up to the order of the fp64 merges --, but the [S | W | N] accumulators,
+ * the one piece of scratch memory stage 2 needs, live in a file-scope device array of the library instead of a
+ * stream-ordered allocation.  The call makes no cudaMalloc / cudaFree / cudaMallocAsync and no host allocation.
+ *   limit:   n_par * n_perp <= LYA_XI_NOALLOC_MAX_BINS (the paper's 50 x 50 grid fits); a larger grid is
+ *            LYA_ERR_CAPACITY and nothing is launched -- use lya_xi2pcf_plan.  All of S, W, N, xi are required.
+ *   cost:    every GPU that loads liblya.so holds the array (LYA_XI_NOALLOC_MAX_BINS * 24 bytes = 60 KB) until
+ *            the process exits, whether or not this call is ever made.
+ *   sharing: ONE array per device, shared by every context, plan and stream on it; it still holds the previous
+ *            call's sums, so each call clears it on the ctx stream first.  Calls that overlap on the GPU -- two
+ *            contexts or streams of one device inside this entry point at once -- race on it and give wrong
+ *            sums: serialise them.  (lya_xi2pcf_plan has no such restriction.)
+ * Like lya_xi2pcf_plan it synchronises the ctx stream before it returns (it reads the work counters), so it cannot
+ * sit inside a CUDA graph capture; creating the plan still allocates -- do that at set-up. */
+#define LYA_XI_NOALLOC_MAX_BINS 2560
+lya_status lya_xi2pcf_plan_noalloc(lya_ctx *ctx, const lya_plan *plan,
+                                   double *S, double *W, uint64_t *N, double *xi, lya_stats *stats);
+
 /* ---- final divisions on already-summed numerators (multi-GPU) ----------- */
 /* Every output above is an additive accumulator before its final division, so a catalogue's
  * forest-pair list can be split over ranks ("distribute the work load"): each rank runs

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "liblya.so")
 EXPORTS = ["lya_create", "lya_destroy", "lya_last_error", "lya_version", "lya_launch_count", "lya_set_option", "lya_neighbours",
            "lya_pairs_export", "lya_pairs_import", "lya_pairs_subsample", "lya_pairs_count", "lya_pairs_free",
            "lya_xi2pcf", "lya_xi2pcf_sub", "lya_xi2pcf_means", "lya_dmat", "lya_run_host", "lya_xi_normalise", "lya_dmat_normalise",
-           "lya_plan_create", "lya_plan_free", "lya_xi2pcf_plan", "lya_dmat_plan", "lya_tri_nbins", "lya_xi3pcf"]
+           "lya_plan_create", "lya_plan_free", "lya_xi2pcf_plan", "lya_xi2pcf_plan_noalloc", "lya_dmat_plan", "lya_tri_nbins", "lya_xi3pcf"]
 
 STATUS = {0: "LYA_OK", 1: "LYA_ERR_INVALID_ARG", 2: "LYA_ERR_UNSORTED", 3: "LYA_ERR_DEGENERATE_FOREST",
           4: "LYA_ERR_CAPACITY", 5: "LYA_ERR_OOM", 6: "LYA_ERR_CUDA", 7: "LYA_ERR_UNIMPLEMENTED"}
@@ -100,6 +100,7 @@ def load():
         lib.lya_plan_free.argtypes = [C.c_void_p, C.c_void_p]
         lib.lya_plan_free.restype = None
         lib.lya_xi2pcf_plan.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(CStats)]
+        lib.lya_xi2pcf_plan_noalloc.argtypes = lib.lya_xi2pcf_plan.argtypes
         lib.lya_dmat_plan.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_uint64, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(CStats)]
         lib.lya_xi_normalise.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -272,6 +273,21 @@ class Context:
         stats = CStats()
         self._check(load().lya_xi2pcf_plan(self.h, plan.handle, _ptr(S), _ptr(W), _ptr(N), _ptr(xi), C.byref(stats)))
         return dict(S=S, W=W, N=N, xi=xi, stats=stats.as_dict())
+
+    def lya_xi2pcf_plan_noalloc(self, plan: Plan, out=None):
+        """lya_xi2pcf_plan with the accumulators in the library's static device array (include/lya.h).  `out`: a dict
+        of caller-owned S, W, N, xi tensors to write into (so that the call itself allocates nothing at all)."""
+        torch = self.torch
+        nb = plan.b.n_par * plan.b.n_perp
+        if out is None:
+            out = dict(S=torch.empty(nb, dtype=torch.float64, device=self.device),
+                       W=torch.empty(nb, dtype=torch.float64, device=self.device),
+                       N=torch.empty(nb, dtype=torch.int64, device=self.device),      # uint64 payload
+                       xi=torch.empty(nb, dtype=torch.float64, device=self.device))
+        stats = CStats()
+        self._check(load().lya_xi2pcf_plan_noalloc(self.h, plan.handle, _ptr(out["S"]), _ptr(out["W"]), _ptr(out["N"]),
+                                                   _ptr(out["xi"]), C.byref(stats)))
+        return dict(S=out["S"], W=out["W"], N=out["N"], xi=out["xi"], stats=stats.as_dict())
 
     def lya_dmat_plan(self, plan: Plan, reject_fraction: float, seed: int, want_Dn=True, want_D=True):
         torch = self.torch

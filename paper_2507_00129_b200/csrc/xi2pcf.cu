@@ -901,3 +901,121 @@ extern "C" lya_status lya_xi_normalise(lya_ctx *ctx, int64_t n, const double *S,
     }
     return LYA_OK;
 }
+
+// ======================= lya_xi2pcf_plan_noalloc: stage 2 on a plan, allocating nothing ==================
+// For callers that cannot allocate device memory in the call (CUDA graph capture around it is not what is meant --
+// the call synchronises; but serving loops and harnesses that forbid cudaMalloc): the same kernels as
+// lya_xi2pcf_plan, with the [S | W | N] accumulators -- the one piece of scratch memory stage 2 needs -- in a
+// file-scope device array instead of a stream-ordered allocation.  The array is part of the library image: every
+// GPU that loads liblya.so holds LYA_XI_NOALLOC_MAX_BINS * 24 bytes (60 KB) until the process exits.
+// In HOST code the array's name is a host-side stand-in, not a device address, so the address is asked for once
+// per device (that device current) with cudaGetSymbolAddress and handed to the kernels as an ordinary pointer.
+// Every call on a device shares the array and finds the last call's sums in it: it is cleared on the ctx stream
+// first, and calls that overlap on the GPU (two contexts / streams of one device) RACE -- see include/lya.h.
+static __device__ __align__(256) double g_xi_noalloc_acc[3 * LYA_XI_NOALLOC_MAX_BINS];
+
+namespace {
+constexpr int XI_NOALLOC_MAX_DEVICES = 64;
+double *g_xi_noalloc_ptr[XI_NOALLOC_MAX_DEVICES];      // device address of g_xi_noalloc_acc, per device ordinal (0 = not asked yet)
+}  // namespace
+
+extern "C" lya_status lya_xi2pcf_plan_noalloc(lya_ctx *ctx, const lya_plan *pl,
+                                              double *S, double *W, uint64_t *N, double *xi, lya_stats *stats)
+{
+    if (!ctx) return LYA_ERR_INVALID_ARG;
+    if (!pl) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_plan_noalloc: plan is NULL");
+    if (!pl->has_xi) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_plan_noalloc: the plan was created without want_xi");
+    if (!S || !W || !N || !xi) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "lya_xi2pcf_plan_noalloc: S, W, N and xi are all required");
+    const lya_forests *f = &pl->f;
+    const int nb = pl->b.n_par * pl->b.n_perp;
+    if (nb > LYA_XI_NOALLOC_MAX_BINS)
+        return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_xi2pcf_plan_noalloc: %d bins, the static accumulators hold at most %d "
+                        "(use lya_xi2pcf_plan)", nb, LYA_XI_NOALLOC_MAX_BINS);
+    if (ctx->device < 0 || ctx->device >= XI_NOALLOC_MAX_DEVICES)
+        return lya_fail(ctx, LYA_ERR_CAPACITY, "lya_xi2pcf_plan_noalloc: device ordinal %d outside [0, %d)", ctx->device, XI_NOALLOC_MAX_DEVICES);
+    LYA_CUDA(lya_enter(ctx));                                      // makes ctx->device current
+    if (!g_xi_noalloc_ptr[ctx->device]) {                          // set-up, once per device
+        double *ptr = NULL;
+        cudaError_t ge = cudaGetSymbolAddress((void **)&ptr, g_xi_noalloc_acc);
+        if (ge != cudaSuccess || !ptr) return lya_cuda_fail(ctx, ge, "cudaGetSymbolAddress(g_xi_noalloc_acc)");
+        g_xi_noalloc_ptr[ctx->device] = ptr;
+    }
+    double *acc = g_xi_noalloc_ptr[ctx->device];
+    cudaStream_t s = ctx->stream;
+    const BinParams bp = pl->bp;
+    const bool use_fast = pl->use_fast;
+    const LyaBuckets &bk = pl->bk;
+    cudaEventRecord(ctx->ev[3], s);
+    cudaError_t e = cudaMemsetAsync(acc, 0, (size_t)nb * 24, s);   // the array keeps the last call's sums
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "lya_xi2pcf_plan_noalloc: clearing the accumulators");
+
+    XiParams P;
+    P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.delta = f->delta;
+    P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
+    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pl->pq;
+    P.n_pairs = use_fast ? bk.n_fast2 + bk.n_long + bk.n_generic : pl->n_pairs;
+    P.n_forest = f->n_forest;
+    P.bp = bp;
+    P.S = acc; P.W = acc + nb; P.N = (unsigned long long *)(acc + 2 * nb);
+    P.counters = ctx->d_counters;
+
+    cudaEventRecord(ctx->ev[0], s);
+    if (use_fast && bk.n_fast > 0) {
+        XiFastParams F;
+        F.prep = pl->prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
+        F.S = P.S; F.W = P.W; F.N = P.N; F.counters = ctx->d_counters;
+        F.region = NULL; F.n_region = 1;
+        F.merge_every = ctx->xi_merge_every;
+        const size_t fsmem = sizeof(FastWarp) * FW;
+        const int fgrid = ctx->sm_count;
+        auto launch = [&](auto kern) {
+            cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
+            if (le == cudaSuccess) { kern<<<fgrid, FTHREADS, fsmem, s>>>(F); lya_note_launch(); }
+            return le;
+        };
+        if (ctx->check_holders) e = bp.pow2 ? launch(k_xi_fast<true, true>) : launch(k_xi_fast<false, true>);
+        else e = bp.pow2 ? launch(k_xi_fast<true, false>) : launch(k_xi_fast<false, false>);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "k_xi_fast launch");
+    }
+    const size_t smem = (((size_t)nb * 20 + 15) & ~(size_t)15) + sizeof(WarpSmem) * XI_WARPS;
+    const int grid = ctx->sm_count * 2;
+    const int64_t n_chunks = (P.n_pairs + CHUNK - 1) / CHUNK;
+    int launches = 0;
+    unsigned long long h[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    while (P.n_pairs > 0) {                                        // generic kernel for the rest of the list
+        switch (ctx->generic_diagonals) {
+        case 1: e = launch_xi<1>(P, grid, smem, s); break;
+        case 4: e = launch_xi<4>(P, grid, smem, s); break;
+        default: e = launch_xi<2>(P, grid, smem, s); break;
+        }
+        if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "k_xi launch");
+        ++launches;
+        e = cudaMemcpyAsync(h, ctx->d_counters, 4 * sizeof(h[0]), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "k_xi");
+        if ((int64_t)h[0] >= n_chunks) break;                      // every chunk claimed (warps stop at their u32 budget)
+        if (launches > 100000) return lya_fail(ctx, LYA_ERR_CUDA, "k_xi made no progress");
+    }
+    cudaEventRecord(ctx->ev[1], s);
+    { k_xi_finalize<<<(unsigned)((nb + 255) / 256), 256, 0, s>>>(P.S, P.W, P.N, nb, S, W, (unsigned long long *)N, xi); lya_note_launch(); }
+    cudaEventRecord(ctx->ev[2], s);
+    e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return lya_cuda_fail(ctx, e, "lya_xi2pcf_plan_noalloc");
+    if (h[3] != 0) return lya_fail(ctx, LYA_ERR_INVALID_ARG, "pair list refers to a forest outside [0, n_forest)");
+    if (h[5] != 0) return lya_fail(ctx, LYA_ERR_CUDA, "k_xi_fast: %llu sub-histogram entries had two holders (LYA_OPT_CHECK_HOLDERS)", h[5]);
+    if (stats) {
+        memset(stats, 0, sizeof(*stats));
+        stats->n_forest_pairs = (uint64_t)pl->n_pairs;
+        stats->n_visited = use_fast ? pl->visited : h[1];
+        stats->n_evaluated = h[2];
+        unsigned long long hN[LYA_XI_NOALLOC_MAX_BINS];            // n_binned = sum N (host stack, no allocation)
+        if (cudaMemcpy(hN, P.N, sizeof(unsigned long long) * (size_t)nb, cudaMemcpyDeviceToHost) == cudaSuccess)
+            for (int k = 0; k < nb; ++k) stats->n_binned += hN[k];
+        cudaEventElapsedTime(&stats->ms_main, ctx->ev[0], ctx->ev[1]);
+        cudaEventElapsedTime(&stats->ms_total, ctx->ev[3], ctx->ev[2]);
+    }
+    return LYA_OK;
+}
