@@ -93,7 +93,7 @@ def micro_peaks(device=0):
     lib = C.CDLL(build.build_peaks())
     lib.lya_measure_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
     out = {}
-    for kind, name in enumerate(("fp64_fma", "fp64_add", "smem_cas64", "smem_add32", "l2_red64")):
+    for kind, name in enumerate(("fp64_fma", "fp64_add", "smem_cas64", "smem_add32", "l2_red64", "l2_red64_scatter")):
         r = C.c_double()
         rc = lib.lya_measure_peak(device, kind, C.byref(r))
         out[name] = r.value if rc == 0 else None
@@ -208,6 +208,45 @@ def cpu_baseline(wl, n_forests, dmat_div):
             "sample": smp.describe() + f" (xi {t_xi:.1f} s, D {t_d:.1f} s; single-thread xi on 1/16 of the forest pairs)"}
 
 
+def run_xi3(args):
+    """--xi3 RMAX: throughput of lya_xi3pcf (NEXT-4, eq. 2.8) on the workload's catalogue; its own JSON line, never
+    the default bench line.  Triangle bins of PAPER.md:225 (20 x 20 x 20 x 10 x 10); pair list = lya_neighbours with
+    r_perp_max = r_max; warm-up calls, then `steps` timed calls (CUDA events of the k_xi3 launch, stats.ms_main)."""
+    import torch
+    from paper_2507_00129_b200 import binding as B, build, gen
+    build.build()
+    wl = WORKLOADS[args.workload]
+    f = gen.make_config(wl["cfg"], n_forest=args.forests or None, fine=args.fine)
+    ctx = B.Context("cuda:0")
+    d = B.DeviceForests(f, device="cuda:0")
+    tb = B.tri_binning(args.xi3, 20, 10, 20)
+    ce = np.cos(np.pi * np.arange(1, 10) / 10)
+    pairs = ctx.lya_neighbours(d, B.binning(args.xi3, args.xi3, 20, 20))
+    for _ in range(max(args.warmup, 1)):
+        g = ctx.lya_xi3pcf(d, tb, ce, pairs)
+    ms = []
+    for _ in range(args.steps):
+        g = ctx.lya_xi3pcf(d, tb, ce, pairs)
+        ms.append(g["stats"]["ms_main"])
+    st = g["stats"]
+    t = float(np.mean(ms)) * 1e-3
+    mp = micro_peaks(0)
+    print(json.dumps({
+        "metric": "ordered triples (i; j, k) binned per second by lya_xi3pcf", "value": st["n_binned"] / t, "unit": "triples/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 1), "ms_per_step": t * 1e3, "higher_is_better": True,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "n_forest": f.n_forest, "n_pix": f.n_pix, "r_max": args.xi3,
+                   "bins": "20x20x20x10x10", "forest_pairs": st["n_forest_pairs"], "triples": st["n_binned"],
+                   "bins_touched": int((g["N3"] > 0).sum().item())},
+        "roofline": {"bound": "l2-atomics", "kernel": "k_xi3", "achieved": 1.5 * st["n_binned"] / t / 1e9,
+                     "peak": (mp.get("l2_red64_scatter") or 0) / 1e9 or None, "unit": "G red.global 8-byte/s",
+                     "frac": (1.5 * st["n_binned"] / t / mp["l2_red64_scatter"]) if mp.get("l2_red64_scatter") else None,
+                     "note": "1.5 reductions per ordered triple (S3, W3, N3 once per unordered {j, k}), scattered over "
+                             "the 19 MB accumulators; peak = liblya_peaks' red.global.add.f64 rate with every lane on "
+                             "its own random element of a 19 MB array"},
+        "measured_peaks": mp}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -229,9 +268,13 @@ def main():
                     help="route every forest pair to the generic kernels (lya_set_option force_generic): the comparison figure for the fast / long-forest kernels")
     ap.add_argument("--fine", type=int, default=1,
                     help="NEXT-3 shapes: divide the pixel step by this factor (gen.make_config(fine=...)); throughput only")
+    ap.add_argument("--xi3", type=float, default=0.0, metavar="RMAX",
+                    help="NEXT-4: time lya_xi3pcf with this r_max (Mpc/h) on the workload's catalogue instead of the 2PCF step")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.xi3 > 0:
+        return run_xi3(args)
 
     import torch
     import torch.distributed as dist

@@ -17,10 +17,12 @@ extern "C" {
  *                         random bins of a 2500-entry histogram
  *   LYA_PEAK_SMEM_ADD32   lane-level native shared-memory u32 atomic adds per second
  *   LYA_PEAK_L2_RED64     lane-level red.global.add.f64 per second into an L2-resident
- *                         2500 x 2500 double matrix (random row, contiguous segment) */
+ *                         2500 x 2500 double matrix (random row, contiguous segment)
+ *   LYA_PEAK_L2_RED64_SCATTER  the same with every lane on its own random element of a 19 MB
+ *                         array (the triangle-bin accumulators of lya_xi3pcf) */
 typedef enum {
     LYA_PEAK_FP64_FMA = 0, LYA_PEAK_FP64_ADD = 1, LYA_PEAK_SMEM_CAS64 = 2,
-    LYA_PEAK_SMEM_ADD32 = 3, LYA_PEAK_L2_RED64 = 4
+    LYA_PEAK_SMEM_ADD32 = 3, LYA_PEAK_L2_RED64 = 4, LYA_PEAK_L2_RED64_SCATTER = 5
 } lya_peak_kind;
 int lya_measure_peak(int device, lya_peak_kind kind, double *rate);
 

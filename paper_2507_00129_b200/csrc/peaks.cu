@@ -60,6 +60,16 @@ __global__ void k_peak_red(double *mat, int nb, int iters)
     }
 }
 
+// every lane its own random element of an n-element array (the access pattern of k_xi3: 32 sectors per instruction)
+__global__ void k_peak_red_scatter(double *mat, unsigned n, int iters)
+{
+    unsigned x = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 4242u;
+    for (int i = 0; i < iters; ++i) {
+        x = x * 1664525u + 1013904223u;
+        atomicAdd(&mat[(unsigned)(((unsigned long long)x * n) >> 32)], 1.0);
+    }
+}
+
 }  // namespace
 
 extern "C" int lya_measure_peak(int device, lya_peak_kind kind, double *rate)
@@ -107,6 +117,11 @@ extern "C" int lya_measure_peak(int device, lya_peak_kind kind, double *rate)
         case LYA_PEAK_L2_RED64: {
             int iters = 1 << 10;
             k_peak_red<<<grid, PK_THREADS, 0, s>>>(buf, nb, iters);
+            ops = (double)grid * PK_THREADS * iters;
+            break; }
+        case LYA_PEAK_L2_RED64_SCATTER: {
+            int iters = 1 << 10;
+            k_peak_red_scatter<<<grid, PK_THREADS, 0, s>>>(buf, 2400000u, iters);      // 19 MB: three 800,000-bin accumulators
             ops = (double)grid * PK_THREADS * iters;
             break; }
         default:

@@ -16,16 +16,17 @@
 // pairs with two pixels closer than r_max, e.g. lya_neighbours with rperp_max = r_max: r_perp <= the 3-D
 // separation) is turned into an adjacency list in both directions.  One CTA per main-vertex forest p; for each
 // of its pixels i the CTA gathers the pixels of p's neighbours that lie inside the sphere of radius r_max
-// (side vector, length, bins, weights) into shared memory, then its threads take one side-1 pixel j each and
-// run over all side-2 pixels k (broadcast reads), with three reductions per triple into the L2-resident
-// accumulators (20 x 20 x 20 x 10 x 10 bins x 24 B = 19 MB).
+// (side vector, length, bins, weights) into shared memory, then its threads run over the UNORDERED pairs {j, k} of
+// that list (the two orders of the sides share cos alpha bit for bit and land in mirrored bins: the second order
+// is added by k_xi3_finalize), with three reductions per unordered pair into the L2-resident accumulators
+// (20 x 20 x 20 x 10 x 10 bins x 24 B = 19 MB).
 #include <math.h>
 #include <stdlib.h>
 #include "lya_internal.cuh"
 
 namespace {
 
-constexpr int T3_THREADS = 256;
+constexpr int T3_THREADS = 512;
 constexpr int T3_CAP = 2048;                 // pixels inside the sphere of one main-vertex pixel (shared-memory list)
 
 struct Tri3Params {
@@ -35,7 +36,7 @@ struct Tri3Params {
     const double *cosedge;                   // [n_theta - 1]
     const unsigned long long *adj_off;       // [n_forest + 1]
     const int32_t *adj;                      // neighbours of every forest (both directions)
-    double *S3, *W3;
+    double *S3, *W3;                         // HALF accumulators: one entry per unordered {j, k} (see k_xi3)
     unsigned long long *N3;
     unsigned long long *counters;            // [0] triples binned, [3] error (capacity)
 };
@@ -60,12 +61,16 @@ __global__ void k_adj_fill(const int32_t *pq, int64_t n, int64_t n_forest, const
 }
 
 struct Tri3Smem {
-    double dx[T3_CAP], dy[T3_CAP], dz[T3_CAP], r[T3_CAP], a[T3_CAP], w[T3_CAP];
-    int bins[T3_CAP];                        // b_r | b_theta << 8
-    int fid[T3_CAP];
+    double2 xy[T3_CAP], zr[T3_CAP], aw[T3_CAP];   // side vector (dx, dy), (dz, r), (a = w delta, w): three 16-byte reads per pixel
+    int2 bf[T3_CAP];                              // (b_r | b_theta << 8, forest)
     unsigned n;
 };
 
+// The two orders (i; j, k) and (i; k, j) of a triple share every rounded operation of cos alpha (products and
+// r1 r2 commute, the additions keep their order), so they fall in the bins A(b_r1, b_r2, b_a, b_t1, b_t2) and
+// swap(A) = A(b_r2, b_r1, b_a, b_t2, b_t1) with the same weights up to the rounding order of T7.  The kernel therefore
+// walks every UNORDERED {j, k} once and adds it to A only; k_xi3_finalize returns acc[A] + acc[swap(A)] (half the
+// geometry, half the reductions; the counts stay exact, S3 and W3 move by an ulp per term).
 __global__ void __launch_bounds__(T3_THREADS) k_xi3(Tri3Params P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -84,7 +89,9 @@ __global__ void __launch_bounds__(T3_THREADS) k_xi3(Tri3Params P)
         __syncthreads();
         if (threadIdx.x == 0) sm.n = 0u;
         __syncthreads();
-        // ---- gather: warps over the neighbour forests, lanes over their pixels (T3, T4, T5 per side) ----
+        // ---- gather: warps over the neighbour forests, lanes over their pixels (T3, T4, T5 per side).  A pixel
+        //      with |chi_j - chi_i| beyond r_max (plus a margin for |u| = 1 +- 1e-9) cannot be inside the sphere ----
+        const double guard = P.r_max * (1.0 + 1e-6) + 1e-6;
         for (unsigned long long e = a0 + wid; e < a1; e += n_warps) {
             const int q = P.adj[e];
             const int64_t oq = P.f.pix_off[q];
@@ -92,6 +99,7 @@ __global__ void __launch_bounds__(T3_THREADS) k_xi3(Tri3Params P)
             const double qx = P.f.ux[q], qy = P.f.uy[q], qz = P.f.uz[q];
             for (int j = lane; j < nq; j += 32) {
                 const double cj = P.f.chi[oq + j];
+                if (fabs(cj - ci) > guard + 4e-9 * (cj + ci)) continue;
                 const double d0 = __dsub_rn(__dmul_rn(cj, qx), xi0), d1 = __dsub_rn(__dmul_rn(cj, qy), xi1), d2 = __dsub_rn(__dmul_rn(cj, qz), xi2);
                 const double r = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(d0, d0), __dmul_rn(d1, d1)), __dmul_rn(d2, d2)));
                 if (r > 0.0 && r < P.r_max) {
@@ -103,54 +111,70 @@ __global__ void __launch_bounds__(T3_THREADS) k_xi3(Tri3Params P)
                     const unsigned s = atomicAdd(&sm.n, 1u);
                     if (s < (unsigned)T3_CAP) {
                         const double wj = P.f.w[oq + j];
-                        sm.dx[s] = d0; sm.dy[s] = d1; sm.dz[s] = d2; sm.r[s] = r;
-                        sm.w[s] = wj; sm.a[s] = wj * P.f.delta[oq + j];
-                        sm.bins[s] = br | (bt << 8); sm.fid[s] = q;
+                        sm.xy[s] = make_double2(d0, d1); sm.zr[s] = make_double2(d2, r);
+                        sm.aw[s] = make_double2(wj * P.f.delta[oq + j], wj);
+                        sm.bf[s] = make_int2(br | (bt << 8), q);
                     }
                 }
             }
         }
         __syncthreads();
         const unsigned C = sm.n;
-        if (C > (unsigned)T3_CAP) {                            // (warp-uniform) more pixels in the sphere than the list holds
+        if (C > (unsigned)T3_CAP) {                            // (CTA-uniform) more pixels in the sphere than the list holds
             if (threadIdx.x == 0) atomicMax(&P.counters[3], (unsigned long long)LYA_DEV_TOO_LONG);
             return;
         }
-        // ---- ordered pairs (j, k) of gathered pixels from two different forests (T2, T4-T7) ----
-        for (unsigned j = threadIdx.x; j < C; j += T3_THREADS) {
-            const double x1 = sm.dx[j], y1 = sm.dy[j], z1 = sm.dz[j], r1 = sm.r[j];
-            const double aij = ai * sm.a[j], wij = wi * sm.w[j];
-            const int b1 = sm.bins[j], f1 = sm.fid[j];
-            const int br1 = b1 & 0xff, bt1 = b1 >> 8;
-            for (unsigned k = 0; k < C; ++k) {
-                if (sm.fid[k] == f1) continue;
-                const double dot = __dadd_rn(__dadd_rn(__dmul_rn(x1, sm.dx[k]), __dmul_rn(y1, sm.dy[k])), __dmul_rn(z1, sm.dz[k]));
-                const double ca = __ddiv_rn(dot, __dmul_rn(r1, sm.r[k]));
+        if (C < 2u) continue;
+        // ---- unordered pairs {j, k} of gathered pixels from two different forests (T2, T4-T7): k = j + d (mod C)
+        //      for the offsets d = 1 .. (C - 1) / 2 and every j, plus d = C / 2 for j < C / 2 when C is even; the
+        //      threads run over the flat index d * C + j, so a warp reads neighbouring list entries ----
+        const unsigned half = (C - 1u) >> 1;
+        const unsigned total = C * half + ((C & 1u) ? 0u : (C >> 1));
+        const unsigned qd = (unsigned)T3_THREADS / C, rd = (unsigned)T3_THREADS % C;
+        unsigned d = 1u + threadIdx.x / C, j = threadIdx.x % C;
+        for (unsigned t = threadIdx.x; t < total; t += T3_THREADS) {
+            unsigned k = j + d;
+            if (k >= C) k -= C;
+            const int2 bj = sm.bf[j], bk = sm.bf[k];
+            if (bj.y != bk.y) {
+                const double2 xy1 = sm.xy[j], zr1 = sm.zr[j], aw1 = sm.aw[j];
+                const double2 xy2 = sm.xy[k], zr2 = sm.zr[k], aw2 = sm.aw[k];
+                const double dot = __dadd_rn(__dadd_rn(__dmul_rn(xy1.x, xy2.x), __dmul_rn(xy1.y, xy2.y)), __dmul_rn(zr1.x, zr2.x));
+                const double ca = __ddiv_rn(dot, __dmul_rn(zr1.y, zr2.y));
                 int ba = __double2int_rz(__dmul_rn(__dadd_rn(ca, 1.0), P.nhalf));
                 ba = max(0, min(ba, P.n_cosa - 1));
-                const int b2 = sm.bins[k];
-                const unsigned A = (unsigned)((((br1 * P.n_r + (b2 & 0xff)) * P.n_cosa + ba) * P.n_theta + bt1) * P.n_theta + (b2 >> 8));
-                atomicAdd(&P.S3[A], aij * sm.a[k]);
-                atomicAdd(&P.W3[A], wij * sm.w[k]);
+                const unsigned A = (unsigned)(((((bj.x & 0xff) * P.n_r + (bk.x & 0xff)) * P.n_cosa + ba) * P.n_theta + (bj.x >> 8)) * P.n_theta + (bk.x >> 8));
+                atomicAdd(&P.S3[A], (ai * aw1.x) * aw2.x);     // (three RED.E.ADD: the kernel runs at the rate at which L2 takes
+                atomicAdd(&P.W3[A], (wi * aw1.y) * aw2.y);     //  scattered 8-byte reductions, 2.0e11 / s -- profiles/r2l_xi3pcf.md)
                 atomicAdd(&P.N3[A], 1ull);
-                ++n_tri;
+                n_tri += 2;
             }
+            j += rd; d += qd;
+            if (j >= C) { j -= C; ++d; }
         }
     }
-    // triples counted by this CTA
+    // ordered triples counted by this CTA
     for (int o = 16; o > 0; o >>= 1) n_tri += __shfl_xor_sync(0xffffffffu, n_tri, o);
     if (lane == 0 && n_tri) atomicAdd(&P.counters[0], n_tri);
 }
 
-__global__ void k_xi3_finalize(const double *S, const double *W, const unsigned long long *N, int64_t nb,
+// result[A] = acc[A] + acc[swap(A)] (both orders of the two sides, see k_xi3), xi3 = S3 / W3
+__global__ void k_xi3_finalize(const double *S, const double *W, const unsigned long long *N, int64_t nb, int n_r, int n_cosa, int n_theta,
                                double *S_out, double *W_out, unsigned long long *N_out, double *xi_out)
 {
     const int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (k >= nb) return;
-    const double s = S[k], w = W[k];
+    int64_t v = k;
+    const int t2 = (int)(v % n_theta); v /= n_theta;
+    const int t1 = (int)(v % n_theta); v /= n_theta;
+    const int ba = (int)(v % n_cosa); v /= n_cosa;
+    const int b2 = (int)(v % n_r), b1 = (int)(v / n_r);
+    const int64_t ks = ((((int64_t)b2 * n_r + b1) * n_cosa + ba) * n_theta + t2) * n_theta + t1;
+    const double s = S[k] + S[ks], w = W[k] + W[ks];
+    const unsigned long long n = N[k] + N[ks];
     if (S_out) S_out[k] = s;
     if (W_out) W_out[k] = w;
-    if (N_out) N_out[k] = N[k];
+    if (N_out) N_out[k] = n;
     if (xi_out) xi_out[k] = (w != 0.0) ? s / w : 0.0;
 }
 
@@ -220,7 +244,7 @@ extern "C" lya_status lya_xi3pcf(lya_ctx *ctx, const lya_forests *f, const lya_t
         cudaEventRecord(ctx->ev[0], s);
         cudaEventRecord(ctx->ev[1], s);
     }
-    { k_xi3_finalize<<<(unsigned)((nb + 255) / 256), 256, 0, s>>>(acc, acc + nb, (unsigned long long *)(acc + 2 * nb), nb, S3, W3, (unsigned long long *)N3, xi3); lya_note_launch(); }
+    { k_xi3_finalize<<<(unsigned)((nb + 255) / 256), 256, 0, s>>>(acc, acc + nb, (unsigned long long *)(acc + 2 * nb), nb, tb->n_r, tb->n_cosa, tb->n_theta, S3, W3, (unsigned long long *)N3, xi3); lya_note_launch(); }
     cudaEventRecord(ctx->ev[2], s);
     e = cudaMemcpyAsync(h, ctx->d_counters, sizeof(h), cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
