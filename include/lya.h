@@ -229,7 +229,9 @@ lya_status lya_dmat(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
  *   A = (((b_r1 n_r + b_r2) n_cosa + b_alpha) n_theta + b_theta1) n_theta + b_theta2   (lya_tri_nbins entries).
  * pairs: any list holding every pair of forests with two pixels closer than r_max -- lya_neighbours with
  * rperp_max = r_max is one (r_perp never exceeds the 3-D separation).  S3, W3, xi3: device double [n_bins]; N3:
- * device uint64 [n_bins] (ordered triples per bin); any may be NULL.  stats: n_binned = triples counted.
+ * device uint64 [n_bins] (ordered triples per bin); any may be NULL.  stats: n_binned = ordered triples counted.
+ * (The kernel visits each unordered pair of sides once and returns acc[A] + acc[A with the two sides swapped]:
+ * cos alpha is bit-identical for both orders, so the counts are exact and S3, W3 move by an ulp per term.)
  * Limits (LYA_ERR_CAPACITY): at most 255 bins per variable and 2^24 bins in all; at most 2048 pixels of other
  * forests inside the sphere of radius r_max around one pixel.  Synchronises the ctx stream. */
 typedef struct { double r_max; int32_t n_r, n_theta, n_cosa; } lya_tri_binning;   /* 80, 20, 10, 20 */
