@@ -458,7 +458,9 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             const int key = lya_pair_key<POW2>(bp, g, hp, hq, c0);
             if (key >= 2 * bp.n_perp) continue;              // cannot happen in the fast ranges
             const unsigned lim = (unsigned)min(LYA_NCOL, bp.n_perp - c0);
-            const int ds = lya_pair_stride(bp, g, hq);              // lanes of a row step sit ds pixels of q apart
+            // lanes of a row step sit ds pixels of q apart; the class-0 range of the bucketed list holds only forest pairs
+            // with ds == 1 (lya_pair_key), and a compile-time 1 folds the divisions by the stride out of the walk set-up
+            const int ds = (CLS == 0) ? 1 : lya_pair_stride(bp, g, hq);
             __syncwarp();
             // ---- stage p (when it changes) and q: (chi, ea) pairs with 16-byte loads, eg, q's stage-4 keys ----
             if (p != cur_p) {
