@@ -321,19 +321,34 @@ __device__ __forceinline__ void dm_drain_t123(DmFastWarp<CLS> &ws, unsigned *kep
         const double ci = ws.pce[i].x, cj = qce[j].x;
         const unsigned row = (rec >> 16) * nb;
         const int jh = ws.jhi[i];
-#pragma unroll 1
-        for (int j2 = ws.jlo[i] + lane; j2 < jh; j2 += 32) {                      // T2
-            const double2 q2 = qce[j2];
-            dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, ci, q2.x)), fma(m1, qeg[j2], m0 * q2.y));
-            n_red += 1u;
-        }
-#pragma unroll 1
-        for (int i2 = lane; i2 < mp; i2 += 32) {                                  // T3
-            const unsigned lo2 = ws.jlo[i2];
-            if ((unsigned)j - lo2 < (unsigned)ws.jhi[i2] - lo2) {
-                const double2 p2 = ws.pce[i2];
-                dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, p2.x, cj)), fma(m2, ws.peg[i2], m0 * p2.y));
-                n_red += 1u;
+        // T2 and T3 with the 32-wide blocks of the row window / of the rows unrolled: the window tests of every block
+        // are issued before the first body, and there is no loop bookkeeping
+        {
+            const int j20 = ws.jlo[i] + lane;
+            bool in3[FD_RPL];
+#pragma unroll
+            for (int k = 0; k < FD_RPL; ++k) {
+                const int i2 = lane + 32 * k;
+                in3[k] = false;
+                if (i2 < mp) { const unsigned lo2 = ws.jlo[i2]; in3[k] = (unsigned)j - lo2 < (unsigned)ws.jhi[i2] - lo2; }
+            }
+#pragma unroll
+            for (int k = 0; k < FD_RPL; ++k) {                                       // T2
+                const int j2 = j20 + 32 * k;
+                if (j2 < jh) {
+                    const double2 q2 = qce[j2];
+                    dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, ci, q2.x)), fma(m1, qeg[j2], m0 * q2.y));
+                    n_red += 1u;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < FD_RPL; ++k) {                                       // T3
+                const int i2 = lane + 32 * k;
+                if (in3[k]) {
+                    const double2 p2 = ws.pce[i2];
+                    dm_red(Dn + (row + (unsigned)dm_bin_in<POW2>(bp, g, p2.x, cj)), fma(m2, ws.peg[i2], m0 * p2.y));
+                    n_red += 1u;
+                }
             }
         }
     }
@@ -498,7 +513,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 const int i = ib + lane;
                 if (i < mp) {
                     int jlo, jx, jhi;
-                    lya_row_window<POW2>(bp, g, qce, mq, ws.pce[i].x, R, Tchi, jlo, jx, jhi);
+                    lya_row_window_ilp<POW2, (FD_T < 128 ? 64 : 128)>(bp, g, qce, mq, ws.pce[i].x, R, Tchi, jlo, jx, jhi);
                     ws.jlo[i] = (unsigned char)jlo; ws.jx[i] = (unsigned char)jx; ws.jhi[i] = (unsigned char)jhi;
                     binned += (unsigned)(jhi - jlo);
                 }
@@ -541,13 +556,17 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
                 int jend = (row >= mp) ? (1 << 30) : (int)ws.jhi[row];
                 unsigned long long pki = ws.u.a.pk[min(row, FD_T - 1)];
                 const unsigned n_it = __reduce_max_sync(0xffffffffu, last - first);
+                unsigned long long qv = ws.u.a.qk[min(j, FD_T - 1)];
                 for (unsigned t = 0; t < n_it; ++t) {
                     if (j >= jend) {                             // next non-empty row (the stop row ends the search)
                         do { ++row; } while (ws.jlo[row] == ws.jhi[row]);
                         j = ws.jlo[row]; jend = (row >= mp) ? (1 << 30) : (int)ws.jhi[row];
                         pki = ws.u.a.pk[min(row, FD_T - 1)];
+                        qv = ws.u.a.qk[min(j, FD_T - 1)];
                     }
-                    const unsigned h = lya_pair_hash32(pki, ws.u.a.qk[min(j, FD_T - 1)]);
+                    const unsigned long long qn = ws.u.a.qk[min(j + 1, FD_T - 1)];      // the row's next pixel, ahead of its use
+                    const unsigned h = lya_pair_hash32(pki, qv);
+                    qv = qn;
                     if ((first + t < last) & (h >= thr32)) {
                         const unsigned idx = atomicAdd(&ws.nkept, 1u);
                         if (idx < FD_KCAP) ws.kept[idx] = ((unsigned)row << 8) | (unsigned)j;
@@ -603,10 +622,7 @@ __global__ void __launch_bounds__(FD_THREADS, 1) k_dmat_fast(DmFastParams P)
             for (int t0 = 0; t0 < n_slots; t0 += 32) {
                 const int t = t0 + lane;
                 bool nzf = false;
-                if (t < n_slots) {
-                    const double2 a = tb.H01[t], b = tb.H23[t];
-                    nzf = (a.x != 0.0) | (a.y != 0.0) | (b.x != 0.0) | (b.y != 0.0);
-                }
+                if (t < n_slots) nzf = tb.H01[t].x != 0.0;     // H_aa: a sum of products of non-negative ea, zero only where the other three are
                 const unsigned bal = __ballot_sync(0xffffffffu, nzf);
                 if (nzf) ws.u.b.nz[nnz + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)t;
                 nnz += __popc(bal);

@@ -98,3 +98,25 @@ __device__ __forceinline__ void lya_row_window(const BinParams &bp, const PairBi
     while (lo < hi) { const int mid = (lo + hi) >> 1; if (qce[mid].x > x) hi = mid; else lo = mid + 1; }
     jx = lo;
 }
+
+// The same window with the three searches as ONE branch-free loop of fixed trip count (three independent
+// dependency chains in flight instead of three data-dependent loops one after the other).  STEP0: a power of two
+// with 2 * STEP0 > the longest q; qce[mq] must be a sentinel (chi far above every real pixel).
+template <bool POW2, int STEP0>
+__device__ __forceinline__ void lya_row_window_ilp(const BinParams &bp, const PairBin &g, const double2 *qce, int mq,
+                                                   double x, double R, double Tchi, int &jlo, int &jx, int &jhi)
+{
+    const double ta = x - R, tb = fmin(x + R, Tchi - x);
+    int a = 0, b = 0, c = 0;                     // first j with chi_j > ta / chi_j >= tb / chi_j > x
+#pragma unroll
+    for (int s = STEP0; s > 0; s >>= 1) {
+        const double va = qce[min(a + s - 1, mq)].x, vb = qce[min(b + s - 1, mq)].x, vc = qce[min(c + s - 1, mq)].x;
+        a += (va > ta) ? 0 : s;
+        b += (vb >= tb) ? 0 : s;
+        c += (vc > x) ? 0 : s;
+    }
+    jlo = a; jhi = max(b, a);
+    while (jlo < jhi && !lya_in_grid<POW2>(bp, g, x, qce[jlo].x)) ++jlo;
+    while (jhi > jlo && !lya_in_grid<POW2>(bp, g, x, qce[jhi - 1].x)) --jhi;
+    jx = min(max(c, jlo), jhi);
+}
