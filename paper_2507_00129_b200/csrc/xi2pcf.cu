@@ -421,6 +421,10 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
                                     (src < lane || (src == lane && k2 < k))) conflicts += 1u;
                         }
                 }
+                // row i + 1's new q pixel and p pixel are read BEFORE the hand-over (they do not depend on it; the
+                // volatile accesses below would otherwise pin these loads behind them)
+                const unsigned jn = min((unsigned)(i + dl + D + FPAD), (unsigned)(mq + 2 * FPAD - 1));
+                const double qcn = ws.qc[jn], qan = ws.qa[jn], qwn = ws.qw[jn], pcn = ws.pc[i + 1];
 #pragma unroll
                 for (int k = 0; k < D; ++k) {
                     ch[k] = key[k] != cur[k];
@@ -439,9 +443,8 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
                 unsigned key_n[D];
                 {
                     // (one unsigned min clamps both ends: a negative index wraps to the right-hand sentinel)
-                    const unsigned j = min((unsigned)(i + dl + D + FPAD), (unsigned)(mq + 2 * FPAD - 1));
-                    wc[u] = ws.qc[j]; wa[u] = ws.qa[j]; ww[u] = ws.qw[j];
-                    const double pci = ws.pc[i + 1];
+                    wc[u] = qcn; wa[u] = qan; ww[u] = qwn;
+                    const double pci = pcn;
 #pragma unroll
                     for (int k = 0; k < D; ++k) {
                         const int sl = (k + u + 1) % D;
@@ -584,16 +587,23 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
             // per row of p: the window of q with r_par < rpar_max and r_perp < rperp_max (conservative superset)
             const double R = (c > 0.0) ? (bp.rpar_max / c) * (1.0 + 1e-12) + 1e-9 : 1e300;
             const double Tchi = (s > 0.0) ? (bp.rperp_max / s) * (1.0 + 1e-12) + 1e-9 : 1e300;
-            for (int i = lane; i < mp; i += 32) {
-                const double x = ws.pc[i];
-                int lo = 0, hi = mq;                         // first j with qc[j] > x - R
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] > x - R) hi = mid; else lo = mid + 1; }
-                const int jlo = lo;
-                const double top = fmin(x + R, Tchi - x);    // first j with qc[j] >= top
-                hi = mq;
-                while (lo < hi) { const int mid = (lo + hi) >> 1; if (qc[mid] >= top) hi = mid; else lo = mid + 1; }
-                ws.jlo[i] = (unsigned char)jlo;
-                ws.jhi[i] = (unsigned char)lo;
+            // (branch-free lower bounds of fixed trip count, two rows per lane: four independent chains in flight
+            //  instead of two data-dependent loops one after the other; qc[mq] is a sentinel, so a probe past the
+            //  end reads "true" and the position never exceeds mq)
+            for (int ib = 0; ib < mp; ib += 64) {
+                const int i0 = ib + lane, i1 = i0 + 32;
+                const double x0 = ws.pc[min(i0, FTP - 1)], x1 = ws.pc[min(i1, FTP - 1)];
+                const double ta0 = x0 - R, ta1 = x1 - R, tb0 = fmin(x0 + R, Tchi - x0), tb1 = fmin(x1 + R, Tchi - x1);
+                int a0 = 0, b0 = 0, a1 = 0, b1 = 0;          // first j with qc[j] > ta / qc[j] >= tb
+#pragma unroll
+                for (int st = 64; st > 0; st >>= 1) {
+                    const double va0 = qc[min(a0 + st - 1, mq)], vb0 = qc[min(b0 + st - 1, mq)];
+                    const double va1 = qc[min(a1 + st - 1, mq)], vb1 = qc[min(b1 + st - 1, mq)];
+                    a0 += (va0 > ta0) ? 0 : st; b0 += (vb0 >= tb0) ? 0 : st;
+                    a1 += (va1 > ta1) ? 0 : st; b1 += (vb1 >= tb1) ? 0 : st;
+                }
+                if (i0 < mp) { ws.jlo[i0] = (unsigned char)a0; ws.jhi[i0] = (unsigned char)max(a0, b0); }
+                if (i1 < mp) { ws.jlo[i1] = (unsigned char)a1; ws.jhi[i1] = (unsigned char)max(a1, b1); }
             }
             __syncwarp();
             // walk FROWS rows at a time over exactly the diagonals those rows need
