@@ -540,8 +540,18 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
         chunk = __shfl_sync(0xffffffffu, chunk, 0);
         if ((int64_t)chunk >= n_chunks) break;
         const int64_t k0 = (int64_t)chunk * FCHUNK, k1 = min(k0 + FCHUNK, P.n_pairs);
+        // the chunk's list entries in one coalesced read (lane l holds entry k0 + l), and the 80-byte records of its
+        // q forests on their way into L1 while the first pairs are worked on (the chain list entry -> record ->
+        // pixel arrays was three dependent L2 round trips per forest pair)
+        int2 e_l = make_int2(0, 0);
+        if (lane < (int)(k1 - k0)) {
+            e_l = ((const int2 *)P.pq)[k0 + lane];
+            const char *hq_addr = (const char *)(P.prep.head + e_l.y);
+            asm volatile("prefetch.global.L1 [%0];" :: "l"(hq_addr));
+            asm volatile("prefetch.global.L1 [%0];" :: "l"(hq_addr + sizeof(ForestHead) - 1));
+        }
         for (int64_t k = k0; k < k1; ++k) {
-            const int2 e = ((const int2 *)P.pq)[k];
+            const int2 e = make_int2(__shfl_sync(0xffffffffu, e_l.x, (int)(k - k0)), __shfl_sync(0xffffffffu, e_l.y, (int)(k - k0)));
             const int p = e.x, q = e.y;
             if (p != head_p) { hp = P.prep.head[p]; head_p = p; }
             const ForestHead hq = P.prep.head[q];
