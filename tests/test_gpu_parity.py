@@ -208,6 +208,31 @@ def test_long_and_ragged_forests_tiles(ctx, B, orc):
     check_dmat(g, orc.dmat(f2, ref2, 0.97, 9), "long forests D")
 
 
+def test_window_search_edges(ctx, B, orc):
+    """Forests at the size limits of the fast kernels (72 px for k_xi_fast / class 0 of k_dmat_fast, 144 px for class 1)
+    and at the power-of-two lengths the branch-free window searches step through (31..33, 63..65, 127..129), with chi
+    ranges that overlap fully, partly (windows that run off either end of q) and not at all."""
+    rng = np.random.default_rng(17)
+    for lens, (smin, smax), frac in (([72, 72, 71, 65, 64, 63, 33, 32, 31, 2], (4.8, 6.9), 0.9),
+                                     ([144, 143, 129, 128, 127, 100, 65], (1.4, 2.6), 0.97)):
+        chis, ws, ds, lls = [], [], [], []
+        for k, n in enumerate(lens):
+            c0 = 3600.0 + (0.0, 30.0, 150.0, 330.0)[k % 4] + rng.uniform(0, 5)       # same start, shifted, barely overlapping, beyond
+            chis.append(c0 + np.cumsum(rng.uniform(smin, smax, n)))
+            ws.append(rng.uniform(0.5, 2.0, n)); ds.append(rng.normal(0, 0.3, n))
+            lls.append(3.55 + 1e-4 * np.arange(n) + rng.uniform(0, 1e-5, n))
+        off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+        ra = rng.uniform(0, 0.03, len(lens)); dec = rng.uniform(-0.015, 0.015, len(lens))
+        ux, uy, uz = gen.unit_vectors(ra, dec)
+        f = gen.Forests(ra, dec, ux, uy, uz, np.zeros(len(lens)), off, np.concatenate(chis), np.concatenate(ws),
+                        np.concatenate(ds), np.concatenate(lls))
+        d = B.DeviceForests(f)
+        ref = orc.pairs_brute(f)
+        pairs = ctx.lya_pairs_import(ref)
+        check_xi(ctx.lya_xi2pcf(d, B.binning(), pairs), orc.xi(f, ref), f"window edges xi {lens[0]}")
+        check_dmat(ctx.lya_dmat(d, B.binning(), pairs, frac, 5), orc.dmat(f, ref, frac, 5), f"window edges D {lens[0]}")
+
+
 def test_kernel_routes_fast_and_generic(B, orc):
     """The same catalogue through (a) the fast kernels (bucketed list, warp-private tables), (b) the
     generic kernels forced for the whole list, (c) a grid whose 8 Mpc/h r_par bins exceed the pixel
