@@ -378,7 +378,10 @@ __device__ __forceinline__ unsigned xi_key(const BinParams &bp, const PairBin &g
 // width), so an entry has one holder at a time; all releases of a row come before its acquires (warp
 // barrier in between).  The keys of row i+1 are computed between the acquire of row i and the FMAs
 // that need it.  r1 - r0 + 1 is a multiple of D; rows >= mp of p are sentinels.
-template <int D, bool POW2, bool CHECK>
+// AL2 (D == 2 only, first row even, dlo even): the new q pixels of the two rows of a loop step are neighbours at an
+// even index, so ONE 16-byte read per array serves both rows -- and unlike the 8-byte reads at a stride of two
+// pixels it has no bank conflict.
+template <int D, bool POW2, bool CHECK, bool AL2 = false>
 __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
                                         int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
                                         unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts)
@@ -391,6 +394,7 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
         double accS[D], accW[D], fa[D], fw[D];
         double wc[D], wa[D], ww[D];                         // sliding window over q
         double pa_c, pw_c;
+        double2 qc2 = make_double2(0.0, 0.0), qa2 = qc2, qw2 = qc2;   // AL2: the q pixels of rows ib + 1 and ib + 2
 #pragma unroll
         for (int k = 0; k < D; ++k) { cur[k] = garbage; cnt[k] = 0u; accS[k] = 0.0; accW[k] = 0.0; }
         {   // prologue: window and keys of row r0
@@ -423,8 +427,18 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
                 }
                 // row i + 1's new q pixel and p pixel are read BEFORE the hand-over (they do not depend on it; the
                 // volatile accesses below would otherwise pin these loads behind them)
-                const unsigned jn = min((unsigned)(i + dl + D + FPAD), (unsigned)(mq + 2 * FPAD - 1));
-                const double qcn = ws.qc[jn], qan = ws.qa[jn], qwn = ws.qw[jn], pcn = ws.pc[i + 1];
+                double qcn, qan, qwn;
+                if (AL2) {
+                    if (u == 0) {                           // (even index: 16-byte aligned; beyond either end -> two sentinels)
+                        const unsigned jc = min((unsigned)(i + dl + D + FPAD), (unsigned)((mq + 3) & ~1));
+                        qc2 = *(const double2 *)&ws.qc[jc]; qa2 = *(const double2 *)&ws.qa[jc]; qw2 = *(const double2 *)&ws.qw[jc];
+                    }
+                    qcn = u == 0 ? qc2.x : qc2.y; qan = u == 0 ? qa2.x : qa2.y; qwn = u == 0 ? qw2.x : qw2.y;
+                } else {
+                    const unsigned jn = min((unsigned)(i + dl + D + FPAD), (unsigned)(mq + 2 * FPAD - 1));
+                    qcn = ws.qc[jn]; qan = ws.qa[jn]; qwn = ws.qw[jn];
+                }
+                const double pcn = ws.pc[i + 1];
 #pragma unroll
                 for (int k = 0; k < D; ++k) {
                     ch[k] = key[k] != cur[k];
@@ -483,7 +497,10 @@ __device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsi
 #define XI_WALK_D(D_) do { const int a = i0 + ((r0 - i0) / D_) * D_, b = a + ((r1 - a) / D_ + 1) * D_ - 1; \
         xi_walk<D_, POW2, CHECK>(ws, sw_base, n_base, a, b, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts); } while (0)
     if (nd <= 32) XI_WALK_D(1);
-    else if (nd <= 64) XI_WALK_D(2);
+    else if (nd <= 64 && dhi - (dlo - (dlo & 1)) <= 63) {    // two diagonals per lane from an EVEN first diagonal (AL2);
+        const int a = i0 + ((r0 - i0) / 2) * 2, b = a + ((r1 - a) / 2 + 1) * 2 - 1;          // 64 diagonals from an odd one take D = 3
+        xi_walk<2, POW2, CHECK, true>(ws, sw_base, n_base, a, b, mq, dlo - (dlo & 1), dhi, bp, g, c0, np1, lane, evaluated, conflicts);
+    }
     else if (nd <= 96) XI_WALK_D(3);
     else XI_WALK_D(4);
 #undef XI_WALK_D
