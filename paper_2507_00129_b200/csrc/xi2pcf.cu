@@ -305,7 +305,16 @@ cudaError_t launch_xi(const XiParams &P, int grid, size_t smem, cudaStream_t s)
 }
 
 // ======================= fast kernel: warp-private sub-histograms ================================
-constexpr int FW = 14;                       // warps per block, one block per SM (16.2 KB of shared memory per warp)
+// Two size classes (template parameter CLS), as in k_dmat_fast:
+//   class 0: forests of up to LYA_FAST_TILE (72) pixels whose spacing exceeds the r_par bin width -- the BASELINE
+//            configs; 14 warps per SM (16.2 KB of shared memory per warp);
+//   class 1: forests of up to LYA_FAST_TILE2 (144) pixels, spacing down to bin width / 8 -- native-resolution shapes
+//            (NEXT-3): one diagonal per lane at a DIAGONAL STRIDE ds (the lanes of a row step sit ds pixels of q
+//            apart, so they still hold different r_par bins on each side); 11 warps per SM (19.6 KB per warp).
+template <int CLS> struct XiCfg;
+template <> struct XiCfg<0> { static constexpr int T = LYA_FAST_TILE, WARPS = 14; };
+template <> struct XiCfg<1> { static constexpr int T = LYA_FAST_TILE2, WARPS = 11; };
+constexpr int FW = XiCfg<0>::WARPS;          // (class 0 under its old names: the no-allocation entry point uses them)
 constexpr int FTHREADS = FW * 32;
 constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
 #ifndef LYA_FROWS
@@ -335,13 +344,16 @@ struct XiFastParams {
 //   side: 0 when chi_i >= chi_j, 1 otherwise (the two sides of a bin are added when the warp merges);
 //   row n_par is GARBAGE: a pixel pair outside the grid (or a sentinel pixel) maps to entry
 //   (column 0, side 0, row n_par), so the pair loop has no validity branch; the merge drops that row.
-struct __align__(16) FastWarp {
+template <int T_> struct __align__(16) FastWarpT {
+    static constexpr int T = T_, TP = ((T_ + 15) / 16) * 16 + 2;   // longest forest; p rows incl. sentinel rows
     double2 SW[FSLOTS];                      // (S, W) per slot
     unsigned N[(FSLOTS + 3) & ~3];           // (padded: the arrays below need 16-byte alignment)
-    double pc[FTP], pa[FTP], pw[FTP];        // rows >= len are sentinels (walks cover whole row groups)
-    double qc[FT + 2 * FPAD], qa[FT + 2 * FPAD], qw[FT + 2 * FPAD];
-    unsigned char jlo[FT], jhi[FT];          // per row of p: window [jlo, jhi) of q that can be in the grid
+    double pc[TP], pa[TP], pw[TP];           // rows >= len are sentinels (walks cover whole row groups)
+    double qc[T_ + 2 * FPAD], qa[T_ + 2 * FPAD], qw[T_ + 2 * FPAD];
+    unsigned char jlo[T_], jhi[T_];          // per row of p: window [jlo, jhi) of q that can be in the grid
 };
+using FastWarp = FastWarpT<FT>;
+static_assert(sizeof(FastWarpT<LYA_FAST_TILE>) * XiCfg<0>::WARPS <= 232448 && sizeof(FastWarpT<LYA_FAST_TILE2>) * XiCfg<1>::WARPS <= 232448, "k_xi_fast shared memory");
 
 // (predicated shared-memory accesses: lya_walk.cuh)
 
@@ -381,15 +393,21 @@ __device__ __forceinline__ unsigned xi_key(const BinParams &bp, const PairBin &g
 // AL2 (D == 2 only, first row even, dlo even): the new q pixels of the two rows of a loop step are neighbours at an
 // even index, so ONE 16-byte read per array serves both rows -- and unlike the 8-byte reads at a stride of two
 // pixels it has no bank conflict.
-template <int D, bool POW2, bool CHECK, bool AL2 = false>
-__device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
+// ds (D == 1 only; 1 otherwise): diagonal stride -- blocks of 32 * ds diagonals, ds passes per block (one per
+// residue), lane l on diagonal d0 + ds * l.
+template <int D, bool POW2, bool CHECK, bool AL2 = false, class WS>
+__device__ __forceinline__ void xi_walk(WS &ws, unsigned sw_base, unsigned n_base, int r0, int r1, int mq,
                                         int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
-                                        unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts)
+                                        unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts, int ds = 1)
 {
     const double *qc = ws.qc + FPAD, *qa = ws.qa + FPAD, *qw = ws.qw + FPAD;
     const unsigned garbage = (np1 - 1u) * 16u;              // entry (column 0, side 0, row n_par)
-    for (int d0 = dlo; d0 <= dhi; d0 += 32 * D) {
-        const int dl = d0 + lane * D;                       // first diagonal of this lane
+    const int step = (D == 1) ? ds : D, n_res = (D == 1) ? ds : 1;
+    const int n_pass = ((dhi - dlo) / (32 * step) + 1) * n_res;
+    for (int pass = 0; pass < n_pass; ++pass) {
+        const int d0 = dlo + (pass / n_res) * (32 * step) + pass % n_res;
+        if (d0 > dhi) continue;
+        const int dl = d0 + lane * step;                    // first diagonal of this lane
         unsigned cur[D], cnt[D], key[D];
         double accS[D], accW[D], fa[D], fw[D];
         double wc[D], wa[D], ww[D];                         // sliding window over q
@@ -486,14 +504,18 @@ __device__ __forceinline__ void xi_walk(FastWarp &ws, unsigned sw_base, unsigned
     }
 }
 
-template <bool POW2, bool CHECK>
-__device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsigned n_base, int i0, int r0, int r1, int mq,
+template <bool POW2, bool CHECK, class WS>
+__device__ __forceinline__ void xi_walk_any(WS &ws, unsigned sw_base, unsigned n_base, int i0, int r0, int r1, int mq,
                                             int dlo, int dhi, const BinParams &bp, const PairBin &g, unsigned c0,
-                                            unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts)
+                                            unsigned np1, int lane, unsigned long long &evaluated, unsigned &conflicts, int ds)
 {
     // D diagonals per lane, the smallest that covers the group in one pass; the rows [r0, r1] (inside one group of
     // FROWS rows, i0 its first) are widened to a multiple of D rows aligned to the group
     const int nd = dhi - dlo + 1;
+    if (ds > 1) {                                            // pixels finer than the bins: one diagonal per lane, ds apart
+        xi_walk<1, POW2, CHECK>(ws, sw_base, n_base, r0, r1, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts, ds);
+        return;
+    }
 #define XI_WALK_D(D_) do { const int a = i0 + ((r0 - i0) / D_) * D_, b = a + ((r1 - a) / D_ + 1) * D_ - 1; \
         xi_walk<D_, POW2, CHECK>(ws, sw_base, n_base, a, b, mq, dlo, dhi, bp, g, c0, np1, lane, evaluated, conflicts); } while (0)
     if (nd <= 32) XI_WALK_D(1);
@@ -507,7 +529,8 @@ __device__ __forceinline__ void xi_walk_any(FastWarp &ws, unsigned sw_base, unsi
 }
 
 // merge a warp's sub-histogram (first column c0) into the global accumulators and clear it
-__device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, int c0, int reg, int lane)
+template <class WS>
+__device__ __forceinline__ void xi_merge(WS &ws, const XiFastParams &P, int c0, int reg, int lane)
 {
     const size_t roff = (size_t)reg * (size_t)(P.bp.n_par * P.bp.n_perp);   // accumulators of sub-sample reg
     const int np1 = P.bp.n_par + 1;
@@ -531,12 +554,14 @@ __device__ __forceinline__ void xi_merge(FastWarp &ws, const XiFastParams &P, in
     __syncwarp();
 }
 
-template <bool POW2, bool CHECK>
-__global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
+template <bool POW2, bool CHECK, int CLS = 0>
+__global__ void __launch_bounds__(XiCfg<CLS>::WARPS * 32, 1) k_xi_fast(XiFastParams P)
 {
+    using WS = FastWarpT<XiCfg<CLS>::T>;
+    constexpr int FTP = WS::TP;                                // (shadows the class-0 constant)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    FastWarp &ws = ((FastWarp *)smem_raw)[wid];
+    WS &ws = ((WS *)smem_raw)[wid];
     const BinParams bp = P.bp;
     const unsigned np1 = (unsigned)bp.n_par + 1u;
     for (int t = lane; t < FSLOTS; t += 32) { ws.SW[t] = make_double2(0.0, 0.0); ws.N[t] = 0u; }
@@ -578,7 +603,8 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
             const PairBin g = lya_make_pairbin(bp, s, c);
             int c0;
             const int key = lya_pair_key<POW2>(bp, g, hp, hq, c0);
-            if (key >= bp.n_perp) continue;                  // cannot happen in the fast range
+            if (key >= (CLS + 1) * bp.n_perp || key < CLS * bp.n_perp) continue;     // cannot happen in this class's range
+            const int ds = (CLS == 0) ? 1 : lya_pair_stride(bp, g, hq);                // lanes of a row step sit ds pixels of q apart
             since_merge += (unsigned long long)mp * mq;
             const int reg = P.region ? P.region[p] : 0;       // a pixel pair belongs to the sub-sample of forest p
             if (c0 != win_c0 || reg != win_reg || since_merge > P.merge_every) {
@@ -623,7 +649,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
                 const double ta0 = x0 - R, ta1 = x1 - R, tb0 = fmin(x0 + R, Tchi - x0), tb1 = fmin(x1 + R, Tchi - x1);
                 int a0 = 0, b0 = 0, a1 = 0, b1 = 0;          // first j with qc[j] > ta / qc[j] >= tb
 #pragma unroll
-                for (int st = 64; st > 0; st >>= 1) {
+                for (int st = (WS::T < 128 ? 64 : 128); st > 0; st >>= 1) {
                     const double va0 = qc[min(a0 + st - 1, mq)], vb0 = qc[min(b0 + st - 1, mq)];
                     const double va1 = qc[min(a1 + st - 1, mq)], vb1 = qc[min(b1 + st - 1, mq)];
                     a0 += (va0 > ta0) ? 0 : st; b0 += (vb0 >= tb0) ? 0 : st;
@@ -643,7 +669,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) k_xi_fast(XiFastParams P)
                 }
                 dlo = __reduce_min_sync(0xffffffffu, dlo); dhi = __reduce_max_sync(0xffffffffu, dhi);
                 r0 = __reduce_min_sync(0xffffffffu, r0); r1 = __reduce_max_sync(0xffffffffu, r1);
-                if (r1 >= r0) xi_walk_any<POW2, CHECK>(ws, sw_base, n_base, i0, r0, r1, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated, conflicts);
+                if (r1 >= r0) xi_walk_any<POW2, CHECK>(ws, sw_base, n_base, i0, r0, r1, mq, dlo, dhi, bp, g, (unsigned)c0, np1, lane, evaluated, conflicts, ds);
             }
         }
     }
@@ -707,31 +733,43 @@ static lya_status xi_run(lya_ctx *ctx, const lya_plan *pl, const int32_t *region
     XiParams P;
     P.pix_off = f->pix_off; P.chi = f->chi; P.w = f->w; P.delta = f->delta;
     P.ux = f->ux; P.uy = f->uy; P.uz = f->uz;
-    P.pq = use_fast ? bk.pq + 2 * bk.n_fast : pl->pq;
-    P.n_pairs = use_fast ? bk.n_fast2 + bk.n_long + bk.n_generic : pl->n_pairs;     // (class-1 and long pairs take the generic xi kernel)
+    P.pq = use_fast ? bk.pq + 2 * (bk.n_fast + bk.n_fast2) : pl->pq;
+    P.n_pairs = use_fast ? bk.n_long + bk.n_generic : pl->n_pairs;     // (long pairs take the generic xi kernel)
     P.n_forest = f->n_forest;
     P.bp = bp;
     P.S = acc; P.W = acc + nbt; P.N = (unsigned long long *)(acc + 2 * nbt);
     P.counters = ctx->d_counters;
 
     cudaEventRecord(ctx->ev[0], s);
-    if (use_fast && bk.n_fast > 0) {
+    if (use_fast && bk.n_fast + bk.n_fast2 > 0) {
         XiFastParams F;
         F.prep = pl->prep; F.pq = bk.pq; F.n_pairs = bk.n_fast; F.bp = bp;
         F.S = P.S; F.W = P.W; F.N = P.N; F.counters = ctx->d_counters;
         F.region = region; F.n_region = n_reg;
         F.merge_every = ctx->xi_merge_every;
-        const size_t fsmem = sizeof(FastWarp) * FW;
         const int fgrid = ctx->sm_count;
-        auto launch = [&](auto kern) {
+        auto launch = [&](auto kern, size_t fsmem, int threads) {
             cudaError_t le = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem);
-            if (le == cudaSuccess) { kern<<<fgrid, FTHREADS, fsmem, s>>>(F); lya_note_launch(); }
+            if (le == cudaSuccess) { kern<<<fgrid, threads, fsmem, s>>>(F); lya_note_launch(); }
             return le;
         };
-        if (ctx->check_holders) e = bp.pow2 ? launch(k_xi_fast<true, true>) : launch(k_xi_fast<false, true>);
-        else e = bp.pow2 ? launch(k_xi_fast<true, false>) : launch(k_xi_fast<false, false>);
-        if (e == cudaSuccess) e = cudaGetLastError();
-        if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_fast launch"); }
+        if (bk.n_fast > 0) {                                   // class 0
+            const size_t fsmem = sizeof(FastWarp) * FW;
+            if (ctx->check_holders) e = bp.pow2 ? launch(k_xi_fast<true, true, 0>, fsmem, FTHREADS) : launch(k_xi_fast<false, true, 0>, fsmem, FTHREADS);
+            else e = bp.pow2 ? launch(k_xi_fast<true, false, 0>, fsmem, FTHREADS) : launch(k_xi_fast<false, false, 0>, fsmem, FTHREADS);
+            if (e == cudaSuccess) e = cudaGetLastError();
+            if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_fast launch"); }
+        }
+        if (bk.n_fast2 > 0) {                                  // class 1: its own range of the bucketed list, its own chunk counter
+            F.pq = bk.pq + 2 * bk.n_fast; F.n_pairs = bk.n_fast2;
+            cudaMemsetAsync(ctx->d_counters + 4, 0, sizeof(unsigned long long), s);
+            const size_t fsmem = sizeof(FastWarpT<XiCfg<1>::T>) * XiCfg<1>::WARPS;
+            const int threads = XiCfg<1>::WARPS * 32;
+            if (ctx->check_holders) e = bp.pow2 ? launch(k_xi_fast<true, true, 1>, fsmem, threads) : launch(k_xi_fast<false, true, 1>, fsmem, threads);
+            else e = bp.pow2 ? launch(k_xi_fast<true, false, 1>, fsmem, threads) : launch(k_xi_fast<false, false, 1>, fsmem, threads);
+            if (e == cudaSuccess) e = cudaGetLastError();
+            if (e != cudaSuccess) { cleanup(); return lya_cuda_fail(ctx, e, "k_xi_fast (class 1) launch"); }
+        }
     }
     const size_t smem = (((size_t)nb * 20 + 15) & ~(size_t)15) + sizeof(WarpSmem) * XI_WARPS;
     const int grid = ctx->sm_count * 2;
