@@ -162,7 +162,10 @@ void       lya_pairs_free(lya_ctx *ctx, lya_pairs *pairs);
 /* S, W: double [n_par*n_perp]; N: uint64 [n_par*n_perp]; xi: double [n_par*n_perp]
  * (xi_A = S_A / W_A, 0 where W_A == 0); row-major [b_par][b_perp].  Any of S, W,
  * N, xi may be NULL.  Each unordered pixel pair of each listed forest pair counts
- * once.  stats: host out, may be NULL.  The call synchronises the ctx stream either way. */
+ * once.  stats: host out, may be NULL.  The call synchronises the ctx stream either way.
+ * Kernel routes (results do not depend on them): forests of up to 72 pixels whose spacing exceeds the r_par bin
+ * width take the atomic-free fast kernel, forests of up to 144 pixels with a spacing down to an eighth of the bin
+ * width its second size class, everything else a generic kernel with shared-memory atomics. */
 lya_status lya_xi2pcf(lya_ctx *ctx, const lya_forests *f, const lya_binning *b,
                       const lya_pairs *pairs,
                       double *S, double *W, uint64_t *N, double *xi, lya_stats *stats);
