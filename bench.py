@@ -432,6 +432,11 @@ def main():
                    "unit": "Tops/s (fp64 lane-operations)", "frac": alg_xi / t_xi / peak_alu, "traffic": None,
                    "peak_source": peak_src, "frac_at_sampled_clock": alg_xi / t_xi / (ctx.sm_count() * FP64_LANES_PER_SM * sm_clk),
                    "evaluated_per_binned": sx["n_evaluated"] / max(sx["n_binned"], 1)}
+        # DRAM bytes per launch, measured ONCE under ncu on this workload (profiles/r2p_dram_cfg4_full.md); null elsewhere
+        full_cfg4 = args.workload == "cfg4" and not args.forests and args.fine == 1 and not args.force_generic and world == 1
+        if full_cfg4:
+            roof_xi["traffic"] = 150.64e9 + 0.09e9
+            roof_xi["traffic_note"] = "dram__bytes_read + write of one k_xi_fast launch, ncu capture profiles/r2p_dram_cfg4_full.md (37 GB/s: not HBM-bound)"
         roof = roof_xi
         extra = {"xi": {"binned_pairs_per_s": sx["n_binned"] / t_xi, "visited_pairs_per_s": sx["n_visited"] / t_xi,
                         "evaluated_pairs_per_s": sx["n_evaluated"] / t_xi, "ms": t_xi * 1e3,
@@ -447,6 +452,9 @@ def main():
                       "evaluated_per_scanned": sd["n_evaluated"] / max(sd["n_binned"], 1)}
             extra["dmat"] = {"scanned_pairs_per_s": sd["n_binned"] / t_dm, "kept_pairs_per_s": sd["n_kept"] / t_dm,
                              "ms": t_dm * 1e3, "n_kept": sd["n_kept"], "n_scatter": sd["n_scatter"], "roofline": roof_d}
+            if full_cfg4:
+                roof_d["traffic"] = 232.23e9 + 0.28e9
+                roof_d["traffic_note"] = "dram__bytes_read + write of one k_dmat_fast launch, ncu capture profiles/r2p_dram_cfg4_full.md (15 GB/s: not HBM-bound)"
             if t_dm > t_xi:
                 roof = roof_d
         if world == 1:
