@@ -414,6 +414,30 @@ def test_region_subsamples_next1(ctx, B, orc):
         ctx.lya_xi2pcf_sub(d, B.binning(), pairs, region + 3, n_region)
 
 
+def test_region_subsamples_native_resolution(ctx, B, orc):
+    """NEXT-1 on NEXT-3 shapes: per-region S, W, N of a fine-spacing catalogue (second size class of k_xi_fast, with the
+    warp-private sub-histograms merged per region) against the oracle, and adding up to lya_xi2pcf."""
+    f = gen.make_config(2, n_forest=160, fine=2)
+    d = B.DeviceForests(f)
+    rng = np.random.default_rng(6)
+    n_region = 3
+    region = rng.integers(0, n_region, f.n_forest).astype(np.int32)
+    b, ob = B.binning(), orc.binning()
+    pairs = ctx.lya_neighbours(d, b)
+    pq = pairs.export().cpu().numpy()
+    g = ctx.lya_xi2pcf_sub(d, b, pairs, region, n_region)
+    full = ctx.lya_xi2pcf(d, b, pairs)
+    want = orc.xi_sub(f, pq, region, n_region, ob)
+    N = g["N"].cpu().numpy().view(np.uint64); S = g["S"].cpu().numpy(); W = g["W"].cpu().numpy()
+    for r in range(n_region):
+        o = want[r]
+        assert np.array_equal(N[r], o["N"]), f"region {r}"
+        assert np.all(np.abs(W[r] - o["W"]) <= 1e-9 * o["W"])
+        assert np.all(np.abs(S[r] - o["S"]) <= 1e-9 * np.maximum(np.abs(o["S"]), 1e-4 * o["Sabs"]))
+    assert np.array_equal(N.sum(0), full["N"].cpu().numpy().view(np.uint64))
+    check_xi(full, orc.xi(f, pq), "fine-spacing xi")
+
+
 def test_sharded_halves_sum_to_full(ctx, B, orc):
     """SURVEY 8(e) on one device: the two chunks of shard.split_pairs, run separately and summed,
     equal the un-split run (N, n_kept exactly) and, after lya_xi_normalise / lya_dmat_normalise,
