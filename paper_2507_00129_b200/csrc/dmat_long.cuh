@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(DL_THREADS, 1) k_dmat_long(DmFastParams P)
         const double Tchi = (s > 0.0) ? (bp.rperp_max / s) * (1.0 + 1e-12) + 1e-9 : 1e300;
         for (int i = tid; i < mp; i += DL_THREADS) {
             int jlo, jx, jhi;
-            lya_row_window<POW2>(bp, g, qce, mq, sh.pce[i].x, R, Tchi, jlo, jx, jhi);
+            lya_row_window_ilp<POW2, DL_T>(bp, g, qce, mq, sh.pce[i].x, R, Tchi, jlo, jx, jhi);
             sh.jlo[i] = (unsigned short)jlo; sh.jx[i] = (unsigned short)jx; sh.jhi[i] = (unsigned short)jhi;
             binned_total += (unsigned)(jhi - jlo);
         }

@@ -78,29 +78,11 @@ __device__ __forceinline__ bool lya_in_grid(const BinParams &bp, const PairBin &
 // EXACT window of row x = chi_i against the increasing chi of q (shared memory, mq pixels):
 // [jlo, jhi) = the q pixels whose pair with i is inside the grid, jx = first j with chi_j > chi_i
 // (clamped into [jlo, jhi]).  The in-grid set of a row is contiguous: r_perp grows with j, r_par
-// falls towards chi_j = chi_i and grows after it, and every rounded operation is monotone.  Two
-// binary searches give a conservative superset (margins R, Tchi); the ends are then moved with the
-// exact bin test, so that callers can take "j in [jlo, jhi)" for "in the grid" without redoing geometry.
-template <bool POW2>
-__device__ __forceinline__ void lya_row_window(const BinParams &bp, const PairBin &g, const double2 *qce, int mq,
-                                               double x, double R, double Tchi, int &jlo, int &jx, int &jhi)
-{
-    int lo = 0, hi = mq;                         // first j with chi_j > x - R
-    while (lo < hi) { const int mid = (lo + hi) >> 1; if (qce[mid].x > x - R) hi = mid; else lo = mid + 1; }
-    jlo = lo;
-    const double top = fmin(x + R, Tchi - x);    // first j with chi_j >= top
-    hi = mq;
-    while (lo < hi) { const int mid = (lo + hi) >> 1; if (qce[mid].x >= top) hi = mid; else lo = mid + 1; }
-    jhi = lo;
-    while (jlo < jhi && !lya_in_grid<POW2>(bp, g, x, qce[jlo].x)) ++jlo;
-    while (jhi > jlo && !lya_in_grid<POW2>(bp, g, x, qce[jhi - 1].x)) --jhi;
-    lo = jlo; hi = jhi;                          // first j with chi_j > x
-    while (lo < hi) { const int mid = (lo + hi) >> 1; if (qce[mid].x > x) hi = mid; else lo = mid + 1; }
-    jx = lo;
-}
-
-// The same window with the three searches as ONE branch-free loop of fixed trip count (three independent
-// dependency chains in flight instead of three data-dependent loops one after the other).  STEP0: a power of two
+// falls towards chi_j = chi_i and grows after it, and every rounded operation is monotone.  Lower-bound
+// searches give a conservative superset (margins R, Tchi); the ends are then moved with the exact bin
+// test, so that callers can take "j in [jlo, jhi)" for "in the grid" without redoing geometry.
+// The three searches run as ONE branch-free loop of fixed trip count (three independent dependency chains in
+// flight; as three data-dependent binary searches one after the other they were pure latency).  STEP0: a power of two
 // with 2 * STEP0 > the longest q; qce[mq] must be a sentinel (chi far above every real pixel).
 template <bool POW2, int STEP0>
 __device__ __forceinline__ void lya_row_window_ilp(const BinParams &bp, const PairBin &g, const double2 *qce, int mq,
