@@ -23,7 +23,7 @@ namespace {
 // Two size classes of the same kernel (template parameter CLS):
 //   class 0: forests of up to LYA_FAST_TILE (72) pixels -- the BASELINE configs; 15 warps per SM;
 //   class 1: forests of up to LYA_FAST_TILE2 (144) pixels -- native-resolution shapes (DESIGN.md NEXT-3): longer
-//            staging tiles and kept-pair queue, 10 warps per SM.
+//            staging tiles and kept-pair queue, 11 warps per SM (what its 20.5 KB per warp allow).
 // In both, pass A takes a DIAGONAL STRIDE ds: a pass covers the diagonals d0 + ds * lane, so the lanes of a row
 // step sit ds pixels of q apart; ds is the smallest integer with ds * (q's pixel spacing) > r_par bin width, which
 // keeps "one holder per table entry" true when the pixels are finer than the bins (ds passes, one per residue,
@@ -32,7 +32,7 @@ namespace {
 #define LYA_FD_WARPS 15
 #endif
 #ifndef LYA_FD_WARPS2
-#define LYA_FD_WARPS2 10
+#define LYA_FD_WARPS2 11
 #endif
 template <int CLS> struct DmCfg;
 template <> struct DmCfg<0> { static constexpr int T = LYA_FAST_TILE, WARPS = LYA_FD_WARPS, KCAP = 48; };
