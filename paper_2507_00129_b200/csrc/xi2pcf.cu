@@ -318,7 +318,7 @@ constexpr int FW = XiCfg<0>::WARPS;          // (class 0 under its old names: th
 constexpr int FTHREADS = FW * 32;
 constexpr int FT = LYA_FAST_TILE;            // longest forest (pixels)
 #ifndef LYA_FROWS
-#define LYA_FROWS 12
+#define LYA_FROWS 24
 #endif
 constexpr int FROWS = LYA_FROWS;             // rows of p walked per pass (keeps lanes busy: DESIGN.md)
 static_assert(FROWS % 12 == 0 && FROWS <= 32, "a row group holds whole blocks of 1, 2, 3 or 4 rows");
